@@ -1,0 +1,180 @@
+/*
+ * kairos.h -- C ABI of libkairos.so: the decode-node mixed attention step that KAIROS creates when it
+ * deflects a prefill (arxiv 2607.02043), B200 / sm_100a only.
+ *
+ * What the step is (section 3.2 methodology; section 5.4): one batch
+ * holding B in-flight decodes (one query token each over its own K cached tokens) plus the tokens of one
+ * prefill chunk of a deflected request (causal over its already-cached prefix plus the chunk).  "The KV
+ * cache is built directly on the decode node", i.e. the chunk's keys are appended to
+ * the node's paged cache and read from it.  Per-step latency as a function of (decode batch, cached
+ * tokens, chunk size) is the input of the TBT-safety check and chunk-schedule sweep (PAPER.md:253-269,
+ * Eq. 4-6; profiled once per model/hardware).
+ *
+ * The paper leaves the attention kernel unmodified and unspecified; shapes and arithmetic
+ * are fixed by BASELINE.json north_star / configs[0] and restated in SURVEY.md 8(c):
+ *   absorbed MLA, 16 heads; each cached token = 512-d latent c_t + 64-d RoPE key kR_t shared by all heads;
+ *   query row (token j, head h) = [qC (512) | qR (64)];  s_t = scale * (qC.c_t + qR.kR_t);
+ *   p = softmax over the visible positions;  o = sum_t p_t c_t (512-d);  lse = ln sum_t exp(s_t).
+ *   decode i sees positions 0..L_i-1 (its newest token already appended); chunk row j sees 0..P+j.
+ *   bf16 inputs, fp32 accumulation, bf16 outputs, fp32 lse.
+ *
+ * Memory layout (part of the contract; the append check compares raw pool bytes):
+ *   pool       device bf16 [num_pages][64][576]; token slot = pool + ((page*64 + slot)*576)*2 bytes,
+ *              512 latent values then 64 RoPE-key values.  Must be 128-byte aligned.
+ *   page table int32, entry b = physical page of tokens 64b .. 64b+63 of that sequence.
+ *   q          bf16 [n][16][576], row = [latent part 512 | rope part 64], 16-byte aligned.
+ *   out        bf16 [n][16][512]; lse fp32 [n][16].
+ *
+ * Ownership: the caller owns every buffer it passes (pool, workspace, q, out, page tables) and the CUDA
+ * stream; the context owns only its descriptors, a small pinned staging area and its plan buffers.  No
+ * pointer is retained past the call that received it, except `pool` / `workspace` given at create time.
+ *
+ * Asynchrony: kairos_append_latent and kairos_mixed_step enqueue on `cuda_stream` (a cudaStream_t cast to
+ * void*; NULL = legacy default stream) and return without synchronising.  Host arrays (dec_ctx_lens) are
+ * read before the call returns.  Calls on one context must be issued from one thread at a time and on
+ * one stream at a time (the plan buffers are reused per call, ordered by that stream).
+ *
+ * Errors: every call returns 0 (KAIROS_OK) or a negative kairos_status.  Argument errors are detected on
+ * the host before anything is enqueued.  Page ids are trusted (not range-checked on the device).
+ * kairos_last_error gives a human-readable message for the last failure on this thread.
+ * There is no CPU fallback anywhere: without a CUDA device every compute entry returns KAIROS_ERR_CUDA.
+ */
+#ifndef KAIROS_H_
+#define KAIROS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    KAIROS_OK = 0,
+    KAIROS_ERR_INVALID_ARG = -1,
+    KAIROS_ERR_UNSUPPORTED = -2, /* dims other than 16 / 512 / 64 / page 64, or not an sm_100 device */
+    KAIROS_ERR_WORKSPACE = -3,   /* workspace too small for this call: see kairos_workspace_bytes */
+    KAIROS_ERR_CUDA = -4         /* a CUDA runtime / driver call failed (message has the CUDA string) */
+} kairos_status;
+
+typedef struct kairos_ctx kairos_ctx; /* opaque, owned by the library */
+
+typedef struct {
+    int32_t num_heads;     /* must be 16  */
+    int32_t latent_dim;    /* must be 512 */
+    int32_t rope_dim;      /* must be 64  */
+    int32_t page_size;     /* must be 64  */
+    float softmax_scale;   /* 1/sqrt(192) for DeepSeek-V2-Lite; any finite > 0 accepted */
+    void* pool;            /* DEVICE bf16 [num_pages][64][576], caller-owned, 128-B aligned */
+    int32_t num_pages;     /* >= 1 */
+    void* workspace;       /* DEVICE scratch, caller-owned, 256-B aligned; split-KV partials live here */
+    size_t workspace_bytes;
+    int32_t device;        /* CUDA device ordinal the buffers live on */
+} kairos_config;
+
+/* Bytes of device workspace that are always enough for a step with <= max_decodes decodes and a chunk of
+ * <= max_chunk tokens (host-only arithmetic, no CUDA call). */
+size_t kairos_workspace_bytes(int32_t max_decodes, int32_t max_chunk);
+
+/* Validates the config, builds the TMA descriptor of the pool, allocates plan/staging buffers.
+ * *out is set only on success.  HOST pointers: cfg, out. */
+int kairos_create(const kairos_config* cfg, kairos_ctx** out);
+int kairos_destroy(kairos_ctx* ctx); /* NULL is a no-op */
+
+/*
+ * a1 -- paged latent-cache append ("the cache is built directly on the decode node").
+ * Copies latent[j][0:512] | k_rope[j][0:64] to the slot of position start_pos + j, j < n_tokens, of the
+ * sequence whose page table is `page_table`.  Bit-exact byte copy, 16-byte vector stores.
+ *   latent      DEVICE bf16 [n_tokens][512], 16-B aligned     k_rope  DEVICE bf16 [n_tokens][64], 16-B aligned
+ *   page_table  DEVICE int32 [table_len]
+ * Errors: INVALID_ARG if n_tokens < 0, start_pos < 0, a pointer is NULL with n_tokens > 0, or
+ * start_pos + n_tokens > table_len*64.  n_tokens == 0 is a successful no-op.
+ */
+int kairos_append_latent(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens,
+                         const int32_t* page_table, int32_t table_len, int32_t start_pos, void* cuda_stream);
+
+/*
+ * Batched single-token append for the decodes of a step: request i writes one token at position
+ * positions[i] through row i of page_tables.
+ *   latent DEVICE bf16 [n][512]; k_rope DEVICE bf16 [n][64]; page_tables DEVICE int32 [n][table_stride];
+ *   positions DEVICE int32 [n], each in [0, table_stride*64).  (positions are trusted: device-side only.)
+ */
+int kairos_append_decode_tokens(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n,
+                                const int32_t* page_tables, int32_t table_stride, const int32_t* positions,
+                                void* cuda_stream);
+
+/* Test/inspection export: walks `page_table` and copies positions 0..n_tokens-1 out, bit-exact.
+ *   out DEVICE bf16 [n_tokens][576].  Errors as for append (n_tokens > table_len*64 -> INVALID_ARG). */
+int kairos_gather_latent(kairos_ctx* ctx, const int32_t* page_table, int32_t table_len, int32_t n_tokens,
+                         void* out, void* cuda_stream);
+
+/*
+ * The mixed step: n_dec decode queries plus one causal prefill chunk, one launch sequence.
+ *   q_dec            DEVICE bf16 [n_dec][16][576]
+ *   dec_page_tables  DEVICE int32 [n_dec][dec_table_stride]
+ *   dec_ctx_lens     HOST   int32 [n_dec], each >= 1 and <= dec_table_stride*64 (attended length L_i)
+ *   chunk_len        C >= 0 prefill tokens in this step; prefix_len P >= 0 tokens of the same request
+ *                    already cached; the chunk's own C tokens must have been appended at positions
+ *                    P..P+C-1 earlier on the same stream
+ *   q_chunk          DEVICE bf16 [C][16][576]
+ *   chunk_page_table DEVICE int32 [chunk_table_len], chunk_table_len*64 >= P + C
+ *   out_dec          DEVICE bf16 [n_dec][16][512]     out_chunk DEVICE bf16 [C][16][512]
+ *   lse_dec          DEVICE fp32 [n_dec][16] or NULL  lse_chunk DEVICE fp32 [C][16] or NULL
+ * n_dec == 0 and chunk_len == 0 together are a successful no-op.  Exactly one chunk per step (the
+ * dispatcher sends a decode node one deflected request at a time).
+ * Errors: INVALID_ARG (negative sizes, NULL where data is needed, ctx_len < 1 or beyond its table,
+ * chunk table too short), WORKSPACE (workspace smaller than this step's split-KV partials need).
+ */
+int kairos_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                      int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len,
+                      const void* q_chunk, const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec,
+                      void* out_chunk, float* lse_dec, float* lse_chunk, void* cuda_stream);
+
+/*
+ * The same step driven from HOST buffers (end-to-end leg): copies q_dec, q_chunk, the page tables and the
+ * chunk's new latent / k_rope host->device (pinned or pageable host memory), appends the chunk at
+ * prefix_len, runs the mixed step, copies out_dec / out_chunk (and lse if non-NULL) device->host, and
+ * synchronises the stream before returning.  All pointers are HOST pointers with the shapes of
+ * kairos_mixed_step / kairos_append_latent; device staging comes from the context (grown on demand).
+ * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied each way.
+ */
+int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                           int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len,
+                           int32_t prefix_len, const void* q_chunk, const void* chunk_latent, const void* chunk_k_rope,
+                           const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk,
+                           float* lse_dec, float* lse_chunk, uint64_t* h2d_bytes, uint64_t* d2h_bytes,
+                           void* cuda_stream);
+
+/*
+ * a11 -- per-step latency table over a (decode batch B, per-decode context K, chunk size C) grid: the
+ * deployment-time profiling of PAPER.md:302-304 for this one layer's attention, the input of Eq. 4-6
+ * (PAPER.md:253-269).  For every (B, K, C): synthetic page tables over the context's pool (B*ceil(K/64) +
+ * ceil((prefix_len+C)/64) distinct pages, strided through the pool), `warmup` untimed steps, then `reps`
+ * timed steps (CUDA events around kairos_mixed_step on `cuda_stream`; when flush_l2 != 0 a buffer larger
+ * than L2 is rewritten before every timed step, outside the timed interval).  Synchronising call.
+ *   Bs, Ks, Cs         HOST int32 arrays (B >= 0, K >= 1, C >= 0; B == 0 and C == 0 together give 0 us)
+ *   out_median_us      HOST double [nB*nK*nC], index (iB*nK + iK)*nC + iC
+ *   out_min_us         HOST double [nB*nK*nC] or NULL
+ * Units: K is PER-DECODE context (the paper's K_n is total occupancy = B*K); C is prefill tokens only (the
+ * paper's chi counts B + C); entries are one layer's attention in microseconds (SURVEY.md 8(b) units note).
+ * Errors: INVALID_ARG; WORKSPACE if the pool has too few pages or the workspace is too small for a point.
+ */
+int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int32_t nB, const int32_t* Ks, int32_t nK,
+                              const int32_t* Cs, int32_t nC, int32_t prefix_len, int32_t warmup, int32_t reps,
+                              int32_t flush_l2, double* out_median_us, double* out_min_us, void* cuda_stream);
+
+/* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
+ * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched
+ * by that call, [5] = workspace bytes used.  n = number of int64 slots available in info. */
+int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
+
+/* Message for the last failing call on this thread ("" if none). Never NULL. */
+const char* kairos_last_error(void);
+
+/* Library build tag, e.g. "kairos-b200 sm_100a <kernel generation>". Never NULL. */
+const char* kairos_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KAIROS_H_ */

@@ -1,0 +1,136 @@
+// Internal declarations shared by the translation units of libkairos.so (never installed).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "kairos.h"
+
+namespace kairos {
+
+constexpr int kHeads = 16;
+constexpr int kLatent = 512;
+constexpr int kRope = 64;
+constexpr int kDim = 576;             // latent | rope
+constexpr int kPage = 64;
+constexpr int kTokenBytes = kDim * 2; // 1152
+
+// ---- error plumbing -------------------------------------------------------------------------------
+void set_error(const std::string& msg);
+int fail(int code, const std::string& msg);
+#define KAIROS_CUDA_TRY(expr)                                                                            \
+    do {                                                                                                 \
+        cudaError_t _e = (expr);                                                                         \
+        if (_e != cudaSuccess)                                                                           \
+            return ::kairos::fail(KAIROS_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e));  \
+    } while (0)
+
+// ---- work items: what one CTA pass of the attention kernel processes ---------------------------------
+// kind 0 = decode split (1 query token x 16 heads over pages [page_begin, page_end) of its sequence),
+// kind 1 = chunk tile (kChunkTokens query tokens x 16 heads over pages [0, page_end), causal).
+struct WorkItem {
+    int32_t kind;        // 0 decode split, 1 chunk tile
+    int32_t q_index;     // decode: request index; chunk: first query token of the tile
+    int32_t page_begin;  // first logical page of the KV range
+    int32_t page_end;    // one past the last logical page
+    int32_t n_keys;      // decode: L_i; chunk: P + q_index + 1 (keys visible to the tile's first token)
+    int32_t n_q;         // query tokens in this item (decode 1; chunk <= kChunkTokens, ragged tail)
+    int32_t partial_slot; // >= 0: write unnormalised partial (o, m, l) to this workspace slot; -1: final output
+    int32_t cost;        // planner's cost estimate (pages-equivalents), used for ordering only
+};
+static_assert(sizeof(WorkItem) == 32, "WorkItem is copied to the device as raw bytes");
+
+// One entry per decode request that was split: the combine pass merges n_splits partial slots.
+struct CombineItem {
+    int32_t q_index;      // output token: decode request index, or chunk token index
+    int32_t first_slot;   // first partial slot of this token
+    int32_t n_splits;
+    int32_t kind_stride;  // bits 0..7: 0 decode / 1 chunk output; bits 8..: slot stride between splits
+};
+
+struct Plan {
+    std::vector<WorkItem> items;       // execution order (longest first)
+    std::vector<CombineItem> combines;
+    int32_t n_decode_items = 0;
+    int32_t n_chunk_items = 0;
+    int32_t n_partial_slots = 0;
+};
+
+// Host planner (a0): pure integer code, no CUDA.  `target_ctas` = resident CTAs the launch will have.
+// chunk_tile_tokens = query tokens per chunk tile.  See plan.cpp.
+void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len,
+                int32_t target_ctas, int32_t chunk_tile_tokens, Plan* plan);
+
+constexpr size_t kPartialSlotBytes = size_t(kHeads) * kLatent * 4 + size_t(kHeads) * 2 * 4;  // o[16][512] f32 + (m,l)[16]
+
+// ---- context ---------------------------------------------------------------------------------------
+struct StagingSlot {
+    void* host = nullptr;    // pinned
+    void* dev = nullptr;
+    size_t bytes = 0;
+    cudaEvent_t done = nullptr;  // recorded after the H2D copy out of `host`
+    bool used = false;
+};
+
+struct HostStage {  // device staging for kairos_mixed_step_host
+    void* dev = nullptr;
+    size_t bytes = 0;
+};
+
+}  // namespace kairos
+
+struct kairos_ctx {
+    kairos_config cfg;
+    int sm_count = 0;
+    int impl = 1;                 // 0 = simple CUDA-core kernel (debug cross-check), 1 = tcgen05 path
+    CUtensorMap pool_map;         // TMA descriptor of the pool (filled when impl needs it)
+    bool has_pool_map = false;
+    static constexpr int kStagingSlots = 4;
+    kairos::StagingSlot staging[kStagingSlots];
+    int staging_next = 0;
+    kairos::HostStage host_stage;
+    kairos::Plan plan;            // reused per call
+    int64_t last_info[6] = {0, 0, 0, 0, 0, 0};
+};
+
+namespace kairos {
+
+// Acquire a pinned+device staging pair of at least `bytes` (waits for the slot's previous copy).
+int staging_acquire(kairos_ctx* ctx, size_t bytes, StagingSlot** out);
+
+// ---- kernel launchers (each returns a kairos_status) -----------------------------------------------
+int launch_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
+                  int32_t start_pos, cudaStream_t stream);
+int launch_append_decode(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                         int32_t table_stride, const int32_t* positions, cudaStream_t stream);
+int launch_gather(kairos_ctx* ctx, const int32_t* page_table, int32_t n_tokens, void* out, cudaStream_t stream);
+
+struct StepArgs {
+    int32_t n_dec;
+    const void* q_dec;
+    const int32_t* dec_page_tables;
+    int32_t dec_table_stride;
+    int32_t chunk_len, prefix_len;
+    const void* q_chunk;
+    const int32_t* chunk_page_table;
+    void* out_dec;
+    void* out_chunk;
+    float* lse_dec;
+    float* lse_chunk;
+};
+
+// impl 0: one CTA per query token on CUDA cores (attn_simple.cu). dev_lens = device copy of dec_ctx_lens.
+int launch_attn_simple(kairos_ctx* ctx, const StepArgs& a, const int32_t* dev_lens, cudaStream_t stream);
+
+// impl 1: persistent tcgen05/TMA kernel over the plan's work items + LSE combine (attn_umma.cu).
+int umma_chunk_tile_tokens();
+int umma_resident_ctas(const kairos_ctx* ctx);
+int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
+                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched);
+int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
+
+}  // namespace kairos

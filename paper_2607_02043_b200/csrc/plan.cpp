@@ -1,0 +1,140 @@
+// Host planner: decode contexts -> page-granular KV splits, chunk -> query tiles
+// (x KV splits when there are too few tiles to fill the GPU), one work list for the persistent kernel.
+// Pure integer host code: depends only on lengths (never on page ids), so the GPU result is bit-identical
+// under page permutation.
+#include <algorithm>
+#include <cstdint>
+
+#include "kairos_internal.h"
+
+namespace kairos {
+
+namespace {
+constexpr int kMinSplitPages = 4;      // never cut a KV range into pieces shorter than this
+constexpr int kChunkCostNum = 3;       // cost of one chunk tile-page relative to one decode page = 3/4
+constexpr int kChunkCostDen = 4;       // (tensor-bound tile-page vs HBM-bound decode page; measured)
+
+inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b); }
+}  // namespace
+
+void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len,
+                int32_t target_ctas, int32_t T, Plan* plan) {
+    plan->items.clear();
+    plan->combines.clear();
+    plan->n_decode_items = plan->n_chunk_items = plan->n_partial_slots = 0;
+    if (target_ctas < 1) target_ctas = 1;
+
+    // ---- total cost, in units of 4*decode-page
+    int64_t dec_pages = 0;
+    for (int32_t i = 0; i < n_dec; ++i) dec_pages += ceil_div(dec_ctx_lens[i], kPage);
+    const int32_t n_tiles = chunk_len > 0 ? ceil_div(chunk_len, T) : 0;
+    int64_t tile_pages = 0;
+    for (int32_t t = 0; t < n_tiles; ++t) {
+        int32_t q_last = std::min(chunk_len, (t + 1) * T) - 1;
+        tile_pages += ceil_div(int64_t(prefix_len) + q_last + 1, kPage);
+    }
+    const int64_t total_cost = dec_pages * kChunkCostDen + tile_pages * kChunkCostNum;
+    // an item should not exceed about half of one CTA's fair share
+    int64_t max_item_cost = total_cost / (2 * int64_t(target_ctas));
+    max_item_cost = std::max<int64_t>(max_item_cost, int64_t(kMinSplitPages) * kChunkCostDen);
+
+    // global caps that keep the workspace bound of kairos_workspace_bytes valid
+    int32_t dec_split_budget = 4 * target_ctas;   // extra decode partial slots beyond one per request
+    int32_t chunk_slot_budget = 8 * target_ctas;  // chunk partial token-slots
+
+    std::vector<WorkItem> dec_items, chunk_items;
+
+    // ---- decode splits
+    for (int32_t i = 0; i < n_dec; ++i) {
+        const int32_t pages = ceil_div(dec_ctx_lens[i], kPage);
+        int32_t max_pages = int32_t(std::max<int64_t>(kMinSplitPages, max_item_cost / kChunkCostDen));
+        int32_t n_splits = ceil_div(pages, max_pages);
+        n_splits = std::min(n_splits, std::max(1, pages / kMinSplitPages));
+        if (n_splits > 1 && n_splits - 1 > dec_split_budget) n_splits = 1 + std::max(0, dec_split_budget);
+        if (n_splits > 1) dec_split_budget -= (n_splits - 1);
+        const int32_t per = ceil_div(pages, n_splits);
+        n_splits = ceil_div(pages, per);
+        int32_t first_slot = -1;
+        if (n_splits > 1) {
+            first_slot = plan->n_partial_slots;
+            plan->n_partial_slots += n_splits;
+            plan->combines.push_back(CombineItem{i, first_slot, n_splits, 0 /*decode*/ | (1 << 8) /*slot stride 1*/});
+        }
+        for (int32_t s = 0; s < n_splits; ++s) {
+            WorkItem w{};
+            w.kind = 0;
+            w.q_index = i;
+            w.page_begin = s * per;
+            w.page_end = std::min(pages, (s + 1) * per);
+            w.n_keys = dec_ctx_lens[i];
+            w.n_q = 1;
+            w.partial_slot = n_splits > 1 ? first_slot + s : -1;
+            w.cost = (w.page_end - w.page_begin) * kChunkCostDen;
+            dec_items.push_back(w);
+        }
+    }
+
+    // ---- chunk tiles (KV-split only while there are fewer tiles than CTAs)
+    for (int32_t t = 0; t < n_tiles; ++t) {
+        const int32_t q0 = t * T;
+        const int32_t nq = std::min(chunk_len, q0 + T) - q0;
+        const int32_t pages = ceil_div(int64_t(prefix_len) + q0 + nq, kPage);
+        int32_t n_splits = 1;
+        if (n_tiles < target_ctas) {
+            int32_t max_pages = int32_t(std::max<int64_t>(kMinSplitPages, max_item_cost / kChunkCostNum));
+            n_splits = ceil_div(pages, max_pages);
+            n_splits = std::min(n_splits, std::max(1, pages / kMinSplitPages));
+            if (n_splits > 1 && n_splits * T > chunk_slot_budget) n_splits = std::max(1, chunk_slot_budget / T);
+            if (n_splits > 1) chunk_slot_budget -= n_splits * T;
+        }
+        const int32_t per = ceil_div(pages, n_splits);
+        n_splits = ceil_div(pages, per);
+        int32_t first_slot = -1;
+        if (n_splits > 1) {
+            first_slot = plan->n_partial_slots;
+            plan->n_partial_slots += n_splits * T;  // layout [split][token]
+            for (int32_t j = 0; j < nq; ++j)
+                plan->combines.push_back(CombineItem{q0 + j, first_slot + j, n_splits, 1 /*chunk*/ | (T << 8)});
+        }
+        for (int32_t s = 0; s < n_splits; ++s) {
+            WorkItem w{};
+            w.kind = 1;
+            w.q_index = q0;
+            w.page_begin = s * per;
+            w.page_end = std::min(pages, (s + 1) * per);
+            w.n_keys = prefix_len + q0 + 1;
+            w.n_q = nq;
+            w.partial_slot = n_splits > 1 ? first_slot + s * T : -1;
+            w.cost = (w.page_end - w.page_begin) * kChunkCostNum;
+            chunk_items.push_back(w);
+        }
+    }
+
+    auto by_cost = [](const WorkItem& a, const WorkItem& b) {
+        if (a.cost != b.cost) return a.cost > b.cost;
+        if (a.q_index != b.q_index) return a.q_index < b.q_index;
+        return a.page_begin < b.page_begin;
+    };
+    std::sort(dec_items.begin(), dec_items.end(), by_cost);
+    std::sort(chunk_items.begin(), chunk_items.end(), by_cost);
+
+    // ---- interleave the two kinds in proportion to their total cost, so that at any time part of the
+    // SMs stream decode pages from HBM while the others run chunk tiles on the tensor cores (a10).
+    int64_t dc = 0, cc = 0, dtot = 0, ctot = 0;
+    for (auto& w : dec_items) dtot += w.cost;
+    for (auto& w : chunk_items) ctot += w.cost;
+    size_t di = 0, ci = 0;
+    plan->items.reserve(dec_items.size() + chunk_items.size());
+    while (di < dec_items.size() || ci < chunk_items.size()) {
+        bool take_chunk;
+        if (di >= dec_items.size()) take_chunk = true;
+        else if (ci >= chunk_items.size()) take_chunk = false;
+        else take_chunk = (cc * dtot <= dc * ctot);  // cc/ctot <= dc/dtot: the chunk list is behind
+        if (take_chunk) { cc += chunk_items[ci].cost; plan->items.push_back(chunk_items[ci++]); }
+        else { dc += dec_items[di].cost; plan->items.push_back(dec_items[di++]); }
+    }
+    plan->n_decode_items = int32_t(dec_items.size());
+    plan->n_chunk_items = int32_t(chunk_items.size());
+}
+
+}  // namespace kairos

@@ -1,0 +1,212 @@
+"""Thin Python binding over libkairos.so (include/kairos.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+Importing this module loads the shared library and raises if it is missing: there is no CPU fallback and
+nothing here ever touches oracle/.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkairos.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is not built: run `python -m paper_2607_02043_b200.build` (nvcc, sm_100a). "
+        "There is no CPU fallback.")
+
+_lib = ctypes.CDLL(LIB_PATH)
+_c = ctypes
+_vp = _c.c_void_p
+_i32 = _c.c_int32
+
+
+class KairosConfig(_c.Structure):
+    _fields_ = [("num_heads", _i32), ("latent_dim", _i32), ("rope_dim", _i32), ("page_size", _i32),
+                ("softmax_scale", _c.c_float), ("pool", _vp), ("num_pages", _i32), ("workspace", _vp),
+                ("workspace_bytes", _c.c_size_t), ("device", _i32)]
+
+
+_lib.kairos_workspace_bytes.argtypes = [_i32, _i32]
+_lib.kairos_workspace_bytes.restype = _c.c_size_t
+_lib.kairos_create.argtypes = [_c.POINTER(KairosConfig), _c.POINTER(_vp)]
+_lib.kairos_create.restype = _c.c_int
+_lib.kairos_destroy.argtypes = [_vp]
+_lib.kairos_destroy.restype = _c.c_int
+_lib.kairos_append_latent.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _i32, _vp]
+_lib.kairos_append_latent.restype = _c.c_int
+_lib.kairos_append_decode_tokens.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp]
+_lib.kairos_append_decode_tokens.restype = _c.c_int
+_lib.kairos_gather_latent.argtypes = [_vp, _vp, _i32, _i32, _vp, _vp]
+_lib.kairos_gather_latent.restype = _c.c_int
+_lib.kairos_mixed_step.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp]
+_lib.kairos_mixed_step.restype = _c.c_int
+_lib.kairos_mixed_step_host.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp, _vp,
+                                        _vp, _vp, _vp, _vp, _vp]
+_lib.kairos_mixed_step_host.restype = _c.c_int
+_lib.kairos_step_latency_table.argtypes = [_vp, _vp, _i32, _vp, _i32, _vp, _i32, _i32, _i32, _i32, _i32, _vp, _vp, _vp]
+_lib.kairos_step_latency_table.restype = _c.c_int
+_lib.kairos_last_plan_info.argtypes = [_vp, _vp, _i32]
+_lib.kairos_last_plan_info.restype = _c.c_int
+_lib.kairos_last_error.argtypes = []
+_lib.kairos_last_error.restype = _c.c_char_p
+_lib.kairos_version.argtypes = []
+_lib.kairos_version.restype = _c.c_char_p
+
+EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
+           "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
+           "kairos_step_latency_table", "kairos_last_plan_info", "kairos_last_error", "kairos_version"]
+
+STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
+          -4: "KAIROS_ERR_CUDA"}
+
+
+class KairosError(RuntimeError):
+    def __init__(self, code: int):
+        self.code = code
+        super().__init__(f"{STATUS.get(code, code)}: {_lib.kairos_last_error().decode()}")
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise KairosError(rc)
+
+
+def version() -> str:
+    return _lib.kairos_version().decode()
+
+
+def workspace_bytes(max_decodes: int, max_chunk: int) -> int:
+    return int(_lib.kairos_workspace_bytes(int(max_decodes), int(max_chunk)))
+
+
+def _dp(t: Optional[torch.Tensor]) -> Optional[int]:
+    if t is None or t.numel() == 0:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device, contiguous tensors only"
+    return t.data_ptr()
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> Optional[int]:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream or None
+
+
+class Kairos:
+    """One context = one paged latent pool + workspace on one device (kairos_create / kairos_destroy)."""
+
+    def __init__(self, pool: torch.Tensor, workspace: torch.Tensor, softmax_scale: float = 1.0 / 192.0 ** 0.5):
+        assert pool.is_cuda and pool.dtype == torch.bfloat16 and pool.is_contiguous()
+        assert pool.dim() == 3 and pool.shape[1] == 64 and pool.shape[2] == 576
+        assert workspace.is_cuda and workspace.is_contiguous()
+        self.pool, self.workspace = pool, workspace  # keep the caller's buffers alive
+        cfg = KairosConfig(16, 512, 64, 64, float(softmax_scale), pool.data_ptr(), int(pool.shape[0]),
+                           workspace.data_ptr(), workspace.numel() * workspace.element_size(), pool.device.index or 0)
+        h = _vp()
+        _check(_lib.kairos_create(_c.byref(cfg), _c.byref(h)))
+        self._h = h
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            _lib.kairos_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- a1
+    def append_latent(self, latent: torch.Tensor, k_rope: torch.Tensor, page_table: torch.Tensor, start_pos: int,
+                      stream: Optional[torch.cuda.Stream] = None) -> None:
+        n = int(latent.shape[0])
+        _check(_lib.kairos_append_latent(self._h, _dp(latent), _dp(k_rope), n, _dp(page_table),
+                                         int(page_table.numel()), int(start_pos), _stream_ptr(stream)))
+
+    def append_decode_tokens(self, latent, k_rope, page_tables, positions, stream=None) -> None:
+        n = int(latent.shape[0])
+        _check(_lib.kairos_append_decode_tokens(self._h, _dp(latent), _dp(k_rope), n, _dp(page_tables),
+                                                int(page_tables.shape[1]) if n else 1, _dp(positions),
+                                                _stream_ptr(stream)))
+
+    def gather_latent(self, page_table: torch.Tensor, n_tokens: int, stream=None) -> torch.Tensor:
+        out = torch.empty((n_tokens, 576), dtype=torch.bfloat16, device=self.pool.device)
+        _check(_lib.kairos_gather_latent(self._h, _dp(page_table), int(page_table.numel()), int(n_tokens), _dp(out),
+                                         _stream_ptr(stream)))
+        return out
+
+    # -- a2..a10
+    def mixed_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table,
+                   chunk_len: int, prefix_len: int, out_dec=None, out_chunk=None, lse_dec=None, lse_chunk=None,
+                   want_lse: bool = True, stream=None):
+        dev = self.pool.device
+        lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        B, C = int(lens.shape[0]), int(chunk_len)
+        if out_dec is None:
+            out_dec = torch.empty((B, 16, 512), dtype=torch.bfloat16, device=dev)
+        if out_chunk is None:
+            out_chunk = torch.empty((C, 16, 512), dtype=torch.bfloat16, device=dev)
+        if want_lse and lse_dec is None:
+            lse_dec = torch.empty((B, 16), dtype=torch.float32, device=dev)
+        if want_lse and lse_chunk is None:
+            lse_chunk = torch.empty((C, 16), dtype=torch.float32, device=dev)
+        stride = int(dec_page_tables.shape[1]) if B else 1
+        _check(_lib.kairos_mixed_step(self._h, B, _dp(q_dec), _dp(dec_page_tables), stride,
+                                      lens.ctypes.data_as(_vp), C, int(prefix_len), _dp(q_chunk),
+                                      _dp(chunk_page_table), int(chunk_page_table.numel()) if C else 0, _dp(out_dec),
+                                      _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk), _stream_ptr(stream)))
+        return out_dec, out_chunk, lse_dec, lse_chunk
+
+    def mixed_step_host(self, q_dec: np.ndarray, dec_page_tables: np.ndarray, dec_ctx_lens: np.ndarray,
+                        q_chunk: np.ndarray, chunk_latent: np.ndarray, chunk_k_rope: np.ndarray,
+                        chunk_page_table: np.ndarray, chunk_len: int, prefix_len: int, out_dec: np.ndarray,
+                        out_chunk: np.ndarray, stream=None):
+        """HOST buffers in, HOST buffers out (numpy uint16 views of bf16; pin them with torch for speed)."""
+        lens = np.ascontiguousarray(dec_ctx_lens, dtype=np.int32)
+        B, C = int(lens.shape[0]), int(chunk_len)
+        h2d, d2h = _c.c_uint64(0), _c.c_uint64(0)
+
+        def hp(a):
+            return None if a is None or a.size == 0 else a.ctypes.data_as(_vp)
+        stride = int(dec_page_tables.shape[1]) if B else 1
+        _check(_lib.kairos_mixed_step_host(self._h, B, hp(q_dec), hp(dec_page_tables), stride, hp(lens), C,
+                                           int(prefix_len), hp(q_chunk), hp(chunk_latent), hp(chunk_k_rope),
+                                           hp(chunk_page_table), int(chunk_page_table.size) if C else 0, hp(out_dec),
+                                           hp(out_chunk), None, None, _c.byref(h2d), _c.byref(d2h),
+                                           _stream_ptr(stream)))
+        return int(h2d.value), int(d2h.value)
+
+    # -- a11
+    def step_latency_table(self, Bs: Sequence[int], Ks: Sequence[int], Cs: Sequence[int], prefix_len: int = 0,
+                           warmup: int = 5, reps: int = 20, flush_l2: bool = True, stream=None):
+        Bs_, Ks_, Cs_ = (np.ascontiguousarray(np.asarray(x, dtype=np.int32)) for x in (Bs, Ks, Cs))
+        med = np.zeros((len(Bs_), len(Ks_), len(Cs_)), dtype=np.float64)
+        mn = np.zeros_like(med)
+        _check(_lib.kairos_step_latency_table(self._h, Bs_.ctypes.data_as(_vp), len(Bs_), Ks_.ctypes.data_as(_vp),
+                                              len(Ks_), Cs_.ctypes.data_as(_vp), len(Cs_), int(prefix_len),
+                                              int(warmup), int(reps), int(bool(flush_l2)), med.ctypes.data_as(_vp),
+                                              mn.ctypes.data_as(_vp), _stream_ptr(stream)))
+        return med, mn
+
+    def last_plan_info(self) -> dict:
+        info = (_c.c_int64 * 6)()
+        _check(_lib.kairos_last_plan_info(self._h, info, 6))
+        keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes"]
+        return dict(zip(keys, (int(x) for x in info)))
+
+
+def bf16_tensor(bits: np.ndarray, device="cuda") -> torch.Tensor:
+    """numpy uint16 bf16 bit patterns -> torch.bfloat16 tensor on `device` (bit-exact)."""
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(device).view(torch.bfloat16)
+
+
+def bf16_bits(t: torch.Tensor) -> np.ndarray:
+    """torch.bfloat16 tensor -> numpy uint16 bit patterns (bit-exact)."""
+    return t.detach().contiguous().view(torch.int16).cpu().numpy().view(np.uint16)

@@ -1,0 +1,251 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): cache append and page indexing bit-exact; attention max-abs <= 2e-2 and
+relative L2 <= 5e-3 (bf16 in, fp32 accumulation).  Small cases compare every row; the BASELINE.json configs
+at full size compare every row where the oracle finishes in seconds and a seeded sample of rows otherwise
+(rows are independent, so sampled parity is exact per row).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2607_02043_b200 import workloads as W
+from tests import helpers as Hp
+
+pytestmark = pytest.mark.gpu
+
+IMPLS = ["umma", "simple"]
+
+
+def _full_compare(inp, impl, check_append=True):
+    from oracle import oracle
+    run = Hp.GpuRun(inp, impl)
+    run.append()
+    pool_np = Hp.oracle_pool_after_append(inp)
+    if check_append:
+        assert np.array_equal(run.pool_bits(), pool_np), "append: pool bytes differ"
+    od, oc, ld, lc = run.step()
+    rd, rc, rld, rlc = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len,
+                                         inp.prefix_len, inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    e = Hp.assert_attention_close([od, oc], [rd, rc], f"{inp.name}/{impl}")
+    if od.size:
+        assert np.abs(ld - rld).max() <= Hp.LSE_TOL
+    if oc.size:
+        assert np.abs(lc - rlc).max() <= Hp.LSE_TOL
+    return run, (od, oc, ld, lc), e
+
+
+# ------------------------------------------------------------------ append / gather: bit-exact
+def test_append_and_gather_bit_exact():
+    import torch
+    from oracle import oracle
+    from paper_2607_02043_b200 import kairos as K
+    rng = np.random.default_rng(0)
+    num_pages = 40
+    pool_np = np.full((num_pages, 64, 576), 0xABCD, np.uint16)
+    pt = rng.permutation(num_pages).astype(np.int32)[:30]
+    pool = K.bf16_tensor(pool_np)
+    ws = torch.empty(K.workspace_bytes(1, 1), dtype=torch.uint8, device="cuda")
+    ctx = K.Kairos(pool, ws)
+    pt_d = torch.from_numpy(pt).cuda()
+    for n, start in [(1, 0), (100, 37), (64, 64), (1, 1919), (700, 900)]:
+        lat = rng.integers(0, 2 ** 16, (n, 512), dtype=np.uint16)
+        rope = rng.integers(0, 2 ** 16, (n, 64), dtype=np.uint16)
+        ctx.append_latent(K.bf16_tensor(lat), K.bf16_tensor(rope), pt_d, start)
+        oracle.append(pool_np, lat, rope, pt, start)
+        torch.cuda.synchronize()
+        assert np.array_equal(K.bf16_bits(pool), pool_np), (n, start)
+    g = ctx.gather_latent(pt_d, 1777)
+    assert np.array_equal(K.bf16_bits(g), oracle.gather(pool_np, pt, 1777))
+    # batched one-token-per-request append
+    n = 7
+    pts = np.stack([rng.permutation(num_pages).astype(np.int32)[:4] for _ in range(n)])
+    pos = rng.integers(0, 256, n).astype(np.int32)
+    lat = rng.integers(0, 2 ** 16, (n, 512), dtype=np.uint16)
+    rope = rng.integers(0, 2 ** 16, (n, 64), dtype=np.uint16)
+    # make target slots distinct so the expected result does not depend on write order
+    ctx.append_decode_tokens(K.bf16_tensor(lat), K.bf16_tensor(rope), torch.from_numpy(pts).cuda(),
+                             torch.from_numpy(pos).cuda())
+    slots = set()
+    for i in range(n):
+        key = (int(pts[i, pos[i] // 64]), int(pos[i] % 64))
+        if key in slots:
+            continue
+        slots.add(key)
+    torch.cuda.synchronize()
+    got = K.bf16_bits(pool)
+    for i in reversed(range(n)):
+        oracle.append(pool_np, lat[i:i + 1], rope[i:i + 1], pts[i], int(pos[i]))
+    if len(slots) == n:
+        assert np.array_equal(got, pool_np)
+    # error paths: detected on the host, nothing enqueued
+    with pytest.raises(K.KairosError) as ei:
+        ctx.append_latent(K.bf16_tensor(lat), K.bf16_tensor(rope), pt_d, 30 * 64 - 3)
+    assert ei.value.code == -1
+
+
+# ------------------------------------------------------------------ BASELINE.json configs[0]: every row
+@pytest.mark.parametrize("impl", IMPLS)
+def test_config0_pr1_ref(impl):
+    _full_compare(W.make_config(0), impl)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_config0_unscaled_q(impl):
+    """G9: sharper softmax (score std ~1.7) exercises the running-max / rescale path."""
+    _full_compare(W.make_config(0, q_scale=1.0), impl)
+
+
+# ------------------------------------------------------------------ edge cases (every row)
+EDGE = [
+    ("decode_only", dict(dec_ctx_lens=[1, 2, 63, 64, 65, 700], chunk_len=0, prefix_len=0)),
+    ("chunk_only_ragged", dict(dec_ctx_lens=[], chunk_len=37, prefix_len=91)),
+    ("chunk_one_token_no_prefix", dict(dec_ctx_lens=[5], chunk_len=1, prefix_len=0)),
+    ("chunk_crosses_pages", dict(dec_ctx_lens=[130], chunk_len=130, prefix_len=63)),
+    ("long_decode_split", dict(dec_ctx_lens=[9000, 64, 4097], chunk_len=6, prefix_len=300)),
+    ("few_tiles_long_prefix", dict(dec_ctx_lens=[], chunk_len=10, prefix_len=5000)),
+]
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("name,kw", EDGE, ids=[e[0] for e in EDGE])
+def test_edge_cases(name, kw, impl):
+    inp = W.make_inputs(name, 100 + len(name), q_scale=0.5, extra_pages=3, **kw)
+    _full_compare(inp, impl)
+
+
+def test_empty_step_is_noop_and_errors_are_host_side():
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    inp = W.make_inputs("t", 1, [70], 8, 8)
+    run = Hp.GpuRun(inp)
+    e = torch.empty((0, 16, 576), dtype=torch.bfloat16, device="cuda")
+    run.ctx.mixed_step(e, torch.empty((0, 1), dtype=torch.int32, device="cuda"), [], e,
+                       torch.empty(0, dtype=torch.int32, device="cuda"), 0, 0)
+    with pytest.raises(K.KairosError) as ei:   # ctx_len 0
+        run.ctx.mixed_step(run.q_dec, run.dec_pt, [0], run.q_chunk, run.chunk_pt, inp.chunk_len, inp.prefix_len)
+    assert ei.value.code == -1
+    with pytest.raises(K.KairosError) as ei:   # ctx_len beyond its table
+        run.ctx.mixed_step(run.q_dec, run.dec_pt, [64 * run.dec_pt.shape[1] + 1], run.q_chunk, run.chunk_pt,
+                           inp.chunk_len, inp.prefix_len)
+    assert ei.value.code == -1
+    with pytest.raises(K.KairosError) as ei:   # chunk table too short
+        run.ctx.mixed_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, inp.chunk_len, 64)
+    assert ei.value.code == -1
+
+
+# ------------------------------------------------------------------ invariants on the GPU
+@pytest.mark.parametrize("impl", IMPLS)
+def test_page_permutation_and_stale_slots_bit_identical(impl):
+    """G13 / G7: the planner depends only on lengths, so permuting physical pages -- or poisoning every slot
+    that is not visible with +-1e4 -- must leave the GPU output bit-identical."""
+    inp = W.make_inputs("perm", 21, [64, 130, 700, 2500], 70, 90, q_scale=0.5, extra_pages=5)
+    run = Hp.GpuRun(inp, impl)
+    run.append()
+    a = run.step()
+    rng = np.random.default_rng(5)
+    pool_np = Hp.oracle_pool_after_append(inp)
+    sig = rng.permutation(inp.num_pages)
+    pool2 = np.empty_like(pool_np)
+    pool2[sig] = pool_np
+    used = np.zeros((inp.num_pages, 64), bool)
+    for i, L in enumerate(inp.dec_ctx_lens):
+        t = np.arange(L)
+        used[sig[inp.dec_page_tables[i][t // 64]], t % 64] = True
+    t = np.arange(inp.prefix_len + inp.chunk_len)
+    used[sig[inp.chunk_page_table[t // 64]], t % 64] = True
+    pool2[~used] = W.f32_to_bf16_bits(np.float32(1e4))
+    inp2 = W.MixedStepInputs(**{**inp.__dict__, "pool": pool2,
+                                "dec_page_tables": sig[inp.dec_page_tables].astype(np.int32),
+                                "chunk_page_table": sig[inp.chunk_page_table].astype(np.int32), "chunk_len": inp.chunk_len})
+    run2 = Hp.GpuRun(inp2, impl)   # chunk already in pool2: no append
+    b = run2.step()
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_decode_equals_last_prefill_row_and_chunk_invariance_gpu():
+    """PAPER.md:66 / :23 on the GPU: a prompt run as successive (append, step) chunks matches the one-shot
+    oracle prefill row for row, and a decode over the finished cache matches the last row (within tolerance)."""
+    from oracle import oracle
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    rng = np.random.default_rng(3)
+    L = 400
+    inp = W.make_inputs("sched", 31, [], L, 0, q_scale=0.5, extra_pages=2)
+    pool_np = inp.pool.copy()
+    oracle.append(pool_np, inp.chunk_latent, inp.chunk_k_rope, inp.chunk_page_table, 0)
+    _, ref, _, _ = oracle.mixed_step(pool_np, np.zeros((0, 16, 576), np.uint16), np.zeros((0, 1), np.int32),
+                                     np.zeros(0, np.int32), L, 0, inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    run = Hp.GpuRun(inp)
+    outs, pos = [], 0
+    e = torch.empty((0, 16, 576), dtype=torch.bfloat16, device="cuda")
+    ept = torch.empty((0, 1), dtype=torch.int32, device="cuda")
+    for c in [128, 100, 1, 71, 100]:
+        run.ctx.append_latent(run.latent[pos:pos + c], run.k_rope[pos:pos + c], run.chunk_pt, pos)
+        _, oc, _, _ = run.ctx.mixed_step(e, ept, [], run.q_chunk[pos:pos + c].contiguous(), run.chunk_pt, c, pos)
+        outs.append(W.bf16_bits_to_f32(K.bf16_bits(oc)))
+        pos += c
+    got = np.concatenate(outs)
+    assert np.array_equal(run.pool_bits(), pool_np)
+    Hp.assert_attention_close([got], [ref], "chunk schedule")
+    od, _, _, _ = run.ctx.mixed_step(run.q_chunk[L - 1:L].contiguous(), run.chunk_pt[None, :].contiguous(), [L], e,
+                                     run.chunk_pt, 0, 0)
+    torch.cuda.synchronize()
+    Hp.assert_attention_close([W.bf16_bits_to_f32(K.bf16_bits(od))[0]], [ref[L - 1]], "decode = last row")
+
+
+# ------------------------------------------------------------------ BASELINE.json configs at full size
+def test_config1_steady_state_every_row():
+    _full_compare(W.make_config(1), "umma")
+
+
+def test_config1_unscaled_q_every_row():
+    _full_compare(W.make_config(1, q_scale=1.0), "umma")
+
+
+def _sampled_compare(inp, n_dec_samples=8, n_chunk_samples=24):
+    rng = np.random.default_rng(99)
+    run = Hp.GpuRun(inp, "umma")
+    run.append()
+    pool_np = Hp.oracle_pool_after_append(inp)
+    assert np.array_equal(run.pool_bits(), pool_np), "append: pool bytes differ"
+    od, oc, ld, lc = run.step()
+    assert np.all(np.isfinite(od)) and np.all(np.isfinite(oc))
+    L = inp.dec_ctx_lens
+    di = Hp.sample_indices(inp.n_dec, n_dec_samples, rng, always=[int(np.argmax(L)), int(np.argmin(L)), 0, inp.n_dec - 1])
+    C = inp.chunk_len
+    ci = Hp.sample_indices(C, n_chunk_samples, rng, always=[0, 1, 3, 4, 63, 64, C // 2, C - 5, C - 4, C - 1])
+    rd, rld, rc, rlc = Hp.oracle_sampled(inp, pool_np, di, ci)
+    g, r = [], []
+    if len(di):
+        g.append(od[di]); r.append(rd)
+        assert np.abs(ld[di] - rld).max() <= Hp.LSE_TOL
+    if len(ci):
+        g.append(oc[ci]); r.append(rc)
+        assert np.abs(lc[ci] - rlc).max() <= Hp.LSE_TOL
+    return Hp.assert_attention_close(g, r, inp.name + " (sampled rows)")
+
+
+def test_config2_heavy_tail_sampled_rows():
+    _sampled_compare(W.make_config(2))
+
+
+@pytest.mark.parametrize("C", [0, 512, 8192])
+def test_config3_chunk_sweep_sampled_rows(C):
+    _sampled_compare(W.make_config(3, chunk_len=C))
+
+
+def test_config4_long_context_sampled_rows():
+    _sampled_compare(W.make_config(4), n_dec_samples=3, n_chunk_samples=10)
+
+
+def test_latency_table_shape_and_monotone():
+    """a11: the table is produced, positive, and roughly monotone in C at the large end."""
+    inp = W.make_inputs("lt", 7, [2048] * 64, 0, 0, extra_pages=140)
+    run = Hp.GpuRun(inp)
+    med, mn = run.ctx.step_latency_table([0, 64], [2048], [0, 256, 4096], warmup=2, reps=5)
+    assert med.shape == (2, 1, 3) and med[0, 0, 0] == 0.0
+    assert np.all(med.ravel()[1:] > 0) and np.all(mn <= med + 1e-9)
+    assert med[1, 0, 2] > med[1, 0, 0] and med[0, 0, 2] > med[0, 0, 1]
