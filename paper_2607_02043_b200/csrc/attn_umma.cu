@@ -1,10 +1,565 @@
-// placeholder: replaced by the tcgen05 kernel
+// impl 1 (the product path): persistent, warp-specialised tcgen05 / TMA / TMEM kernel for the mixed step.
+//
+// One CTA per SM pops work items (decode KV splits and prefill-chunk tiles) from one
+// queue.  Both item kinds run the same "swapped operand" pipeline on one 64-token page per iteration, because all
+// 16 heads of a token share one latent tile (BASELINE.json north_star):
+//
+//   S^T[64 keys x N]  = K_page[64 x 576] . Q^T[576 x N]      tcgen05.mma M=64,  K-major A (page) and B (queries)
+//   P^T = exp2(S^T*c - m)  (column statistics across the 64 key lanes, lazy max update)
+//   O^T[512 x N]     += V^T[512 x 64] . P^T[64 x N]          tcgen05.mma M=128 x4, MN-major A = the SAME smem page
+//
+//   N = 16 query rows (1 decode token x 16 heads) or 64 (4 chunk tokens x 16 heads).  The page tile is loaded once
+//   by one 3-D TMA (SWIZZLE_128B, [9 chunks][64 tokens][128 B]) and serves as K (K-major) and as V (MN-major).
+//   Accumulators live in TMEM: S^T double-buffered (2 x 64 columns), O^T 4 x 64 columns, fp32.
+//
+// Warp roles (192 threads): warp 0 = TMA producer + work-queue pop, warp 1 = MMA issuer (one lane) + TMEM owner,
+// warps 2-5 = softmax / correction / epilogue (one TMEM lane quadrant each).
+// Descriptor encodings were validated on B200 by profiles/r01_tcgen05_probe.txt.
+#include <cuda_bf16.h>
+
+#include <algorithm>
+
 #include "kairos_internal.h"
+#include "umma_ptx.cuh"
+
 namespace kairos {
-int umma_chunk_tile_tokens() { return 4; }
+namespace {
+using namespace ptx;
+
+constexpr int kThreads = 192;
+constexpr int kChunkTileTokens = 4;
+constexpr int kStageBytes = kPage * kTokenBytes;  // 73,728: one page
+constexpr int kQBytes = 64 * kTokenBytes;         // 73,728: up to 64 query rows
+constexpr int kPBytes = 64 * 64 * 2;              // 8,192: P^T [64 keys][<=64 rows] bf16
+constexpr int kOffQ = 0;
+constexpr int kOffKV = kQBytes;
+constexpr int kOffP = kOffKV + 2 * kStageBytes;
+constexpr int kOffSmall = kOffP + kPBytes;        // 229,376
+constexpr int kSmallBytes = 2048;
+constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;  // + alignment slack = 232,448 = the 227 KB limit
+static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
+
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64
+constexpr uint32_t kColO = 128;  // O^T blocks at 128 + 64*b
+constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the max grows by more than 2^8
+constexpr float kLn2 = 0.6931471805599453f;
+
+struct Small {
+    uint64_t q_full, q_empty, kv_full[2], kv_empty[2], s_full[2], s_empty[2], p_full, pv_done, o_full, o_empty;
+    uint64_t item_full[2], item_empty[2];
+    int32_t item_ring[2];
+    uint32_t tmem_base;
+    uint32_t pad;
+    float m_ref[64];   // running reference max per query row (log2 domain); -inf while nothing visible yet
+    float alpha[64];   // O / l rescale factor decided for the current page
+    float red[4][64];  // per-warp column maxima (per page) / column sums (epilogue)
+    float linv[64];
+};
+static_assert(sizeof(Small) <= kSmallBytes, "Small does not fit");
+
+struct KParams {
+    const WorkItem* items;
+    int32_t n_items;
+    int32_t* counters;  // [0] queue head, [1] finished CTAs
+    const int32_t* dec_pt;
+    int32_t dec_stride;
+    const int32_t* chunk_pt;
+    __nv_bfloat16* out_dec;
+    __nv_bfloat16* out_chunk;
+    float* lse_dec;
+    float* lse_chunk;
+    uint8_t* partials;
+    float scale_log2;
+};
+
+__device__ __forceinline__ WorkItem load_item(const WorkItem* p) {
+    const int4 a = __ldg(reinterpret_cast<const int4*>(p));
+    const int4 b = __ldg(reinterpret_cast<const int4*>(p) + 1);
+    WorkItem w;
+    w.kind = a.x; w.q_index = a.y; w.page_begin = a.z; w.page_end = a.w;
+    w.n_keys = b.x; w.n_q = b.y; w.partial_slot = b.z; w.cost = b.w;
+    return w;
+}
+
+__device__ __forceinline__ void tma_load_page(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t row, uint64_t policy) {
+    // 3-D box (64 elems, 64 rows, 9 chunks) of the pool viewed as [chunk][row][64]: lands as [9][64][128 B]
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5}], [%2], %6;"
+        ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(0), "r"(row), "r"(0),
+          "l"(policy)
+        : "memory");
+}
+
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float warp_max(float v) {
+    float r;
+    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+    return r;
+}
+__device__ __forceinline__ void named_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ bool named_or(int id, bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "setp.ne.u32 p, %1, 0;\n\t"
+        "bar.red.or.pred q, %2, 128, p;\n\t"
+        "selp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(r)
+        : "r"(uint32_t(pred)), "r"(id)
+        : "memory");
+    return r != 0;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// softmax / correction / epilogue for one work item; N = 16 (decode) or 64 (chunk tile) query rows
+// ------------------------------------------------------------------------------------------------------------
+template <int N>
+__device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkItem& w, const KParams& p, uint32_t tmem,
+                                             int w4, int lane, uint32_t& g, uint32_t it) {
+    const int tid_s = w4 * 32 + lane;
+    const bool lane_ok = lane < 16;       // M=64 accumulator rows live in lanes 0..15 of each quadrant
+    const int tok_in_page = w4 * 16 + lane;
+    float l[N];
+#pragma unroll
+    for (int c = 0; c < N; ++c) l[c] = 0.f;
+    if (tid_s < N) sm->m_ref[tid_s] = -INFINITY;  // owner thread; others read it only after the named barriers below
+
+    const int npages = w.page_end - w.page_begin;
+    for (int pg = 0; pg < npages; ++pg, ++g) {
+        const int b = g & 1;
+        mbar_wait(&sm->s_full[b], (g >> 1) & 1);
+        tc_fence_after();
+        float x[N];
+#pragma unroll
+        for (int c0 = 0; c0 < N; c0 += 16)
+            tmem_ld16(tmem_addr(tmem, w4 * 32, kColS + b * 64 + c0), *reinterpret_cast<uint32_t(*)[16]>(&x[c0]));
+        tmem_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm->s_empty[b]);
+
+        const int page = w.page_begin + pg;
+        const int key_pos = page * kPage + tok_in_page;
+        const bool boundary = (page + 1) * kPage > w.n_keys;  // some row may not see every key of this page
+#pragma unroll
+        for (int c = 0; c < N; ++c) {
+            const float v = x[c] * p.scale_log2;
+            const bool ok = lane_ok && (!boundary || key_pos < w.n_keys + (N == 64 ? (c >> 4) : 0));
+            x[c] = ok ? v : -INFINITY;
+        }
+        // column (query-row) max over the 64 keys of the page: warp redux, then 4 warps through smem
+#pragma unroll
+        for (int c = 0; c < N; ++c) {
+            const float wm = warp_max(x[c]);
+            if (lane == (c & 31)) sm->red[w4][c] = wm;
+        }
+        named_sync(1);
+        bool need = false;
+        if (tid_s < N) {
+            const float tm = fmaxf(fmaxf(sm->red[0][tid_s], sm->red[1][tid_s]), fmaxf(sm->red[2][tid_s], sm->red[3][tid_s]));
+            const float mo = sm->m_ref[tid_s];
+            float mn = mo, a = 1.f;
+            if (tm > mo + kRescaleThreshold) {  // also true for mo = -inf and finite tm
+                mn = tm;
+                if (mo != -INFINITY) { a = ex2(mo - mn); need = true; }
+            }
+            sm->m_ref[tid_s] = mn;
+            sm->alpha[tid_s] = a;
+        }
+        const bool rescale = named_or(2, need);
+        if (g > 0) mbar_wait(&sm->pv_done, (g - 1) & 1);  // PV of the previous page done: P buffer free, O stable
+        if (rescale) {
+            tc_fence_after();
+#pragma unroll
+            for (int b4 = 0; b4 < 4; ++b4)
+#pragma unroll
+                for (int c0 = 0; c0 < N; c0 += 16) {
+                    uint32_t r[16];
+                    const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0);
+                    tmem_ld16(ta, r);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[c0 + i]);
+                    tmem_st16(ta, r);
+                }
+            tmem_wait_st();
+#pragma unroll
+            for (int c = 0; c < N; ++c) l[c] *= sm->alpha[c];
+        }
+#pragma unroll
+        for (int c = 0; c < N; ++c) {
+            float m = sm->m_ref[c];
+            m = (m == -INFINITY) ? 0.f : m;
+            const float pv = ex2(x[c] - m);
+            l[c] += pv;
+            x[c] = pv;
+        }
+        if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
+#pragma unroll
+            for (int j = 0; j < N / 8; ++j) {
+                uint4 v;
+                v.x = pack_bf16(x[8 * j + 0], x[8 * j + 1]);
+                v.y = pack_bf16(x[8 * j + 2], x[8 * j + 3]);
+                v.z = pack_bf16(x[8 * j + 4], x[8 * j + 5]);
+                v.w = pack_bf16(x[8 * j + 6], x[8 * j + 7]);
+                *reinterpret_cast<uint4*>(ps + sw128_offset(tok_in_page, j)) = v;
+            }
+        }
+        fence_proxy_async_smem();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm->p_full);
+    }
+
+    // ---- epilogue: all PV MMAs of the item are complete
+    mbar_wait(&sm->o_full, it & 1);
+    tc_fence_after();
+#pragma unroll
+    for (int c = 0; c < N; ++c) {
+        float v = l[c];
+        v += __shfl_xor_sync(0xffffffffu, v, 8);
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 1);  // lanes 0..15 hold the data, lanes 16..31 hold zeros
+        if (lane == (c & 15)) sm->red[w4][c] = v;
+    }
+    named_sync(1);
+    const bool is_final = w.partial_slot < 0;
+    if (tid_s < N) {
+        const float L = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
+        sm->linv[tid_s] = 1.f / L;
+        const float m = sm->m_ref[tid_s];
+        const int tok = tid_s >> 4, h = tid_s & 15;
+        if (tok < w.n_q) {
+            if (is_final) {
+                float* lse = w.kind ? p.lse_chunk : p.lse_dec;
+                if (lse) lse[size_t(w.q_index + tok) * kHeads + h] = (m + log2f(L)) * kLn2;
+            } else {
+                float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes +
+                                                     size_t(kHeads) * kLatent * 4);
+                ml[h] = m;
+                ml[kHeads + h] = L;
+            }
+        }
+    }
+    named_sync(2);
+#pragma unroll
+    for (int b4 = 0; b4 < 4; ++b4) {
+        const int d = b4 * 128 + tid_s;
+#pragma unroll
+        for (int c0 = 0; c0 < N; c0 += 16) {
+            const int tok = c0 >> 4;
+            if (tok >= w.n_q) continue;  // ragged chunk tail (uniform across the CTA)
+            uint32_t r[16];
+            tmem_ld16(tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0), r);
+            tmem_wait_ld();
+            if (is_final) {
+                __nv_bfloat16* o = (w.kind ? p.out_chunk : p.out_dec) + size_t(w.q_index + tok) * kHeads * kLatent + d;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) o[i * kLatent] = __float2bfloat16_rn(__uint_as_float(r[i]) * sm->linv[c0 + i]);
+            } else {
+                float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes) + d;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) o[i * kLatent] = __uint_as_float(r[i]);
+            }
+        }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm->o_empty);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads, 1)
+kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_constant__ CUtensorMap qd_map,
+                    const __grid_constant__ CUtensorMap qc_map, const KParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    Small* sm = reinterpret_cast<Small*>(base + kOffSmall);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&sm->q_full, 1);
+        mbar_init(&sm->q_empty, 1);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&sm->kv_full[i], 1);
+            mbar_init(&sm->kv_empty[i], 1);
+            mbar_init(&sm->s_full[i], 1);
+            mbar_init(&sm->s_empty[i], 4);
+            mbar_init(&sm->item_full[i], 1);
+            mbar_init(&sm->item_empty[i], 5);
+        }
+        mbar_init(&sm->p_full, 4);
+        mbar_init(&sm->pv_done, 1);
+        mbar_init(&sm->o_full, 1);
+        mbar_init(&sm->o_empty, 4);
+        fence_barrier_init();
+    }
+    if (warp == 0 && lane == 0) {
+        prefetch_tensormap(&pool_map);
+        prefetch_tensormap(&qd_map);
+        prefetch_tensormap(&qc_map);
+    }
+    if (warp == 1) tmem_alloc(&sm->tmem_base, kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm->tmem_base;
+
+    if (warp == 0) {
+        // ================= producer: pop work items, TMA-load Q tiles and KV pages =================
+        uint32_t g = 0;
+        for (uint32_t it = 0;; ++it) {
+            int idx = 0;
+            if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx >= p.n_items) idx = -1;
+            if (lane == 0) {
+                mbar_wait(&sm->item_empty[it & 1], ((it >> 1) & 1) ^ 1);
+                sm->item_ring[it & 1] = idx;
+                mbar_arrive(&sm->item_full[it & 1]);
+            }
+            if (idx < 0) break;
+            const WorkItem w = load_item(p.items + idx);
+            const int N = w.kind ? 64 : 16;
+            if (lane == 0) {
+                mbar_wait(&sm->q_empty, (it & 1) ^ 1);
+                mbar_arrive_expect_tx(&sm->q_full, uint32_t(9 * N * 128));
+                const CUtensorMap* qm = w.kind ? &qc_map : &qd_map;
+                for (int c = 0; c < 9; ++c)
+                    tma_load_2d(base + kOffQ + c * N * 128, qm, &sm->q_full, c * 64, w.q_index * kHeads, kEvictFirst);
+            }
+            const int32_t* pt = (w.kind ? p.chunk_pt : p.dec_pt + size_t(w.q_index) * p.dec_stride) + w.page_begin;
+            const uint64_t policy = w.kind ? kEvictLast : kEvictFirst;  // chunk KV is re-read by every tile
+            const int npages = w.page_end - w.page_begin;
+            for (int i = 0; i < npages; i += 32) {
+                const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
+                const int cnt = min(32, npages - i);
+                for (int j = 0; j < cnt; ++j, ++g) {
+                    const int pid = __shfl_sync(0xffffffffu, my, j);
+                    if (lane == 0) {
+                        const int st = g & 1;
+                        mbar_wait(&sm->kv_empty[st], ((g >> 1) & 1) ^ 1);
+                        mbar_arrive_expect_tx(&sm->kv_full[st], kStageBytes);
+                        tma_load_page(base + kOffKV + st * kStageBytes, &pool_map, &sm->kv_full[st], pid * kPage, policy);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (one lane) =================
+        if (lane == 0) {
+            const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV), p_base = smem_u32(base + kOffP);
+            uint32_t g = 0;
+            for (uint32_t it = 0;; ++it) {
+                mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
+                const int idx = sm->item_ring[it & 1];
+                mbar_arrive(&sm->item_empty[it & 1]);
+                if (idx < 0) break;
+                const WorkItem w = load_item(p.items + idx);
+                const uint32_t N = w.kind ? 64 : 16;
+                const uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);
+                const uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);
+                const int npages = w.page_end - w.page_begin;
+                mbar_wait(&sm->q_full, it & 1);
+                auto issue_s = [&](uint32_t gg) {
+                    const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
+                    mbar_wait(&sm->kv_full[st], ph);
+                    mbar_wait(&sm->s_empty[st], ph ^ 1);
+                    tc_fence_after();
+                    const uint32_t a0 = kv_base + st * kStageBytes;
+#pragma unroll 1
+                    for (uint32_t c = 0; c < 9; ++c)
+#pragma unroll
+                        for (uint32_t j = 0; j < 4; ++j)
+                            umma_bf16_ss(tmem + kColS + st * 64, make_smem_desc(a0 + c * 8192 + j * 32, 16, 1024),
+                                         make_smem_desc(q_base + c * N * 128 + j * 32, 16, 1024), idesc_s, (c | j) != 0);
+                    umma_commit(&sm->s_full[st]);
+                };
+                issue_s(g);
+                for (int pg = 0; pg < npages; ++pg) {
+                    const uint32_t gg = g + pg;
+                    if (pg + 1 < npages) issue_s(gg + 1);
+                    else umma_commit(&sm->q_empty);  // every S-MMA of the item issued: Q tile free once they retire
+                    if (pg == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
+                    mbar_wait(&sm->p_full, gg & 1);
+                    tc_fence_after();
+                    const uint32_t st = gg & 1, a0 = kv_base + st * kStageBytes;
+#pragma unroll 1
+                    for (uint32_t b4 = 0; b4 < 4; ++b4)
+#pragma unroll
+                        for (uint32_t ks = 0; ks < 4; ++ks)
+                            umma_bf16_ss(tmem + kColO + b4 * 64, make_smem_desc(a0 + (2 * b4) * 8192 + ks * 2048, 8192, 1024),
+                                         make_smem_desc(p_base + ks * 2048, 8192, 1024), idesc_o, (pg > 0 || ks > 0));
+                    umma_commit(&sm->kv_empty[st]);
+                    umma_commit(&sm->pv_done);
+                }
+                umma_commit(&sm->o_full);
+                g += npages;
+            }
+        }
+    } else {
+        // ================= softmax / correction / epilogue warps =================
+        const int w4 = warp & 3;  // TMEM lane quadrant this warp may access
+        uint8_t* ps = base + kOffP;
+        uint32_t g = 0;
+        for (uint32_t it = 0;; ++it) {
+            mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
+            const int idx = sm->item_ring[it & 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
+            if (idx < 0) break;
+            const WorkItem w = load_item(p.items + idx);
+            if (w.kind) softmax_item<64>(sm, ps, w, p, tmem, w4, lane, g, it);
+            else softmax_item<16>(sm, ps, w, p, tmem, w4, lane, g, it);
+        }
+    }
+
+    // ---- teardown
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem, kTmemCols);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const int prev = atomicAdd(&p.counters[1], 1);
+        if (prev == int(gridDim.x) - 1) {  // last CTA out re-arms the queue for the next launch (stream-ordered)
+            p.counters[0] = 0;
+            p.counters[1] = 0;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a5: log-sum-exp combine of split partials: out = sum_k 2^(m_k-m*) O_k / sum_k 2^(m_k-m*) l_k
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) combine_kernel(const CombineItem* __restrict__ items, const uint8_t* __restrict__ partials,
+                                                      __nv_bfloat16* __restrict__ out_dec, __nv_bfloat16* __restrict__ out_chunk,
+                                                      float* __restrict__ lse_dec, float* __restrict__ lse_chunk) {
+    const CombineItem ci = items[blockIdx.x];
+    const int kind = ci.kind_stride & 0xff, stride = ci.kind_stride >> 8;
+    __shared__ float s_mstar[kHeads], s_linv[kHeads];
+    if (threadIdx.x < kHeads) {
+        const int h = threadIdx.x;
+        float ms = -INFINITY;
+        for (int k = 0; k < ci.n_splits; ++k) {
+            const float* ml = reinterpret_cast<const float*>(partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes +
+                                                             size_t(kHeads) * kLatent * 4);
+            ms = fmaxf(ms, ml[h]);
+        }
+        float L = 0.f;
+        for (int k = 0; k < ci.n_splits; ++k) {
+            const float* ml = reinterpret_cast<const float*>(partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes +
+                                                             size_t(kHeads) * kLatent * 4);
+            const float mk = ml[h];
+            L += (mk == -INFINITY) ? 0.f : exp2f(mk - ms) * ml[kHeads + h];
+        }
+        s_mstar[h] = ms;
+        s_linv[h] = 1.f / L;
+        float* lse = kind ? lse_chunk : lse_dec;
+        if (lse) lse[size_t(ci.q_index) * kHeads + h] = (ms + log2f(L)) * kLn2;
+    }
+    __syncthreads();
+    __nv_bfloat16* out = (kind ? out_chunk : out_dec) + size_t(ci.q_index) * kHeads * kLatent;
+    for (int e = threadIdx.x; e < kHeads * kLatent; e += 256) {
+        const int h = e / kLatent;
+        float acc = 0.f;
+        for (int k = 0; k < ci.n_splits; ++k) {
+            const uint8_t* slot = partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes;
+            const float mk = reinterpret_cast<const float*>(slot + size_t(kHeads) * kLatent * 4)[h];
+            const float wk = (mk == -INFINITY) ? 0.f : exp2f(mk - s_mstar[h]);
+            acc += wk * reinterpret_cast<const float*>(slot)[e];
+        }
+        out[e] = __float2bfloat16_rn(acc * s_linv[h]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+int encode_rows_map(CUtensorMap* map, const void* ptr, uint64_t rows, uint32_t box_rows) {
+    cuuint64_t dims[2] = {cuuint64_t(kDim), rows};
+    cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
+    cuuint32_t box[2] = {64, box_rows};
+    cuuint32_t es[2] = {1, 1};
+    CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: " + std::to_string(int(r)));
+    return KAIROS_OK;
+}
+
+}  // namespace
+
+int umma_chunk_tile_tokens() { return kChunkTileTokens; }
 int umma_resident_ctas(const kairos_ctx* ctx) { return ctx->sm_count; }
-int umma_init(kairos_ctx*) { return KAIROS_OK; }
-int launch_attn_umma(kairos_ctx*, const StepArgs&, const WorkItem*, int32_t, const CombineItem*, int32_t, cudaStream_t, int*) {
-    return fail(KAIROS_ERR_UNSUPPORTED, "tcgen05 path not built yet");
+
+int umma_init(kairos_ctx* ctx) {
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        KAIROS_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    // pool viewed as [chunk 9][row num_pages*64][64 elems]: one box = one page as [9][64][128 B]
+    cuuint64_t dims[3] = {64, cuuint64_t(ctx->cfg.num_pages) * kPage, 9};
+    cuuint64_t strides[2] = {cuuint64_t(kTokenBytes), 128};
+    cuuint32_t box[3] = {64, 64, 9};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = g_encode(&ctx->pool_map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->cfg.pool, dims, strides, box, es,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed: " + std::to_string(int(r)));
+    ctx->has_pool_map = true;
+    KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    KAIROS_CUDA_TRY(cudaMemset(ctx->cfg.workspace, 0, 256));  // work-queue counters
+    return KAIROS_OK;
 }
+
+int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
+                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched) {
+    CUtensorMap qd_map = ctx->pool_map, qc_map = ctx->pool_map;  // placeholders when a side is empty (never dereferenced)
+    if (a.n_dec > 0)
+        if (int rc = encode_rows_map(&qd_map, a.q_dec, uint64_t(a.n_dec) * kHeads, 16)) return rc;
+    if (a.chunk_len > 0)
+        if (int rc = encode_rows_map(&qc_map, a.q_chunk, uint64_t(a.chunk_len) * kHeads, 64)) return rc;
+    KParams p;
+    p.items = dev_items;
+    p.n_items = n_items;
+    p.counters = reinterpret_cast<int32_t*>(ctx->cfg.workspace);
+    p.dec_pt = a.dec_page_tables;
+    p.dec_stride = a.dec_table_stride;
+    p.chunk_pt = a.chunk_page_table;
+    p.out_dec = reinterpret_cast<__nv_bfloat16*>(a.out_dec);
+    p.out_chunk = reinterpret_cast<__nv_bfloat16*>(a.out_chunk);
+    p.lse_dec = a.lse_dec;
+    p.lse_chunk = a.lse_chunk;
+    p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
+    p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
+    const int grid = std::min(n_items, umma_resident_ctas(ctx));
+    kairos_mixed_kernel<<<grid, kThreads, kSmemBytes, stream>>>(ctx->pool_map, qd_map, qc_map, p);
+    KAIROS_CUDA_TRY(cudaGetLastError());
+    *kernels_launched = 1;
+    if (n_combines > 0) {
+        combine_kernel<<<n_combines, 256, 0, stream>>>(dev_combines, p.partials, p.out_dec, p.out_chunk, p.lse_dec, p.lse_chunk);
+        KAIROS_CUDA_TRY(cudaGetLastError());
+        *kernels_launched = 2;
+    }
+    return KAIROS_OK;
 }
+
+}  // namespace kairos
