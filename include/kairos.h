@@ -168,6 +168,15 @@ int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int32_t nB, co
  * by that call, [5] = workspace bytes used.  n = number of int64 slots available in info. */
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
 
+/*
+ * Kernel-level timing for the roofline leg of bench.py.  While enabled, kairos_mixed_step brackets the launch of
+ * its main (persistent attention) kernel with a pair of CUDA events on the caller's stream.  kairos_profile_read
+ * synchronises the recorded events, returns the summed main-kernel device time in microseconds and the number of
+ * launches since the last read (HOST pointers, either may be NULL), and clears the record.
+ */
+int kairos_profile_enable(kairos_ctx* ctx, int32_t on);
+int kairos_profile_read(kairos_ctx* ctx, double* main_kernel_us_total, int64_t* launches);
+
 /* Message for the last failing call on this thread ("" if none). Never NULL. */
 const char* kairos_last_error(void);
 

@@ -1,5 +1,7 @@
 // C-ABI entry points of libkairos.so (include/kairos.h): argument validation, host planner, staging, launches.
 #include <algorithm>
+#include <chrono>
+#include <cstdio>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -93,6 +95,11 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     }
 
     // ---- impl 1: plan -> staging -> persistent kernel (+ combine)
+    static const bool dbg = std::getenv("KAIROS_DEBUG_TIMING") != nullptr;
+    static double t_plan = 0, t_stage = 0, t_copy = 0, t_launch = 0; static long n_calls = 0;
+    auto now = [] { return std::chrono::steady_clock::now(); };
+    auto us = [](auto a, auto b) { return std::chrono::duration<double, std::micro>(b - a).count(); };
+    auto T0 = now();
     Plan& plan = ctx->plan;
     build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, umma_resident_ctas(ctx), umma_chunk_tile_tokens(), &plan);
     const size_t ws_needed = kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes;
@@ -102,16 +109,26 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     const size_t comb_bytes = plan.combines.size() * sizeof(CombineItem);
     const size_t comb_off = (items_bytes + 255) / 256 * 256;
     StagingSlot* st = nullptr;
+    auto T1 = now();
     if (int rc = staging_acquire(ctx, comb_off + comb_bytes + 256, &st)) return rc;
+    auto T2 = now();
     std::memcpy(st->host, plan.items.data(), items_bytes);
     if (comb_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + comb_off, plan.combines.data(), comb_bytes);
     KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, comb_off + comb_bytes, cudaMemcpyHostToDevice, stream));
     KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
+    auto T3 = now();
     int kernels = 0;
     if (int rc = launch_attn_umma(ctx, a, reinterpret_cast<const WorkItem*>(st->dev), int32_t(plan.items.size()),
                                   reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
                                   int32_t(plan.combines.size()), stream, &kernels))
         return rc;
+    if (dbg) {
+        auto T4 = now();
+        t_plan += us(T0, T1); t_stage += us(T1, T2); t_copy += us(T2, T3); t_launch += us(T3, T4);
+        if (++n_calls % 500 == 0)
+            std::fprintf(stderr, "[kairos host us/call] plan %.1f staging_wait %.1f copy+record %.1f encode+launch %.1f\n",
+                         t_plan / n_calls, t_stage / n_calls, t_copy / n_calls, t_launch / n_calls);
+    }
     ctx->last_info[0] = int64_t(plan.items.size());
     ctx->last_info[1] = plan.n_decode_items;
     ctx->last_info[2] = plan.n_chunk_items;
@@ -179,6 +196,7 @@ int kairos_destroy(kairos_ctx* ctx) {
         if (s.done) cudaEventDestroy(s.done);
     }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
+    for (auto e : ctx->prof_events) cudaEventDestroy(e);
     delete ctx;
     return KAIROS_OK;
 }
@@ -309,6 +327,27 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n) {
     if (!ctx || !info || n < 0) return fail(KAIROS_ERR_INVALID_ARG, "NULL argument");
     for (int32_t i = 0; i < n && i < 6; ++i) info[i] = ctx->last_info[i];
+    return KAIROS_OK;
+}
+
+int kairos_profile_enable(kairos_ctx* ctx, int32_t on) {
+    if (int rc = check_ctx(ctx)) return rc;
+    ctx->profile = on != 0;
+    return KAIROS_OK;
+}
+
+int kairos_profile_read(kairos_ctx* ctx, double* main_kernel_us_total, int64_t* launches) {
+    if (int rc = check_ctx(ctx)) return rc;
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < ctx->prof_used; i += 2) {
+        KAIROS_CUDA_TRY(cudaEventSynchronize(ctx->prof_events[i + 1]));
+        float ms = 0.f;
+        KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, ctx->prof_events[i], ctx->prof_events[i + 1]));
+        total += double(ms) * 1e3;
+    }
+    if (main_kernel_us_total) *main_kernel_us_total = total;
+    if (launches) *launches = int64_t(ctx->prof_used / 2);
+    ctx->prof_used = 0;
     return KAIROS_OK;
 }
 

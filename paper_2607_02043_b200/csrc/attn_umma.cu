@@ -44,6 +44,7 @@ constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64
 constexpr uint32_t kColO = 128;  // O^T blocks at 128 + 64*b
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the max grows by more than 2^8
 constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
 
 struct Small {
     uint64_t q_full, q_empty, kv_full[2], kv_empty[2], s_full[2], s_empty[2], p_full, pv_done, o_full, o_empty;
@@ -51,14 +52,21 @@ struct Small {
     int32_t item_ring[2];
     uint32_t tmem_base;
     uint32_t pad;
-    float m_ref[64];   // running reference max per query row (log2 domain); -inf while nothing visible yet
+    float m_ref[64];   // running reference max per query row (log2 domain); -1e30 while nothing visible yet
     float alpha[64];   // O / l rescale factor decided for the current page
     float red[4][64];  // per-warp column maxima (per page) / column sums (epilogue)
     float linv[64];
 };
 static_assert(sizeof(Small) <= kSmallBytes, "Small does not fit");
 
+#ifdef KAIROS_TRACE
+#define KTRACE(ev, g) do { if (blockIdx.x == 0 && (g) < 64) p.trace[(ev) * 64 + (g)] = clock64(); } while (0)
+#else
+#define KTRACE(ev, g) do { } while (0)
+#endif
+
 struct KParams {
+    unsigned long long* trace;
     const WorkItem* items;
     int32_t n_items;
     int32_t* counters;  // [0] queue head, [1] finished CTAs
@@ -133,12 +141,14 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
     float l[N];
 #pragma unroll
     for (int c = 0; c < N; ++c) l[c] = 0.f;
-    if (tid_s < N) sm->m_ref[tid_s] = -INFINITY;  // owner thread; others read it only after the named barriers below
+    if (tid_s < N) sm->m_ref[tid_s] = kMinusHuge;  // owner thread writes; the item barrier below orders the readers
+    named_sync(1);
 
     const int npages = w.page_end - w.page_begin;
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const int b = g & 1;
         mbar_wait(&sm->s_full[b], (g >> 1) & 1);
+        if (tid_s == 0) KTRACE(5, g);
         tc_fence_after();
         float x[N];
 #pragma unroll
@@ -148,6 +158,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->s_empty[b]);
+        if (tid_s == 0) KTRACE(6, g);
 
         const int page = w.page_begin + pg;
         const int key_pos = page * kPage + tok_in_page;
@@ -158,50 +169,54 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
             const bool ok = lane_ok && (!boundary || key_pos < w.n_keys + (N == 64 ? (c >> 4) : 0));
             x[c] = ok ? v : -INFINITY;
         }
-        // column (query-row) max over the 64 keys of the page: warp redux, then 4 warps through smem
+        // Lazy running max: the per-row maximum is refreshed only when some key of this page exceeds the row's
+        // reference by more than 2^kRescaleThreshold (always on the first page, where m_ref = -1e30).  The common
+        // path costs one subtraction + max per value and a single bar.red.or over the 128 softmax threads.
+        float dmax = -INFINITY;
 #pragma unroll
-        for (int c = 0; c < N; ++c) {
-            const float wm = warp_max(x[c]);
-            if (lane == (c & 31)) sm->red[w4][c] = wm;
-        }
-        named_sync(1);
-        bool need = false;
-        if (tid_s < N) {
-            const float tm = fmaxf(fmaxf(sm->red[0][tid_s], sm->red[1][tid_s]), fmaxf(sm->red[2][tid_s], sm->red[3][tid_s]));
-            const float mo = sm->m_ref[tid_s];
-            float mn = mo, a = 1.f;
-            if (tm > mo + kRescaleThreshold) {  // also true for mo = -inf and finite tm
-                mn = tm;
-                if (mo != -INFINITY) { a = ex2(mo - mn); need = true; }
-            }
-            sm->m_ref[tid_s] = mn;
-            sm->alpha[tid_s] = a;
-        }
-        const bool rescale = named_or(2, need);
+        for (int c = 0; c < N; ++c) dmax = fmaxf(dmax, x[c] - sm->m_ref[c]);
+        const bool need = named_or(2, dmax > kRescaleThreshold);
+        if (tid_s == 0) KTRACE(7, g);
         if (g > 0) mbar_wait(&sm->pv_done, (g - 1) & 1);  // PV of the previous page done: P buffer free, O stable
-        if (rescale) {
-            tc_fence_after();
+        if (tid_s == 0) KTRACE(8, g);
+        if (need) {
+            // exact column (query-row) max over the 64 keys of the page: warp redux, then 4 warps through smem
 #pragma unroll
-            for (int b4 = 0; b4 < 4; ++b4)
+            for (int c = 0; c < N; ++c) {
+                const float wm = warp_max(x[c]);
+                if (lane == (c & 31)) sm->red[w4][c] = wm;
+            }
+            named_sync(1);
+            if (tid_s < N) {
+                const float tm = fmaxf(fmaxf(sm->red[0][tid_s], sm->red[1][tid_s]), fmaxf(sm->red[2][tid_s], sm->red[3][tid_s]));
+                const float mo = sm->m_ref[tid_s];
+                const float mn = fmaxf(mo, tm);
+                sm->m_ref[tid_s] = mn;
+                sm->alpha[tid_s] = ex2(mo - mn);  // 1 if unchanged, 0 if nothing had been visible before
+            }
+            named_sync(1);
+            if (pg > 0) {  // O^T and l hold data relative to the old reference: rescale (rare)
+                tc_fence_after();
 #pragma unroll
-                for (int c0 = 0; c0 < N; c0 += 16) {
-                    uint32_t r[16];
-                    const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0);
-                    tmem_ld16(ta, r);
-                    tmem_wait_ld();
+                for (int b4 = 0; b4 < 4; ++b4)
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[c0 + i]);
-                    tmem_st16(ta, r);
-                }
-            tmem_wait_st();
+                    for (int c0 = 0; c0 < N; c0 += 16) {
+                        uint32_t r[16];
+                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0);
+                        tmem_ld16(ta, r);
+                        tmem_wait_ld();
 #pragma unroll
-            for (int c = 0; c < N; ++c) l[c] *= sm->alpha[c];
+                        for (int i = 0; i < 16; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[c0 + i]);
+                        tmem_st16(ta, r);
+                    }
+                tmem_wait_st();
+#pragma unroll
+                for (int c = 0; c < N; ++c) l[c] *= sm->alpha[c];
+            }
         }
 #pragma unroll
         for (int c = 0; c < N; ++c) {
-            float m = sm->m_ref[c];
-            m = (m == -INFINITY) ? 0.f : m;
-            const float pv = ex2(x[c] - m);
+            const float pv = ex2(x[c] - sm->m_ref[c]);
             l[c] += pv;
             x[c] = pv;
         }
@@ -220,6 +235,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->p_full);
+        if (tid_s == 0) KTRACE(9, g);
     }
 
     // ---- epilogue: all PV MMAs of the item are complete
@@ -278,6 +294,69 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->o_empty);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// MMA issue for one work item (whole warp, converged).  S(s) may run one page ahead of PV; PV has priority as soon
+// as its P^T is ready, because its completion releases the KV stage to the TMA producer.
+// ------------------------------------------------------------------------------------------------------------
+template <int N>
+__device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base, uint32_t p_base,
+                                         int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p) {
+    constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
+    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
+    mbar_wait(&sm->q_full, it & 1);
+    int s_next = 0, pv_next = 0;
+    uint32_t spins = 0;
+    while (pv_next < npages) {
+        if (pv_next < s_next) {
+            const uint32_t gg = g0 + pv_next;
+            const bool ready = __any_sync(0xffffffffu, mbar_try_wait(&sm->p_full, gg & 1));
+            if (ready || s_next == npages) {
+                if (!ready) mbar_wait(&sm->p_full, gg & 1);
+                if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
+                KTRACE(3, gg);
+                tc_fence_after();
+                const uint32_t st = gg & 1, a0 = kv_base + st * kStageBytes;
+#pragma unroll
+                for (uint32_t b4 = 0; b4 < 4; ++b4)
+#pragma unroll
+                    for (uint32_t ks = 0; ks < 4; ++ks)
+                        umma_bf16_ss(tmem + kColO + b4 * 64, make_smem_desc(a0 + (2 * b4) * 8192 + ks * 2048, 8192, 1024),
+                                     make_smem_desc(p_base + ks * 2048, 8192, 1024), idesc_o, (pv_next > 0 || ks > 0), leader);
+                umma_commit(&sm->kv_empty[st], leader);
+                umma_commit(&sm->pv_done, leader);
+                if (pv_next == npages - 1) umma_commit(&sm->o_full, leader);
+                KTRACE(4, gg);
+                ++pv_next;
+                spins = 0;
+                continue;
+            }
+        }
+        if (s_next < npages && s_next <= pv_next + 1) {
+            const uint32_t gg = g0 + s_next;
+            const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
+            if (__any_sync(0xffffffffu, mbar_try_wait(&sm->kv_full[st], ph))) {
+                KTRACE(1, gg);
+                mbar_wait(&sm->s_empty[st], ph ^ 1);
+                tc_fence_after();
+                const uint32_t a0 = kv_base + st * kStageBytes;
+#pragma unroll
+                for (uint32_t c = 0; c < 9; ++c)
+#pragma unroll
+                    for (uint32_t j = 0; j < 4; ++j)
+                        umma_bf16_ss(tmem + kColS + st * 64, make_smem_desc(a0 + c * 8192 + j * 32, 16, 1024),
+                                     make_smem_desc(q_base + c * N * 128 + j * 32, 16, 1024), idesc_s, (c | j) != 0, leader);
+                umma_commit(&sm->s_full[st], leader);
+                ++s_next;
+                if (s_next == npages) umma_commit(&sm->q_empty, leader);  // Q tile free once every S-MMA retires
+                KTRACE(2, gg);
+                spins = 0;
+                continue;
+            }
+        }
+        if (++spins > (1u << 26)) __trap();
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -351,6 +430,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
                     if (lane == 0) {
                         const int st = g & 1;
                         mbar_wait(&sm->kv_empty[st], ((g >> 1) & 1) ^ 1);
+                        KTRACE(0, g);
                         mbar_arrive_expect_tx(&sm->kv_full[st], kStageBytes);
                         tma_load_page(base + kOffKV + st * kStageBytes, &pool_map, &sm->kv_full[st], pid * kPage, policy);
                     }
@@ -358,56 +438,23 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             }
         }
     } else if (warp == 1) {
-        // ================= MMA issuer (one lane) =================
-        if (lane == 0) {
-            const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV), p_base = smem_u32(base + kOffP);
-            uint32_t g = 0;
-            for (uint32_t it = 0;; ++it) {
-                mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
-                const int idx = sm->item_ring[it & 1];
-                mbar_arrive(&sm->item_empty[it & 1]);
-                if (idx < 0) break;
-                const WorkItem w = load_item(p.items + idx);
-                const uint32_t N = w.kind ? 64 : 16;
-                const uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);
-                const uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);
-                const int npages = w.page_end - w.page_begin;
-                mbar_wait(&sm->q_full, it & 1);
-                auto issue_s = [&](uint32_t gg) {
-                    const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
-                    mbar_wait(&sm->kv_full[st], ph);
-                    mbar_wait(&sm->s_empty[st], ph ^ 1);
-                    tc_fence_after();
-                    const uint32_t a0 = kv_base + st * kStageBytes;
-#pragma unroll 1
-                    for (uint32_t c = 0; c < 9; ++c)
-#pragma unroll
-                        for (uint32_t j = 0; j < 4; ++j)
-                            umma_bf16_ss(tmem + kColS + st * 64, make_smem_desc(a0 + c * 8192 + j * 32, 16, 1024),
-                                         make_smem_desc(q_base + c * N * 128 + j * 32, 16, 1024), idesc_s, (c | j) != 0);
-                    umma_commit(&sm->s_full[st]);
-                };
-                issue_s(g);
-                for (int pg = 0; pg < npages; ++pg) {
-                    const uint32_t gg = g + pg;
-                    if (pg + 1 < npages) issue_s(gg + 1);
-                    else umma_commit(&sm->q_empty);  // every S-MMA of the item issued: Q tile free once they retire
-                    if (pg == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
-                    mbar_wait(&sm->p_full, gg & 1);
-                    tc_fence_after();
-                    const uint32_t st = gg & 1, a0 = kv_base + st * kStageBytes;
-#pragma unroll 1
-                    for (uint32_t b4 = 0; b4 < 4; ++b4)
-#pragma unroll
-                        for (uint32_t ks = 0; ks < 4; ++ks)
-                            umma_bf16_ss(tmem + kColO + b4 * 64, make_smem_desc(a0 + (2 * b4) * 8192 + ks * 2048, 8192, 1024),
-                                         make_smem_desc(p_base + ks * 2048, 8192, 1024), idesc_o, (pg > 0 || ks > 0));
-                    umma_commit(&sm->kv_empty[st]);
-                    umma_commit(&sm->pv_done);
-                }
-                umma_commit(&sm->o_full);
-                g += npages;
-            }
+        // ================= MMA issuer: the whole warp runs converged, one elected lane issues =================
+        const uint32_t leader = elect_one();
+        const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV), p_base = smem_u32(base + kOffP);
+        uint32_t g = 0;
+        for (uint32_t it = 0;; ++it) {
+            mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
+            const int idx = __shfl_sync(0xffffffffu, sm->item_ring[it & 1], 0);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
+            __syncwarp();
+            if (idx < 0) break;
+            const WorkItem w = load_item(p.items + idx);
+            const int kind = __shfl_sync(0xffffffffu, w.kind, 0);
+            const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
+            if (kind) mma_item<64>(sm, tmem, q_base, kv_base, p_base, npages, g, it, leader, p);
+            else mma_item<16>(sm, tmem, q_base, kv_base, p_base, npages, g, it, leader, p);
+            g += npages;
         }
     } else {
         // ================= softmax / correction / epilogue warps =================
@@ -446,41 +493,71 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
 __global__ void __launch_bounds__(256) combine_kernel(const CombineItem* __restrict__ items, const uint8_t* __restrict__ partials,
                                                       __nv_bfloat16* __restrict__ out_dec, __nv_bfloat16* __restrict__ out_chunk,
                                                       float* __restrict__ lse_dec, float* __restrict__ lse_chunk) {
+    constexpr int kMaxK = 32;  // splits whose weights are staged in shared memory per pass
     const CombineItem ci = items[blockIdx.x];
     const int kind = ci.kind_stride & 0xff, stride = ci.kind_stride >> 8;
-    __shared__ float s_mstar[kHeads], s_linv[kHeads];
-    if (threadIdx.x < kHeads) {
-        const int h = threadIdx.x;
-        float ms = -INFINITY;
-        for (int k = 0; k < ci.n_splits; ++k) {
-            const float* ml = reinterpret_cast<const float*>(partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes +
-                                                             size_t(kHeads) * kLatent * 4);
-            ms = fmaxf(ms, ml[h]);
+    __shared__ float s_m[kMaxK][kHeads], s_w[kMaxK][kHeads], s_mstar[kHeads], s_linv[kHeads];
+    const int tid = threadIdx.x;
+    auto slot_ptr = [&](int k) { return partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes; };
+    // pass 1: m* per head over all splits
+    if (tid < kHeads) {
+        float ms = kMinusHuge;
+        for (int k = 0; k < ci.n_splits; ++k)
+            ms = fmaxf(ms, reinterpret_cast<const float*>(slot_ptr(k) + size_t(kHeads) * kLatent * 4)[tid]);
+        s_mstar[tid] = ms;
+    }
+    __syncthreads();
+    // each thread owns 8 consecutive outputs of 4 (head, d) groups: e = (tid + 256*i) * 8 ... covers 16*512 = 8192
+    float acc[4][8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    float L = 0.f;  // threads < 16 accumulate the denominator of their head
+    for (int k0 = 0; k0 < ci.n_splits; k0 += kMaxK) {
+        const int kn = min(kMaxK, ci.n_splits - k0);
+        for (int i = tid; i < kn * kHeads; i += 256) {
+            const int k = i / kHeads, h = i % kHeads;
+            const float* ml = reinterpret_cast<const float*>(slot_ptr(k0 + k) + size_t(kHeads) * kLatent * 4);
+            const float w = exp2f(ml[h] - s_mstar[h]);  // m = -1e30 (nothing visible) -> 0
+            s_w[k][h] = w;
+            s_m[k][h] = w * ml[kHeads + h];
         }
-        float L = 0.f;
-        for (int k = 0; k < ci.n_splits; ++k) {
-            const float* ml = reinterpret_cast<const float*>(partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes +
-                                                             size_t(kHeads) * kLatent * 4);
-            const float mk = ml[h];
-            L += (mk == -INFINITY) ? 0.f : exp2f(mk - ms) * ml[kHeads + h];
+        __syncthreads();
+        if (tid < kHeads)
+            for (int k = 0; k < kn; ++k) L += s_m[k][tid];
+#pragma unroll 4
+        for (int k = 0; k < kn; ++k) {
+            const float4* src = reinterpret_cast<const float4*>(slot_ptr(k0 + k));
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int v = (tid + 256 * i) * 2;  // float4 index; 8 floats = 2 float4
+                const int h = (v * 4) / kLatent;
+                const float w = s_w[k][h];
+                const float4 a = __ldg(src + v), b = __ldg(src + v + 1);
+                acc[i][0] += w * a.x; acc[i][1] += w * a.y; acc[i][2] += w * a.z; acc[i][3] += w * a.w;
+                acc[i][4] += w * b.x; acc[i][5] += w * b.y; acc[i][6] += w * b.z; acc[i][7] += w * b.w;
+            }
         }
-        s_mstar[h] = ms;
-        s_linv[h] = 1.f / L;
+        __syncthreads();
+    }
+    if (tid < kHeads) {
+        s_linv[tid] = 1.f / L;
         float* lse = kind ? lse_chunk : lse_dec;
-        if (lse) lse[size_t(ci.q_index) * kHeads + h] = (ms + log2f(L)) * kLn2;
+        if (lse) lse[size_t(ci.q_index) * kHeads + tid] = (s_mstar[tid] + log2f(L)) * kLn2;
     }
     __syncthreads();
     __nv_bfloat16* out = (kind ? out_chunk : out_dec) + size_t(ci.q_index) * kHeads * kLatent;
-    for (int e = threadIdx.x; e < kHeads * kLatent; e += 256) {
-        const int h = e / kLatent;
-        float acc = 0.f;
-        for (int k = 0; k < ci.n_splits; ++k) {
-            const uint8_t* slot = partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes;
-            const float mk = reinterpret_cast<const float*>(slot + size_t(kHeads) * kLatent * 4)[h];
-            const float wk = (mk == -INFINITY) ? 0.f : exp2f(mk - s_mstar[h]);
-            acc += wk * reinterpret_cast<const float*>(slot)[e];
-        }
-        out[e] = __float2bfloat16_rn(acc * s_linv[h]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int e = (tid + 256 * i) * 8;
+        const float inv = s_linv[e / kLatent];
+        uint4 o;
+        o.x = pack_bf16(acc[i][0] * inv, acc[i][1] * inv);
+        o.y = pack_bf16(acc[i][2] * inv, acc[i][3] * inv);
+        o.z = pack_bf16(acc[i][4] * inv, acc[i][5] * inv);
+        o.w = pack_bf16(acc[i][6] * inv, acc[i][7] * inv);
+        *reinterpret_cast<uint4*>(out + e) = o;
     }
 }
 
@@ -538,6 +615,8 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     if (a.chunk_len > 0)
         if (int rc = encode_rows_map(&qc_map, a.q_chunk, uint64_t(a.chunk_len) * kHeads, 64)) return rc;
     KParams p;
+    p.trace = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctx->cfg.workspace) +
+                                                    ctx->cfg.workspace_bytes - 8192);  // KAIROS_TRACE builds only
     p.items = dev_items;
     p.n_items = n_items;
     p.counters = reinterpret_cast<int32_t*>(ctx->cfg.workspace);
@@ -551,8 +630,23 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
     const int grid = std::min(n_items, umma_resident_ctas(ctx));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->profile) {
+        if (ctx->prof_used + 2 > ctx->prof_events.size()) {
+            for (int i = 0; i < 2; ++i) {
+                cudaEvent_t e;
+                KAIROS_CUDA_TRY(cudaEventCreate(&e));
+                ctx->prof_events.push_back(e);
+            }
+        }
+        e0 = ctx->prof_events[ctx->prof_used];
+        e1 = ctx->prof_events[ctx->prof_used + 1];
+        ctx->prof_used += 2;
+        KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
+    }
     kairos_mixed_kernel<<<grid, kThreads, kSmemBytes, stream>>>(ctx->pool_map, qd_map, qc_map, p);
     KAIROS_CUDA_TRY(cudaGetLastError());
+    if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
     *kernels_launched = 1;
     if (n_combines > 0) {
         combine_kernel<<<n_combines, 256, 0, stream>>>(dev_combines, p.partials, p.out_dec, p.out_chunk, p.lse_dec, p.lse_chunk);

@@ -95,6 +95,9 @@ struct kairos_ctx {
     kairos::HostStage host_stage;
     kairos::Plan plan;            // reused per call
     int64_t last_info[6] = {0, 0, 0, 0, 0, 0};
+    bool profile = false;         // bracket the main kernel with events (kairos_profile_enable)
+    std::vector<cudaEvent_t> prof_events;  // pairs: [2i] start, [2i+1] stop
+    size_t prof_used = 0;         // events in use since the last kairos_profile_read
 };
 
 namespace kairos {

@@ -54,6 +54,10 @@ _lib.kairos_step_latency_table.argtypes = [_vp, _vp, _i32, _vp, _i32, _vp, _i32,
 _lib.kairos_step_latency_table.restype = _c.c_int
 _lib.kairos_last_plan_info.argtypes = [_vp, _vp, _i32]
 _lib.kairos_last_plan_info.restype = _c.c_int
+_lib.kairos_profile_enable.argtypes = [_vp, _i32]
+_lib.kairos_profile_enable.restype = _c.c_int
+_lib.kairos_profile_read.argtypes = [_vp, _vp, _vp]
+_lib.kairos_profile_read.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
 _lib.kairos_last_error.restype = _c.c_char_p
 _lib.kairos_version.argtypes = []
@@ -61,7 +65,7 @@ _lib.kairos_version.restype = _c.c_char_p
 
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
-           "kairos_step_latency_table", "kairos_last_plan_info", "kairos_last_error", "kairos_version"]
+           "kairos_step_latency_table", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
           -4: "KAIROS_ERR_CUDA"}
@@ -94,8 +98,9 @@ def _dp(t: Optional[torch.Tensor]) -> Optional[int]:
 
 
 def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> Optional[int]:
-    s = torch.cuda.current_stream() if stream is None else stream
-    return s.cuda_stream or None
+    if stream is None:  # torch's current stream on the current device, through the fast C accessor
+        return torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()) or None
+    return stream.cuda_stream or None
 
 
 class Kairos:
@@ -194,6 +199,15 @@ class Kairos:
                                               int(warmup), int(reps), int(bool(flush_l2)), med.ctypes.data_as(_vp),
                                               mn.ctypes.data_as(_vp), _stream_ptr(stream)))
         return med, mn
+
+    def profile_enable(self, on: bool) -> None:
+        _check(_lib.kairos_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self):
+        """(summed main-kernel microseconds, launches) since the last read; synchronises the recorded events."""
+        us, n = _c.c_double(0.0), _c.c_int64(0)
+        _check(_lib.kairos_profile_read(self._h, _c.byref(us), _c.byref(n)))
+        return float(us.value), int(n.value)
 
     def last_plan_info(self) -> dict:
         info = (_c.c_int64 * 6)()
