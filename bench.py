@@ -165,6 +165,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2607_02043_b200 import kairos as K  # raises if libkairos.so is missing: no fallback
+    from paper_2607_02043_b200 import replicas as R_
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
@@ -173,7 +174,7 @@ def main():
     dev = torch.device("cuda", local_rank)
     peaks = load_peaks()
 
-    inp = make_workload(args.config, args.chunk, seed_shift=rank)
+    inp = make_workload(args.config, args.chunk, seed_shift=R_.replica_seed_shift(rank))
     alg_bytes, alg_flops = inp.algorithmic_bytes(), inp.algorithmic_flops()
     pool_bytes = inp.pool.nbytes
     step_touch = pool_bytes + inp.q_dec.nbytes + inp.q_chunk.nbytes
@@ -246,11 +247,8 @@ def main():
     ms_prof, kern_us, kern_n = timed_region(args.steps, profile=True)
     clocks = sampler.stop()
 
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    us_per_step = ms_max * 1e3 / (args.steps * world)  # whole-job: world replicas advance one step each per iteration
+    ms_max = R_.max_over_ranks(ms, dev)
+    us_per_step = R_.whole_job_us_per_step(ms, args.steps, world, dev)  # world replicas advance one step per iteration
 
     # ---- end-to-end leg: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
     R = reps[0]
@@ -270,10 +268,7 @@ def main():
                                                inp.prefix_len, h_od, h_oc)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_us = float(te.item()) * 1e6 / (e2e_steps * world)
+    e2e_us = R_.max_over_ranks(e2e_s, dev) * 1e6 / (e2e_steps * world)
 
     if rank != 0:
         if world > 1:
