@@ -26,17 +26,21 @@ namespace kairos {
 namespace {
 using namespace ptx;
 
-constexpr int kThreads = 192;
+constexpr int kSoftmaxWarps = 8;                 // 2 per TMEM lane quadrant: each takes half of the query-row columns
+constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
+constexpr int kThreads = 64 + kSoftmaxThreads;    // warp 0 producer, warp 1 MMA issuer, warps 2-9 softmax
 constexpr int kChunkTileTokens = 4;
 constexpr int kStageBytes = kPage * kTokenBytes;  // 73,728: one page
 constexpr int kQBytes = 64 * kTokenBytes;         // 73,728: up to 64 query rows
-constexpr int kPBytes = 64 * 64 * 2;              // 8,192: P^T [64 keys][<=64 rows] bf16
 constexpr int kOffQ = 0;
 constexpr int kOffKV = kQBytes;
-constexpr int kOffP = kOffKV + 2 * kStageBytes;
-constexpr int kOffSmall = kOffP + kPBytes;        // 229,376
+// P^T [64 keys][<=64 rows] bf16 (8 KB) lives in the RoPE chunk (chunk 8) of its own KV stage: that chunk is only
+// read by the S MMAs, which have completed before the softmax of the page starts, and the stage is not reloaded
+// until the PV MMAs that read P^T have completed.  One P^T per stage = free double buffering, no extra SMEM.
+constexpr int kOffPInStage = 8 * 8192;
+constexpr int kOffSmall = kOffKV + 2 * kStageBytes;  // 221,184
 constexpr int kSmallBytes = 2048;
-constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;  // + alignment slack = 232,448 = the 227 KB limit
+constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;  // + alignment slack
 static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
 
 constexpr uint32_t kTmemCols = 512;
@@ -47,7 +51,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
 
 struct Small {
-    uint64_t q_full, q_empty, kv_full[2], kv_empty[2], s_full[2], s_empty[2], p_full, pv_done, o_full, o_empty;
+    uint64_t q_full, q_empty, kv_full[2], kv_empty[2], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -110,16 +114,16 @@ __device__ __forceinline__ float warp_max(float v) {
     asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
     return r;
 }
-__device__ __forceinline__ void named_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void named_sync(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(kSoftmaxThreads) : "memory"); }
 __device__ __forceinline__ bool named_or(int id, bool pred) {
     uint32_t r;
     asm volatile(
         "{\n\t.reg .pred p, q;\n\t"
         "setp.ne.u32 p, %1, 0;\n\t"
-        "bar.red.or.pred q, %2, 128, p;\n\t"
+        "bar.red.or.pred q, %2, %3, p;\n\t"
         "selp.u32 %0, 1, 0, q;\n\t}"
         : "=r"(r)
-        : "r"(uint32_t(pred)), "r"(id)
+        : "r"(uint32_t(pred)), "r"(id), "n"(kSoftmaxThreads)
         : "memory");
     return r != 0;
 }
@@ -130,17 +134,23 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// softmax / correction / epilogue for one work item; N = 16 (decode) or 64 (chunk tile) query rows
+// softmax / correction / epilogue for one work item; N = 16 (decode) or 64 (chunk tile) query rows.
+// 8 warps: warp sw works on TMEM lane quadrant sw & 3 (16 of its lanes hold the M=64 accumulator rows = keys) and on
+// the column half sw >> 2 (N/2 query rows).
 // ------------------------------------------------------------------------------------------------------------
 template <int N>
-__device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkItem& w, const KParams& p, uint32_t tmem,
-                                             int w4, int lane, uint32_t& g, uint32_t it) {
-    const int tid_s = w4 * 32 + lane;
+__device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkItem& w, const KParams& p, uint32_t tmem,
+                                             int sw, int lane, uint32_t& g, uint32_t it) {
+    constexpr int NC = N / 2;            // columns of this warp
+    constexpr int W = NC < 16 ? NC : 16;  // columns per tcgen05.ld
+    const int w4 = (sw + 2) & 3;         // TMEM lane quadrant of CTA warp 2 + sw (a warp may only touch lanes 32*(warp%4)..)
+    const int cbase = (sw >> 2) * NC;
+    const int tid_s = sw * 32 + lane;
     const bool lane_ok = lane < 16;       // M=64 accumulator rows live in lanes 0..15 of each quadrant
     const int tok_in_page = w4 * 16 + lane;
-    float l[N];
+    float l[NC];
 #pragma unroll
-    for (int c = 0; c < N; ++c) l[c] = 0.f;
+    for (int c = 0; c < NC; ++c) l[c] = 0.f;
     if (tid_s < N) sm->m_ref[tid_s] = kMinusHuge;  // owner thread writes; the item barrier below orders the readers
     named_sync(1);
 
@@ -150,10 +160,10 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
         mbar_wait(&sm->s_full[b], (g >> 1) & 1);
         if (tid_s == 0) KTRACE(5, g);
         tc_fence_after();
-        float x[N];
+        float x[NC];
 #pragma unroll
-        for (int c0 = 0; c0 < N; c0 += 16)
-            tmem_ld16(tmem_addr(tmem, w4 * 32, kColS + b * 64 + c0), *reinterpret_cast<uint32_t(*)[16]>(&x[c0]));
+        for (int c0 = 0; c0 < NC; c0 += W)
+            tmem_ldw<W>(tmem_addr(tmem, w4 * 32, kColS + b * 64 + cbase + c0), reinterpret_cast<uint32_t*>(&x[c0]));
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
@@ -164,27 +174,25 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
         const int key_pos = page * kPage + tok_in_page;
         const bool boundary = (page + 1) * kPage > w.n_keys;  // some row may not see every key of this page
 #pragma unroll
-        for (int c = 0; c < N; ++c) {
+        for (int c = 0; c < NC; ++c) {
             const float v = x[c] * p.scale_log2;
-            const bool ok = lane_ok && (!boundary || key_pos < w.n_keys + (N == 64 ? (c >> 4) : 0));
+            const bool ok = lane_ok && (!boundary || key_pos < w.n_keys + (N == 64 ? ((cbase + c) >> 4) : 0));
             x[c] = ok ? v : -INFINITY;
         }
         // Lazy running max: the per-row maximum is refreshed only when some key of this page exceeds the row's
         // reference by more than 2^kRescaleThreshold (always on the first page, where m_ref = -1e30).  The common
-        // path costs one subtraction + max per value and a single bar.red.or over the 128 softmax threads.
+        // path costs one subtraction + max per value and a single bar.red.or over the softmax threads.
         float dmax = -INFINITY;
 #pragma unroll
-        for (int c = 0; c < N; ++c) dmax = fmaxf(dmax, x[c] - sm->m_ref[c]);
+        for (int c = 0; c < NC; ++c) dmax = fmaxf(dmax, x[c] - sm->m_ref[cbase + c]);
         const bool need = named_or(2, dmax > kRescaleThreshold);
         if (tid_s == 0) KTRACE(7, g);
-        if (g > 0) mbar_wait(&sm->pv_done, (g - 1) & 1);  // PV of the previous page done: P buffer free, O stable
-        if (tid_s == 0) KTRACE(8, g);
         if (need) {
-            // exact column (query-row) max over the 64 keys of the page: warp redux, then 4 warps through smem
+            // exact column (query-row) max over the 64 keys of the page: warp redux, then 4 quadrants through smem
 #pragma unroll
-            for (int c = 0; c < N; ++c) {
+            for (int c = 0; c < NC; ++c) {
                 const float wm = warp_max(x[c]);
-                if (lane == (c & 31)) sm->red[w4][c] = wm;
+                if (lane == (c & 31)) sm->red[w4][cbase + c] = wm;
             }
             named_sync(1);
             if (tid_s < N) {
@@ -196,45 +204,48 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
             }
             named_sync(1);
             if (pg > 0) {  // O^T and l hold data relative to the old reference: rescale (rare)
+                mbar_wait(&sm->pv_done[(g - 1) & 1], ((g - 1) >> 1) & 1);  // every PV issued so far has completed
                 tc_fence_after();
 #pragma unroll
                 for (int b4 = 0; b4 < 4; ++b4)
 #pragma unroll
-                    for (int c0 = 0; c0 < N; c0 += 16) {
-                        uint32_t r[16];
-                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0);
-                        tmem_ld16(ta, r);
+                    for (int c0 = 0; c0 < NC; c0 += W) {
+                        uint32_t r[W];
+                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + cbase + c0);
+                        tmem_ldw<W>(ta, r);
                         tmem_wait_ld();
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[c0 + i]);
-                        tmem_st16(ta, r);
+                        for (int i = 0; i < W; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[cbase + c0 + i]);
+                        tmem_stw<W>(ta, r);
                     }
                 tmem_wait_st();
 #pragma unroll
-                for (int c = 0; c < N; ++c) l[c] *= sm->alpha[c];
+                for (int c = 0; c < NC; ++c) l[c] *= sm->alpha[cbase + c];
             }
         }
+        if (tid_s == 0) KTRACE(8, g);
 #pragma unroll
-        for (int c = 0; c < N; ++c) {
-            const float pv = ex2(x[c] - sm->m_ref[c]);
+        for (int c = 0; c < NC; ++c) {
+            const float pv = ex2(x[c] - sm->m_ref[cbase + c]);
             l[c] += pv;
             x[c] = pv;
         }
         if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
+            uint8_t* ps = kv + b * kStageBytes + kOffPInStage;
 #pragma unroll
-            for (int j = 0; j < N / 8; ++j) {
+            for (int j = 0; j < NC / 8; ++j) {
                 uint4 v;
                 v.x = pack_bf16(x[8 * j + 0], x[8 * j + 1]);
                 v.y = pack_bf16(x[8 * j + 2], x[8 * j + 3]);
                 v.z = pack_bf16(x[8 * j + 4], x[8 * j + 5]);
                 v.w = pack_bf16(x[8 * j + 6], x[8 * j + 7]);
-                *reinterpret_cast<uint4*>(ps + sw128_offset(tok_in_page, j)) = v;
+                *reinterpret_cast<uint4*>(ps + sw128_offset(tok_in_page, cbase / 8 + j)) = v;
             }
         }
         fence_proxy_async_smem();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&sm->p_full);
+        if (lane == 0) mbar_arrive(&sm->p_full[b]);
         if (tid_s == 0) KTRACE(9, g);
     }
 
@@ -242,13 +253,13 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
     mbar_wait(&sm->o_full, it & 1);
     tc_fence_after();
 #pragma unroll
-    for (int c = 0; c < N; ++c) {
+    for (int c = 0; c < NC; ++c) {
         float v = l[c];
         v += __shfl_xor_sync(0xffffffffu, v, 8);
         v += __shfl_xor_sync(0xffffffffu, v, 4);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
         v += __shfl_xor_sync(0xffffffffu, v, 1);  // lanes 0..15 hold the data, lanes 16..31 hold zeros
-        if (lane == (c & 15)) sm->red[w4][c] = v;
+        if (lane == (c & 15)) sm->red[w4][cbase + c] = v;
     }
     named_sync(1);
     const bool is_final = w.partial_slot < 0;
@@ -272,22 +283,23 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
     named_sync(2);
 #pragma unroll
     for (int b4 = 0; b4 < 4; ++b4) {
-        const int d = b4 * 128 + tid_s;
+        const int d = b4 * 128 + w4 * 32 + lane;
 #pragma unroll
-        for (int c0 = 0; c0 < N; c0 += 16) {
-            const int tok = c0 >> 4;
-            if (tok >= w.n_q) continue;  // ragged chunk tail (uniform across the CTA)
-            uint32_t r[16];
-            tmem_ld16(tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + c0), r);
+        for (int c0 = 0; c0 < NC; c0 += W) {
+            const int col = cbase + c0;
+            const int tok = col >> 4;
+            if (tok >= w.n_q) continue;  // ragged chunk tail (uniform across the warp)
+            uint32_t r[W];
+            tmem_ldw<W>(tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + col), r);
             tmem_wait_ld();
             if (is_final) {
-                __nv_bfloat16* o = (w.kind ? p.out_chunk : p.out_dec) + size_t(w.q_index + tok) * kHeads * kLatent + d;
+                __nv_bfloat16* o = (w.kind ? p.out_chunk : p.out_dec) + (size_t(w.q_index + tok) * kHeads + (col & 15)) * kLatent + d;
 #pragma unroll
-                for (int i = 0; i < 16; ++i) o[i * kLatent] = __float2bfloat16_rn(__uint_as_float(r[i]) * sm->linv[c0 + i]);
+                for (int i = 0; i < W; ++i) o[i * kLatent] = __float2bfloat16_rn(__uint_as_float(r[i]) * sm->linv[col + i]);
             } else {
-                float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes) + d;
+                float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes) + (col & 15) * kLatent + d;
 #pragma unroll
-                for (int i = 0; i < 16; ++i) o[i * kLatent] = __uint_as_float(r[i]);
+                for (int i = 0; i < W; ++i) o[i * kLatent] = __uint_as_float(r[i]);
             }
         }
     }
@@ -301,7 +313,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* ps, const WorkI
 // as its P^T is ready, because its completion releases the KV stage to the TMA producer.
 // ------------------------------------------------------------------------------------------------------------
 template <int N>
-__device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base, uint32_t p_base,
+__device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base,
                                          int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p) {
     constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
     constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
@@ -311,13 +323,14 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
     while (pv_next < npages) {
         if (pv_next < s_next) {
             const uint32_t gg = g0 + pv_next;
-            const bool ready = __any_sync(0xffffffffu, mbar_try_wait(&sm->p_full, gg & 1));
+            const uint32_t pst = gg & 1, pph = (gg >> 1) & 1;
+            const bool ready = __any_sync(0xffffffffu, mbar_test_wait(&sm->p_full[pst], pph));
             if (ready || s_next == npages) {
-                if (!ready) mbar_wait(&sm->p_full, gg & 1);
+                if (!ready) mbar_wait(&sm->p_full[pst], pph);
                 if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
                 KTRACE(3, gg);
                 tc_fence_after();
-                const uint32_t st = gg & 1, a0 = kv_base + st * kStageBytes;
+                const uint32_t st = pst, a0 = kv_base + st * kStageBytes, p_base = a0 + kOffPInStage;
 #pragma unroll
                 for (uint32_t b4 = 0; b4 < 4; ++b4)
 #pragma unroll
@@ -325,7 +338,7 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                         umma_bf16_ss(tmem + kColO + b4 * 64, make_smem_desc(a0 + (2 * b4) * 8192 + ks * 2048, 8192, 1024),
                                      make_smem_desc(p_base + ks * 2048, 8192, 1024), idesc_o, (pv_next > 0 || ks > 0), leader);
                 umma_commit(&sm->kv_empty[st], leader);
-                umma_commit(&sm->pv_done, leader);
+                umma_commit(&sm->pv_done[st], leader);
                 if (pv_next == npages - 1) umma_commit(&sm->o_full, leader);
                 KTRACE(4, gg);
                 ++pv_next;
@@ -336,7 +349,7 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
         if (s_next < npages && s_next <= pv_next + 1) {
             const uint32_t gg = g0 + s_next;
             const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
-            if (__any_sync(0xffffffffu, mbar_try_wait(&sm->kv_full[st], ph))) {
+            if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[st], ph))) {
                 KTRACE(1, gg);
                 mbar_wait(&sm->s_empty[st], ph ^ 1);
                 tc_fence_after();
@@ -375,14 +388,14 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             mbar_init(&sm->kv_full[i], 1);
             mbar_init(&sm->kv_empty[i], 1);
             mbar_init(&sm->s_full[i], 1);
-            mbar_init(&sm->s_empty[i], 4);
+            mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
-            mbar_init(&sm->item_empty[i], 5);
+            mbar_init(&sm->item_empty[i], 1 + kSoftmaxWarps);
+            mbar_init(&sm->p_full[i], kSoftmaxWarps);
+            mbar_init(&sm->pv_done[i], 1);
         }
-        mbar_init(&sm->p_full, 4);
-        mbar_init(&sm->pv_done, 1);
         mbar_init(&sm->o_full, 1);
-        mbar_init(&sm->o_empty, 4);
+        mbar_init(&sm->o_empty, kSoftmaxWarps);
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) {
@@ -440,7 +453,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
     } else if (warp == 1) {
         // ================= MMA issuer: the whole warp runs converged, one elected lane issues =================
         const uint32_t leader = elect_one();
-        const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV), p_base = smem_u32(base + kOffP);
+        const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV);
         uint32_t g = 0;
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
@@ -452,14 +465,14 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             const WorkItem w = load_item(p.items + idx);
             const int kind = __shfl_sync(0xffffffffu, w.kind, 0);
             const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
-            if (kind) mma_item<64>(sm, tmem, q_base, kv_base, p_base, npages, g, it, leader, p);
-            else mma_item<16>(sm, tmem, q_base, kv_base, p_base, npages, g, it, leader, p);
+            if (kind) mma_item<64>(sm, tmem, q_base, kv_base, npages, g, it, leader, p);
+            else mma_item<16>(sm, tmem, q_base, kv_base, npages, g, it, leader, p);
             g += npages;
         }
     } else {
         // ================= softmax / correction / epilogue warps =================
-        const int w4 = warp & 3;  // TMEM lane quadrant this warp may access
-        uint8_t* ps = base + kOffP;
+        const int sw = warp - 2;  // 0..7; TMEM lane quadrant = warp & 3 = (sw + 2) & 3
+        uint8_t* kv = base + kOffKV;
         uint32_t g = 0;
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
@@ -468,8 +481,8 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
-            if (w.kind) softmax_item<64>(sm, ps, w, p, tmem, w4, lane, g, it);
-            else softmax_item<16>(sm, ps, w, p, tmem, w4, lane, g, it);
+            if (w.kind) softmax_item<64>(sm, kv, w, p, tmem, sw, lane, g, it);
+            else softmax_item<16>(sm, kv, w, p, tmem, sw, lane, g, it);
         }
     }
 
