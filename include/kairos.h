@@ -163,6 +163,22 @@ int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int32_t nB, co
                               const int32_t* Cs, int32_t nC, int32_t prefix_len, int32_t warmup, int32_t reps,
                               int32_t flush_l2, double* out_median_us, double* out_min_us, void* cuda_stream);
 
+/*
+ * a0 -- the host planner alone (no GPU, no context): the work list kairos_mixed_step would build for these
+ * lengths on a device with `n_ctas` resident CTAs.  Pure integer host code; used by the CPU tests to check that
+ * every (request, page) and every chunk token is covered exactly once and that the partial slots stay inside the
+ * kairos_workspace_bytes bound.
+ *   dec_ctx_lens   HOST int32 [n_dec] (each >= 1)
+ *   items_out      HOST int32 [max_items][8]: kind (0 decode split / 1 chunk tile), q_index (request index or
+ *                  first chunk token), page_begin, page_end, n_keys, n_q, partial_slot (-1 = final output), cost;
+ *                  in queue order.  May be NULL (count only).
+ *   n_items_out    HOST, number of items of the plan (even if > max_items; only max_items are written)
+ *   n_partial_slots_out  HOST or NULL
+ * Errors: INVALID_ARG.
+ */
+int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t n_ctas,
+                     int32_t* items_out, int32_t max_items, int32_t* n_items_out, int32_t* n_partial_slots_out);
+
 /* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
  * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched
  * by that call, [5] = workspace bytes used.  n = number of int64 slots available in info. */

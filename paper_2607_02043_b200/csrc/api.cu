@@ -324,6 +324,22 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     return KAIROS_OK;
 }
 
+int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t n_ctas,
+                     int32_t* items_out, int32_t max_items, int32_t* n_items_out, int32_t* n_partial_slots_out) {
+    if (n_dec < 0 || chunk_len < 0 || prefix_len < 0 || n_ctas < 1 || max_items < 0 || !n_items_out)
+        return fail(KAIROS_ERR_INVALID_ARG, "bad size or NULL n_items_out");
+    if (n_dec > 0 && !dec_ctx_lens) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens is NULL");
+    for (int32_t i = 0; i < n_dec; ++i)
+        if (dec_ctx_lens[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens[" + std::to_string(i) + "] < 1");
+    Plan plan;
+    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, n_ctas, umma_chunk_tile_tokens(), &plan);
+    *n_items_out = int32_t(plan.items.size());
+    if (n_partial_slots_out) *n_partial_slots_out = plan.n_partial_slots;
+    if (items_out)
+        std::memcpy(items_out, plan.items.data(), sizeof(WorkItem) * size_t(std::min<int64_t>(max_items, int64_t(plan.items.size()))));
+    return KAIROS_OK;
+}
+
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n) {
     if (!ctx || !info || n < 0) return fail(KAIROS_ERR_INVALID_ARG, "NULL argument");
     for (int32_t i = 0; i < n && i < 6; ++i) info[i] = ctx->last_info[i];

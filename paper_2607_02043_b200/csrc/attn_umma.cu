@@ -403,6 +403,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
         prefetch_tensormap(&qd_map);
         prefetch_tensormap(&qc_map);
     }
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the combine grid may pre-launch; it waits on griddepcontrol.wait
     if (warp == 1) tmem_alloc(&sm->tmem_base, kTmemCols);
     tc_fence_before();
     __syncthreads();
@@ -502,76 +503,85 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
 
 // ------------------------------------------------------------------------------------------------------------
 // a5: log-sum-exp combine of split partials: out = sum_k 2^(m_k-m*) O_k / sum_k 2^(m_k-m*) l_k
+// grid = (combine items, kCombineSlices): each CTA merges a 128-wide slice of the 512 latent dims for all 16 heads,
+// so that one long request (many splits) is spread over 4 CTAs and every thread streams independent float4 loads.
+// Launched with programmatic stream serialisation: griddepcontrol.wait orders it after the main kernel's writes.
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) combine_kernel(const CombineItem* __restrict__ items, const uint8_t* __restrict__ partials,
+constexpr int kCombineSlices = 4;
+constexpr int kCombineThreads = 256;
+__global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineItem* __restrict__ items, const uint8_t* __restrict__ partials,
                                                       __nv_bfloat16* __restrict__ out_dec, __nv_bfloat16* __restrict__ out_chunk,
                                                       float* __restrict__ lse_dec, float* __restrict__ lse_chunk) {
-    constexpr int kMaxK = 32;  // splits whose weights are staged in shared memory per pass
+    constexpr int kMaxK = 64;  // splits whose weights are staged in shared memory per pass
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const CombineItem ci = items[blockIdx.x];
     const int kind = ci.kind_stride & 0xff, stride = ci.kind_stride >> 8;
-    __shared__ float s_m[kMaxK][kHeads], s_w[kMaxK][kHeads], s_mstar[kHeads], s_linv[kHeads];
+    __shared__ float s_w[kMaxK][kHeads], s_wl[kMaxK][kHeads], s_mstar[kHeads], s_L[kHeads];
     const int tid = threadIdx.x;
     auto slot_ptr = [&](int k) { return partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes; };
-    // pass 1: m* per head over all splits
-    if (tid < kHeads) {
+    auto ml_ptr = [&](int k) { return reinterpret_cast<const float*>(slot_ptr(k) + size_t(kHeads) * kLatent * 4); };
+    // pass 1: m* per head over all splits (16 lanes per head-group: lane h of each 16 reduces a strided subset)
+    {
+        const int h = tid & 15, part = tid >> 4;  // 16 parts
         float ms = kMinusHuge;
-        for (int k = 0; k < ci.n_splits; ++k)
-            ms = fmaxf(ms, reinterpret_cast<const float*>(slot_ptr(k) + size_t(kHeads) * kLatent * 4)[tid]);
-        s_mstar[tid] = ms;
+        for (int k = part; k < ci.n_splits; k += 16) ms = fmaxf(ms, ml_ptr(k)[h]);
+        __shared__ float s_pm[16][kHeads];
+        s_pm[part][h] = ms;
+        __syncthreads();
+        if (tid < kHeads) {
+            float m2 = kMinusHuge;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) m2 = fmaxf(m2, s_pm[i][tid]);
+            s_mstar[tid] = m2;
+            s_L[tid] = 0.f;
+        }
+        __syncthreads();
     }
-    __syncthreads();
-    // each thread owns 8 consecutive outputs of 4 (head, d) groups: e = (tid + 256*i) * 8 ... covers 16*512 = 8192
-    float acc[4][8];
+    // thread -> (head h, 8 consecutive dims of this CTA's 128-dim slice)
+    const int h = tid >> 4;
+    const int d0 = blockIdx.y * 128 + (tid & 15) * 8;
+    const int fo = (h * kLatent + d0) / 4;  // float4 index inside a slot
+    float acc[8];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
-    float L = 0.f;  // threads < 16 accumulate the denominator of their head
+    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
     for (int k0 = 0; k0 < ci.n_splits; k0 += kMaxK) {
         const int kn = min(kMaxK, ci.n_splits - k0);
-        for (int i = tid; i < kn * kHeads; i += 256) {
-            const int k = i / kHeads, h = i % kHeads;
-            const float* ml = reinterpret_cast<const float*>(slot_ptr(k0 + k) + size_t(kHeads) * kLatent * 4);
-            const float w = exp2f(ml[h] - s_mstar[h]);  // m = -1e30 (nothing visible) -> 0
-            s_w[k][h] = w;
-            s_m[k][h] = w * ml[kHeads + h];
+        for (int i = tid; i < kn * kHeads; i += kCombineThreads) {
+            const int k = i / kHeads, hh = i % kHeads;
+            const float* ml = ml_ptr(k0 + k);
+            const float w = exp2f(ml[hh] - s_mstar[hh]);  // m = -1e30 (nothing visible) -> 0
+            s_w[k][hh] = w;
+            s_wl[k][hh] = w * ml[kHeads + hh];
         }
         __syncthreads();
-        if (tid < kHeads)
-            for (int k = 0; k < kn; ++k) L += s_m[k][tid];
-#pragma unroll 4
+        if (tid < kHeads) {  // deterministic order: the result must not depend on scheduling
+            float Ls = s_L[tid];
+            for (int k = 0; k < kn; ++k) Ls += s_wl[k][tid];
+            s_L[tid] = Ls;
+        }
+#pragma unroll 8
         for (int k = 0; k < kn; ++k) {
-            const float4* src = reinterpret_cast<const float4*>(slot_ptr(k0 + k));
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int v = (tid + 256 * i) * 2;  // float4 index; 8 floats = 2 float4
-                const int h = (v * 4) / kLatent;
-                const float w = s_w[k][h];
-                const float4 a = __ldg(src + v), b = __ldg(src + v + 1);
-                acc[i][0] += w * a.x; acc[i][1] += w * a.y; acc[i][2] += w * a.z; acc[i][3] += w * a.w;
-                acc[i][4] += w * b.x; acc[i][5] += w * b.y; acc[i][6] += w * b.z; acc[i][7] += w * b.w;
-            }
+            const float4* src = reinterpret_cast<const float4*>(slot_ptr(k0 + k)) + fo;
+            const float w = s_w[k][h];
+            const float4 a = __ldcg(src), b = __ldcg(src + 1);
+            acc[0] += w * a.x; acc[1] += w * a.y; acc[2] += w * a.z; acc[3] += w * a.w;
+            acc[4] += w * b.x; acc[5] += w * b.y; acc[6] += w * b.z; acc[7] += w * b.w;
         }
         __syncthreads();
     }
-    if (tid < kHeads) {
-        s_linv[tid] = 1.f / L;
+    const float L = s_L[h];
+    if (blockIdx.y == 0 && tid < kHeads) {
         float* lse = kind ? lse_chunk : lse_dec;
-        if (lse) lse[size_t(ci.q_index) * kHeads + tid] = (s_mstar[tid] + log2f(L)) * kLn2;
+        if (lse) lse[size_t(ci.q_index) * kHeads + tid] = (s_mstar[tid] + log2f(s_L[tid])) * kLn2;
     }
-    __syncthreads();
-    __nv_bfloat16* out = (kind ? out_chunk : out_dec) + size_t(ci.q_index) * kHeads * kLatent;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int e = (tid + 256 * i) * 8;
-        const float inv = s_linv[e / kLatent];
-        uint4 o;
-        o.x = pack_bf16(acc[i][0] * inv, acc[i][1] * inv);
-        o.y = pack_bf16(acc[i][2] * inv, acc[i][3] * inv);
-        o.z = pack_bf16(acc[i][4] * inv, acc[i][5] * inv);
-        o.w = pack_bf16(acc[i][6] * inv, acc[i][7] * inv);
-        *reinterpret_cast<uint4*>(out + e) = o;
-    }
+    const float inv = 1.f / L;
+    __nv_bfloat16* out = (kind ? out_chunk : out_dec) + (size_t(ci.q_index) * kHeads + h) * kLatent + d0;
+    uint4 o;
+    o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+    o.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+    o.z = pack_bf16(acc[4] * inv, acc[5] * inv);
+    o.w = pack_bf16(acc[6] * inv, acc[7] * inv);
+    *reinterpret_cast<uint4*>(out) = o;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -662,7 +672,18 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
     *kernels_launched = 1;
     if (n_combines > 0) {
-        combine_kernel<<<n_combines, 256, 0, stream>>>(dev_combines, p.partials, p.out_dec, p.out_chunk, p.lse_dec, p.lse_chunk);
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(unsigned(n_combines), kCombineSlices, 1);
+        cfg.blockDim = dim3(kCombineThreads, 1, 1);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const uint8_t* cparts = p.partials;
+        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, cparts, p.out_dec, p.out_chunk, p.lse_dec, p.lse_chunk));
         KAIROS_CUDA_TRY(cudaGetLastError());
         *kernels_launched = 2;
     }

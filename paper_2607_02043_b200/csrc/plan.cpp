@@ -44,33 +44,66 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
 
     std::vector<WorkItem> dec_items, chunk_items;
 
-    // ---- decode splits
-    for (int32_t i = 0; i < n_dec; ++i) {
-        const int32_t pages = ceil_div(dec_ctx_lens[i], kPage);
-        int32_t max_pages = int32_t(std::max<int64_t>(kMinSplitPages, max_item_cost / kChunkCostDen));
-        int32_t n_splits = ceil_div(pages, max_pages);
-        n_splits = std::min(n_splits, std::max(1, pages / kMinSplitPages));
-        if (n_splits > 1 && n_splits - 1 > dec_split_budget) n_splits = 1 + std::max(0, dec_split_budget);
-        if (n_splits > 1) dec_split_budget -= (n_splits - 1);
-        const int32_t per = ceil_div(pages, n_splits);
-        n_splits = ceil_div(pages, per);
-        int32_t first_slot = -1;
-        if (n_splits > 1) {
-            first_slot = plan->n_partial_slots;
-            plan->n_partial_slots += n_splits;
-            plan->combines.push_back(CombineItem{i, first_slot, n_splits, 0 /*decode*/ | (1 << 8) /*slot stride 1*/});
-        }
-        for (int32_t s = 0; s < n_splits; ++s) {
-            WorkItem w{};
-            w.kind = 0;
-            w.q_index = i;
-            w.page_begin = s * per;
-            w.page_end = std::min(pages, (s + 1) * per);
-            w.n_keys = dec_ctx_lens[i];
-            w.n_q = 1;
-            w.partial_slot = n_splits > 1 ? first_slot + s : -1;
-            w.cost = (w.page_end - w.page_begin) * kChunkCostDen;
-            dec_items.push_back(w);
+    // ---- decode splits.  Two item sizes: "big" pieces (about a third of one CTA's fair share) carry most of the
+    // pages with few partials; a tail budget of kMinSplitPages-sized pieces, peeled off the longest requests, goes
+    // to the END of the queue so that the dynamic queue's finishing imbalance is a few pages, not one big piece.
+    {
+        const int64_t fair_pages = std::max<int64_t>(1, total_cost / (int64_t(kChunkCostDen) * target_ctas));
+        const int32_t big = int32_t(std::max<int64_t>(kMinSplitPages, std::min<int64_t>(max_item_cost / kChunkCostDen, (fair_pages + 2) / 3)));
+        int64_t tail_budget = fair_pages >= 4 * kMinSplitPages ? int64_t(target_ctas) * 2 * kMinSplitPages : 0;  // pages
+        std::vector<int32_t> order(n_dec);
+        for (int32_t i = 0; i < n_dec; ++i) order[i] = i;
+        std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return dec_ctx_lens[a] > dec_ctx_lens[b]; });
+        std::vector<int32_t> cuts;
+        for (int32_t oi = 0; oi < n_dec; ++oi) {
+            const int32_t i = order[oi];
+            const int32_t pages = ceil_div(dec_ctx_lens[i], kPage);
+            // small tail pieces of this request (peeled from its end)
+            int32_t n_small = 0;
+            if (tail_budget > 0 && pages >= 3 * kMinSplitPages) {
+                n_small = int32_t(std::min<int64_t>({int64_t(2), tail_budget / kMinSplitPages, int64_t(pages / kMinSplitPages - 2)}));
+                n_small = std::max(n_small, 0);
+            }
+            const int32_t body = pages - n_small * kMinSplitPages;
+            int32_t n_big = ceil_div(body, big);
+            n_big = std::min(n_big, std::max(1, body / kMinSplitPages));
+            int32_t n_splits = n_big + n_small;
+            if (n_splits > 1 && n_splits - 1 > dec_split_budget) {  // workspace bound: fall back to fewer pieces
+                n_small = 0;
+                n_big = std::min(ceil_div(pages, big), 1 + std::max(0, dec_split_budget));
+                n_big = std::max(1, std::min(n_big, std::max(1, pages / kMinSplitPages)));
+                n_splits = n_big;
+            }
+            const int32_t body2 = pages - n_small * kMinSplitPages;
+            cuts.clear();
+            cuts.push_back(0);
+            const int32_t per = ceil_div(body2, n_big);
+            for (int32_t s = 1; s <= n_big; ++s) {
+                const int32_t e = std::min(body2, s * per);
+                if (e > cuts.back()) cuts.push_back(e);
+            }
+            for (int32_t s = 1; s <= n_small; ++s) cuts.push_back(body2 + s * kMinSplitPages);
+            n_splits = int32_t(cuts.size()) - 1;
+            if (n_splits > 1) dec_split_budget -= (n_splits - 1);
+            tail_budget -= int64_t(n_small) * kMinSplitPages;
+            int32_t first_slot = -1;
+            if (n_splits > 1) {
+                first_slot = plan->n_partial_slots;
+                plan->n_partial_slots += n_splits;
+                plan->combines.push_back(CombineItem{i, first_slot, n_splits, 0 /*decode*/ | (1 << 8) /*slot stride 1*/});
+            }
+            for (int32_t s = 0; s < n_splits; ++s) {
+                WorkItem w{};
+                w.kind = 0;
+                w.q_index = i;
+                w.page_begin = cuts[s];
+                w.page_end = cuts[s + 1];
+                w.n_keys = dec_ctx_lens[i];
+                w.n_q = 1;
+                w.partial_slot = n_splits > 1 ? first_slot + s : -1;
+                w.cost = (w.page_end - w.page_begin) * kChunkCostDen;
+                dec_items.push_back(w);
+            }
         }
     }
 

@@ -52,6 +52,8 @@ _lib.kairos_mixed_step_host.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i
 _lib.kairos_mixed_step_host.restype = _c.c_int
 _lib.kairos_step_latency_table.argtypes = [_vp, _vp, _i32, _vp, _i32, _vp, _i32, _i32, _i32, _i32, _i32, _vp, _vp, _vp]
 _lib.kairos_step_latency_table.restype = _c.c_int
+_lib.kairos_plan_dump.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp, _i32, _vp, _vp]
+_lib.kairos_plan_dump.restype = _c.c_int
 _lib.kairos_last_plan_info.argtypes = [_vp, _vp, _i32]
 _lib.kairos_last_plan_info.restype = _c.c_int
 _lib.kairos_profile_enable.argtypes = [_vp, _i32]
@@ -65,7 +67,7 @@ _lib.kairos_version.restype = _c.c_char_p
 
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
-           "kairos_step_latency_table", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_last_error", "kairos_version"]
+           "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
           -4: "KAIROS_ERR_CUDA"}
@@ -214,6 +216,19 @@ class Kairos:
         _check(_lib.kairos_last_plan_info(self._h, info, 6))
         keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes"]
         return dict(zip(keys, (int(x) for x in info)))
+
+
+def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ctas: int = 148):
+    """Host planner alone (kairos_plan_dump): (items int32 [n, 8] in queue order, n_partial_slots). No GPU needed."""
+    lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+    n, slots = _c.c_int32(0), _c.c_int32(0)
+    lp = lens.ctypes.data_as(_vp) if lens.size else None
+    _check(_lib.kairos_plan_dump(lp, int(lens.size), int(chunk_len), int(prefix_len), int(n_ctas), None, 0,
+                                 _c.byref(n), _c.byref(slots)))
+    items = np.zeros((int(n.value), 8), dtype=np.int32)
+    _check(_lib.kairos_plan_dump(lp, int(lens.size), int(chunk_len), int(prefix_len), int(n_ctas),
+                                 items.ctypes.data_as(_vp), int(n.value), _c.byref(n), _c.byref(slots)))
+    return items, int(slots.value)
 
 
 def bf16_tensor(bits: np.ndarray, device="cuda") -> torch.Tensor:
