@@ -252,6 +252,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
     // ---- epilogue: all PV MMAs of the item are complete
     mbar_wait(&sm->o_full, it & 1);
     tc_fence_after();
+    if (tid_s == 0 && it == 0) KTRACE(10, 5);
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         float v = l[c];
@@ -306,6 +307,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->o_empty);
+    if (tid_s == 0 && it == 0) KTRACE(10, 6);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -317,6 +319,8 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                                          int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p) {
     constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
     constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
+    constexpr uint32_t desc_hi = smem_desc_hi(1024);
+    const uint32_t qb_lo = smem_desc_lo(q_base, 16);
     mbar_wait(&sm->q_full, it & 1);
     int s_next = 0, pv_next = 0;
     uint32_t spins = 0;
@@ -330,16 +334,17 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                 if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
                 KTRACE(3, gg);
                 tc_fence_after();
-                const uint32_t st = pst, a0 = kv_base + st * kStageBytes, p_base = a0 + kOffPInStage;
+                const uint32_t st = pst, a0 = kv_base + st * kStageBytes;
+                const uint32_t va_lo = smem_desc_lo(a0, 8192), pb_lo = smem_desc_lo(a0 + kOffPInStage, 8192);
 #pragma unroll
                 for (uint32_t b4 = 0; b4 < 4; ++b4)
 #pragma unroll
                     for (uint32_t ks = 0; ks < 4; ++ks)
-                        umma_bf16_ss(tmem + kColO + b4 * 64, make_smem_desc(a0 + (2 * b4) * 8192 + ks * 2048, 8192, 1024),
-                                     make_smem_desc(p_base + ks * 2048, 8192, 1024), idesc_o, (pv_next > 0 || ks > 0), leader);
-                umma_commit(&sm->kv_empty[st], leader);
-                umma_commit(&sm->pv_done[st], leader);
-                if (pv_next == npages - 1) umma_commit(&sm->o_full, leader);
+                        umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + (((2 * b4) * 8192 + ks * 2048) >> 4), desc_hi,
+                                          pb_lo + ((ks * 2048) >> 4), desc_hi, idesc_o, (pv_next > 0 || ks > 0));
+                umma_commit_elect(&sm->kv_empty[st]);
+                umma_commit_elect(&sm->pv_done[st]);
+                if (pv_next == npages - 1) umma_commit_elect(&sm->o_full);
                 KTRACE(4, gg);
                 ++pv_next;
                 spins = 0;
@@ -353,16 +358,16 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                 KTRACE(1, gg);
                 mbar_wait(&sm->s_empty[st], ph ^ 1);
                 tc_fence_after();
-                const uint32_t a0 = kv_base + st * kStageBytes;
+                const uint32_t ka_lo = smem_desc_lo(kv_base + st * kStageBytes, 16);
 #pragma unroll
                 for (uint32_t c = 0; c < 9; ++c)
 #pragma unroll
                     for (uint32_t j = 0; j < 4; ++j)
-                        umma_bf16_ss(tmem + kColS + st * 64, make_smem_desc(a0 + c * 8192 + j * 32, 16, 1024),
-                                     make_smem_desc(q_base + c * N * 128 + j * 32, 16, 1024), idesc_s, (c | j) != 0, leader);
-                umma_commit(&sm->s_full[st], leader);
+                        umma_bf16_ss_lohi(tmem + kColS + st * 64, ka_lo + ((c * 8192 + j * 32) >> 4), desc_hi,
+                                          qb_lo + ((c * N * 128 + j * 32) >> 4), desc_hi, idesc_s, (c | j) != 0);
+                umma_commit_elect(&sm->s_full[st]);
                 ++s_next;
-                if (s_next == npages) umma_commit(&sm->q_empty, leader);  // Q tile free once every S-MMA retires
+                if (s_next == npages) umma_commit_elect(&sm->q_empty);  // Q tile free once every S-MMA retires
                 KTRACE(2, gg);
                 spins = 0;
                 continue;
@@ -380,6 +385,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     Small* sm = reinterpret_cast<Small*>(base + kOffSmall);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) KTRACE(10, 0);
 
     if (threadIdx.x == 0) {
         mbar_init(&sm->q_full, 1);
@@ -409,6 +415,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm->tmem_base;
+    if (threadIdx.x == 0) KTRACE(10, 1);
 
     if (warp == 0) {
         // ================= producer: pop work items, TMA-load Q tiles and KV pages =================
@@ -418,6 +425,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
             idx = __shfl_sync(0xffffffffu, idx, 0);
             if (idx >= p.n_items) idx = -1;
+            if (lane == 0 && it == 0) KTRACE(10, 2);
             if (lane == 0) {
                 mbar_wait(&sm->item_empty[it & 1], ((it >> 1) & 1) ^ 1);
                 sm->item_ring[it & 1] = idx;
@@ -426,6 +434,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
             const int N = w.kind ? 64 : 16;
+            if (lane == 0 && it == 0) KTRACE(10, 3);
             if (lane == 0) {
                 mbar_wait(&sm->q_empty, (it & 1) ^ 1);
                 mbar_arrive_expect_tx(&sm->q_full, uint32_t(9 * N * 128));
@@ -439,6 +448,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             for (int i = 0; i < npages; i += 32) {
                 const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
                 const int cnt = min(32, npages - i);
+                if (lane == 0 && it == 0 && i == 0) KTRACE(10, 4);
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
@@ -490,6 +500,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
     // ---- teardown
     tc_fence_before();
     __syncthreads();
+    if (threadIdx.x == 0) KTRACE(10, 7);
     if (warp == 1) tmem_dealloc(tmem, kTmemCols);
     if (threadIdx.x == 0) {
         __threadfence();
