@@ -18,6 +18,7 @@
 #include <cuda_bf16.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 #include "kairos_internal.h"
 #include "umma_ptx.cuh"
@@ -126,6 +127,10 @@ __device__ __forceinline__ bool named_or(int id, bool pred) {
         : "r"(uint32_t(pred)), "r"(id), "n"(kSoftmaxThreads)
         : "memory");
     return r != 0;
+}
+// partial (split) results are re-read by the combine kernel right after this kernel: keep them in L2
+__device__ __forceinline__ void st_f32_evict_last(float* p, float v) {
+    asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(kEvictLast) : "memory");
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     uint32_t r;
@@ -300,7 +305,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
             } else {
                 float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes) + (col & 15) * kLatent + d;
 #pragma unroll
-                for (int i = 0; i < W; ++i) o[i * kLatent] = __uint_as_float(r[i]);
+                for (int i = 0; i < W; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[i]));
             }
         }
     }
@@ -514,12 +519,12 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
 
 // ------------------------------------------------------------------------------------------------------------
 // a5: log-sum-exp combine of split partials: out = sum_k 2^(m_k-m*) O_k / sum_k 2^(m_k-m*) l_k
-// grid = (combine items, kCombineSlices): each CTA merges a 128-wide slice of the 512 latent dims for all 16 heads,
-// so that one long request (many splits) is spread over 4 CTAs and every thread streams independent float4 loads.
+// grid = (combine items, kCombineSlices): each CTA merges a 32-wide slice of the 512 latent dims for all 16 heads,
+// so that one long request (many splits) is spread over 16 CTAs and every thread streams independent float4 loads.
 // Launched with programmatic stream serialisation: griddepcontrol.wait orders it after the main kernel's writes.
 // ------------------------------------------------------------------------------------------------------------
-constexpr int kCombineSlices = 4;
-constexpr int kCombineThreads = 256;
+constexpr int kCombineSlices = 16;
+constexpr int kCombineThreads = 128;
 __global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineItem* __restrict__ items, const uint8_t* __restrict__ partials,
                                                       __nv_bfloat16* __restrict__ out_dec, __nv_bfloat16* __restrict__ out_chunk,
                                                       float* __restrict__ lse_dec, float* __restrict__ lse_chunk) {
@@ -531,30 +536,35 @@ __global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineI
     const int tid = threadIdx.x;
     auto slot_ptr = [&](int k) { return partials + size_t(ci.first_slot + k * stride) * kPartialSlotBytes; };
     auto ml_ptr = [&](int k) { return reinterpret_cast<const float*>(slot_ptr(k) + size_t(kHeads) * kLatent * 4); };
-    // pass 1: m* per head over all splits (16 lanes per head-group: lane h of each 16 reduces a strided subset)
+    // the first kPre splits' data are requested before the (dependent) weight passes, so their latency overlaps
+    constexpr int kPre = 8;
+    const int fo_pre = ((tid >> 3) * kLatent + blockIdx.y * 32 + (tid & 7) * 4) / 4;
+    float4 pre[kPre];
+#pragma unroll
+    for (int k = 0; k < kPre; ++k)
+        pre[k] = k < ci.n_splits ? __ldcs(reinterpret_cast<const float4*>(slot_ptr(k)) + fo_pre) : make_float4(0.f, 0.f, 0.f, 0.f);
+    // pass 1: m* per head over all splits (8 parts x 16 heads)
     {
-        const int h = tid & 15, part = tid >> 4;  // 16 parts
+        const int h = tid & 15, part = tid >> 4;  // 8 parts
         float ms = kMinusHuge;
-        for (int k = part; k < ci.n_splits; k += 16) ms = fmaxf(ms, ml_ptr(k)[h]);
-        __shared__ float s_pm[16][kHeads];
+        for (int k = part; k < ci.n_splits; k += 8) ms = fmaxf(ms, ml_ptr(k)[h]);
+        __shared__ float s_pm[8][kHeads];
         s_pm[part][h] = ms;
         __syncthreads();
         if (tid < kHeads) {
             float m2 = kMinusHuge;
 #pragma unroll
-            for (int i = 0; i < 16; ++i) m2 = fmaxf(m2, s_pm[i][tid]);
+            for (int i = 0; i < 8; ++i) m2 = fmaxf(m2, s_pm[i][tid]);
             s_mstar[tid] = m2;
             s_L[tid] = 0.f;
         }
         __syncthreads();
     }
-    // thread -> (head h, 8 consecutive dims of this CTA's 128-dim slice)
-    const int h = tid >> 4;
-    const int d0 = blockIdx.y * 128 + (tid & 15) * 8;
+    // thread -> (head h, 4 consecutive dims of this CTA's 32-dim slice)
+    const int h = tid >> 3;
+    const int d0 = blockIdx.y * 32 + (tid & 7) * 4;
     const int fo = (h * kLatent + d0) / 4;  // float4 index inside a slot
-    float acc[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
     for (int k0 = 0; k0 < ci.n_splits; k0 += kMaxK) {
         const int kn = min(kMaxK, ci.n_splits - k0);
         for (int i = tid; i < kn * kHeads; i += kCombineThreads) {
@@ -570,13 +580,20 @@ __global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineI
             for (int k = 0; k < kn; ++k) Ls += s_wl[k][tid];
             s_L[tid] = Ls;
         }
+        int kb = 0;
+        if (k0 == 0) {
+#pragma unroll
+            for (int k = 0; k < kPre; ++k) {
+                const float w = k < kn ? s_w[k][h] : 0.f;
+                acc[0] += w * pre[k].x; acc[1] += w * pre[k].y; acc[2] += w * pre[k].z; acc[3] += w * pre[k].w;
+            }
+            kb = kPre;
+        }
 #pragma unroll 8
-        for (int k = 0; k < kn; ++k) {
-            const float4* src = reinterpret_cast<const float4*>(slot_ptr(k0 + k)) + fo;
+        for (int k = kb; k < kn; ++k) {
+            const float4 a = __ldcs(reinterpret_cast<const float4*>(slot_ptr(k0 + k)) + fo);  // streamed: read once
             const float w = s_w[k][h];
-            const float4 a = __ldcg(src), b = __ldcg(src + 1);
             acc[0] += w * a.x; acc[1] += w * a.y; acc[2] += w * a.z; acc[3] += w * a.w;
-            acc[4] += w * b.x; acc[5] += w * b.y; acc[6] += w * b.z; acc[7] += w * b.w;
         }
         __syncthreads();
     }
@@ -587,12 +604,10 @@ __global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineI
     }
     const float inv = 1.f / L;
     __nv_bfloat16* out = (kind ? out_chunk : out_dec) + (size_t(ci.q_index) * kHeads + h) * kLatent + d0;
-    uint4 o;
+    uint2 o;
     o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
     o.y = pack_bf16(acc[2] * inv, acc[3] * inv);
-    o.z = pack_bf16(acc[4] * inv, acc[5] * inv);
-    o.w = pack_bf16(acc[6] * inv, acc[7] * inv);
-    *reinterpret_cast<uint4*>(out) = o;
+    *reinterpret_cast<uint2*>(out) = o;
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -44,12 +44,12 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
 
     std::vector<WorkItem> dec_items, chunk_items;
 
-    // ---- decode splits.  Two item sizes: "big" pieces (about a third of one CTA's fair share) carry most of the
+    // ---- decode splits.  Two item sizes: "big" pieces (about half of one CTA's fair share) carry most of the
     // pages with few partials; a tail budget of kMinSplitPages-sized pieces, peeled off the longest requests, goes
     // to the END of the queue so that the dynamic queue's finishing imbalance is a few pages, not one big piece.
     {
         const int64_t fair_pages = std::max<int64_t>(1, total_cost / (int64_t(kChunkCostDen) * target_ctas));
-        const int32_t big = int32_t(std::max<int64_t>(kMinSplitPages, std::min<int64_t>(max_item_cost / kChunkCostDen, (fair_pages + 2) / 3)));
+        const int32_t big = int32_t(std::max<int64_t>(kMinSplitPages, std::min<int64_t>(max_item_cost / kChunkCostDen, (fair_pages + 1) / 2)));
         int64_t tail_budget = fair_pages >= 4 * kMinSplitPages ? int64_t(target_ctas) * 2 * kMinSplitPages : 0;  // pages
         std::vector<int32_t> order(n_dec);
         for (int32_t i = 0; i < n_dec; ++i) order[i] = i;
