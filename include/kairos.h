@@ -169,15 +169,19 @@ int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int32_t nB, co
  * every (request, page) and every chunk token is covered exactly once and that the partial slots stay inside the
  * kairos_workspace_bytes bound.
  *   dec_ctx_lens   HOST int32 [n_dec] (each >= 1)
- *   items_out      HOST int32 [max_items][8]: kind (0 decode split / 1 chunk tile), q_index (request index or
- *                  first chunk token), page_begin, page_end, n_keys, n_q, partial_slot (-1 = final output), cost;
- *                  in queue order.  May be NULL (count only).
+ *   pair_mode      0 = the chunk runs as 4-token tiles in the same queue as the decode splits; -1 = the planner
+ *                  decides whether the chunk runs as 8-token tiles on 2-CTA clusters beside the decode grid (and on
+ *                  how many), as kairos_mixed_step does; n > 0 = force n clusters
+ *   items_out      HOST int32 [max_items][8]: kind (0 decode split / 1 chunk tile in the queue / 2 chunk tile of the
+ *                  cluster kernel), q_index (request index or first chunk token), page_begin, page_end, n_keys, n_q,
+ *                  partial_slot (-1 = final output), cost; queue order, then the cluster kernel's items.  May be NULL.
  *   n_items_out    HOST, number of items of the plan (even if > max_items; only max_items are written)
- *   n_partial_slots_out  HOST or NULL
+ *   n_partial_slots_out, n_pairs_out  HOST or NULL (clusters the cluster kernel would be launched with; 0 = unused)
  * Errors: INVALID_ARG.
  */
 int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t n_ctas,
-                     int32_t* items_out, int32_t max_items, int32_t* n_items_out, int32_t* n_partial_slots_out);
+                     int32_t pair_mode, int32_t* items_out, int32_t max_items, int32_t* n_items_out,
+                     int32_t* n_partial_slots_out, int32_t* n_pairs_out);
 
 /* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
  * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched

@@ -101,27 +101,69 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     auto us = [](auto a, auto b) { return std::chrono::duration<double, std::micro>(b - a).count(); };
     auto T0 = now();
     Plan& plan = ctx->plan;
-    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, umma_resident_ctas(ctx), umma_chunk_tile_tokens(), &plan);
+    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, umma_resident_ctas(ctx), umma_chunk_tile_tokens(), &plan,
+               ctx->force_pairs, pair_tile_tokens());
     const size_t ws_needed = kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes;
     if (ws_needed > ctx->cfg.workspace_bytes)
         return fail(KAIROS_ERR_WORKSPACE, "workspace too small: need " + std::to_string(ws_needed) + " bytes");
     const size_t items_bytes = plan.items.size() * sizeof(WorkItem);
     const size_t comb_bytes = plan.combines.size() * sizeof(CombineItem);
     const size_t comb_off = (items_bytes + 255) / 256 * 256;
+    const size_t pair_bytes = plan.pair_items.size() * sizeof(WorkItem);
+    const size_t pair_off = (comb_off + comb_bytes + 255) / 256 * 256;
     StagingSlot* st = nullptr;
     auto T1 = now();
-    if (int rc = staging_acquire(ctx, comb_off + comb_bytes + 256, &st)) return rc;
+    if (int rc = staging_acquire(ctx, pair_off + pair_bytes + 256, &st)) return rc;
     auto T2 = now();
     std::memcpy(st->host, plan.items.data(), items_bytes);
     if (comb_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + comb_off, plan.combines.data(), comb_bytes);
-    KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, comb_off + comb_bytes, cudaMemcpyHostToDevice, stream));
+    if (pair_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + pair_off, plan.pair_items.data(), pair_bytes);
+    KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, stream));
     KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
     auto T3 = now();
     int kernels = 0;
-    if (int rc = launch_attn_umma(ctx, a, reinterpret_cast<const WorkItem*>(st->dev), int32_t(plan.items.size()),
-                                  reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
-                                  int32_t(plan.combines.size()), stream, &kernels))
-        return rc;
+    // Roofline leg of bench.py: one pair of events around the attention kernels of the step (the decode grid and, when
+    // the planner uses it, the concurrent pair grid; fork and join are inside the bracket).
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->profile) {
+        if (ctx->prof_used + 2 > ctx->prof_events.size()) {
+            for (int i = 0; i < 2; ++i) {
+                cudaEvent_t e;
+                KAIROS_CUDA_TRY(cudaEventCreate(&e));
+                ctx->prof_events.push_back(e);
+            }
+        }
+        e0 = ctx->prof_events[ctx->prof_used];
+        e1 = ctx->prof_events[ctx->prof_used + 1];
+        ctx->prof_used += 2;
+        KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
+    }
+    const WorkItem* dev_pair = reinterpret_cast<const WorkItem*>(static_cast<uint8_t*>(st->dev) + pair_off);
+    const int n_pairs = plan.n_pairs;
+    const bool have_queue = !plan.items.empty();
+    if (n_pairs > 0 && have_queue) {  // pair grid first (it needs whole SM pairs), decode grid beside it
+        KAIROS_CUDA_TRY(cudaEventRecord(ctx->ev_fork, stream));
+        KAIROS_CUDA_TRY(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_fork, 0));
+        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, ctx->aux_stream)) return rc;
+        KAIROS_CUDA_TRY(cudaEventRecord(ctx->ev_join, ctx->aux_stream));
+    } else if (n_pairs > 0) {
+        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream)) return rc;
+    }
+    if (have_queue) {
+        if (int rc = launch_attn_umma(ctx, a, reinterpret_cast<const WorkItem*>(st->dev), int32_t(plan.items.size()),
+                                      reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
+                                      int32_t(plan.combines.size()), stream, &kernels, umma_resident_ctas(ctx) - 2 * n_pairs))
+            return rc;
+        if (n_pairs > 0) KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, ctx->ev_join, 0));
+    }
+    if (n_pairs > 0) ++kernels;
+    if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
+    if (!plan.combines.empty()) {
+        if (int rc = launch_combine(ctx, a, reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
+                                    int32_t(plan.combines.size()), stream))
+            return rc;
+        ++kernels;
+    }
     if (dbg) {
         auto T4 = now();
         t_plan += us(T0, T1); t_stage += us(T1, T2); t_copy += us(T2, T3); t_launch += us(T3, T4);
@@ -131,7 +173,7 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     }
     ctx->last_info[0] = int64_t(plan.items.size());
     ctx->last_info[1] = plan.n_decode_items;
-    ctx->last_info[2] = plan.n_chunk_items;
+    ctx->last_info[2] = plan.n_chunk_items + int64_t(plan.pair_items.size());
     ctx->last_info[3] = std::min<int64_t>(umma_resident_ctas(ctx), int64_t(plan.items.size()));
     ctx->last_info[4] = kernels;
     ctx->last_info[5] = int64_t(ws_needed);
@@ -181,6 +223,11 @@ int kairos_create(const kairos_config* cfg, kairos_ctx** out) {
             delete ctx;
             return rc;
         }
+        if (int rc = pair_init(ctx)) {
+            delete ctx;
+            return rc;
+        }
+        if (const char* fp = std::getenv("KAIROS_PAIRS")) ctx->force_pairs = std::atoi(fp);  // debug / sweeps: 0 = gen-1 chunk tiles only
     }
     *out = ctx;
     return KAIROS_OK;
@@ -197,6 +244,9 @@ int kairos_destroy(kairos_ctx* ctx) {
     }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
     for (auto e : ctx->prof_events) cudaEventDestroy(e);
+    if (ctx->aux_stream) cudaStreamDestroy(ctx->aux_stream);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete ctx;
     return KAIROS_OK;
 }
@@ -325,14 +375,20 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
 }
 
 int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t n_ctas,
-                     int32_t* items_out, int32_t max_items, int32_t* n_items_out, int32_t* n_partial_slots_out) {
+                     int32_t pair_mode, int32_t* items_out, int32_t max_items, int32_t* n_items_out,
+                     int32_t* n_partial_slots_out, int32_t* n_pairs_out) {
     if (n_dec < 0 || chunk_len < 0 || prefix_len < 0 || n_ctas < 1 || max_items < 0 || !n_items_out)
         return fail(KAIROS_ERR_INVALID_ARG, "bad size or NULL n_items_out");
     if (n_dec > 0 && !dec_ctx_lens) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens is NULL");
     for (int32_t i = 0; i < n_dec; ++i)
         if (dec_ctx_lens[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens[" + std::to_string(i) + "] < 1");
     Plan plan;
-    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, n_ctas, umma_chunk_tile_tokens(), &plan);
+    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, n_ctas, umma_chunk_tile_tokens(), &plan, pair_mode, pair_tile_tokens());
+    for (WorkItem w : plan.pair_items) {  // appended after the queue, marked kind 2
+        w.kind = 2;
+        plan.items.push_back(w);
+    }
+    if (n_pairs_out) *n_pairs_out = plan.n_pairs;
     *n_items_out = int32_t(plan.items.size());
     if (n_partial_slots_out) *n_partial_slots_out = plan.n_partial_slots;
     if (items_out)

@@ -657,7 +657,7 @@ int umma_init(kairos_ctx* ctx) {
 }
 
 int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
-                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched) {
+                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched, int max_ctas) {
     CUtensorMap qd_map = ctx->pool_map, qc_map = ctx->pool_map;  // placeholders when a side is empty (never dereferenced)
     if (a.n_dec > 0)
         if (int rc = encode_rows_map(&qd_map, a.q_dec, uint64_t(a.n_dec) * kHeads, 16)) return rc;
@@ -678,26 +678,23 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.lse_chunk = a.lse_chunk;
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
-    const int grid = std::min(n_items, umma_resident_ctas(ctx));
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (ctx->profile) {
-        if (ctx->prof_used + 2 > ctx->prof_events.size()) {
-            for (int i = 0; i < 2; ++i) {
-                cudaEvent_t e;
-                KAIROS_CUDA_TRY(cudaEventCreate(&e));
-                ctx->prof_events.push_back(e);
-            }
-        }
-        e0 = ctx->prof_events[ctx->prof_used];
-        e1 = ctx->prof_events[ctx->prof_used + 1];
-        ctx->prof_used += 2;
-        KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
-    }
+    const int grid = std::max(1, std::min(n_items, std::min(max_ctas, umma_resident_ctas(ctx))));
     kairos_mixed_kernel<<<grid, kThreads, kSmemBytes, stream>>>(ctx->pool_map, qd_map, qc_map, p);
     KAIROS_CUDA_TRY(cudaGetLastError());
-    if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
     *kernels_launched = 1;
+    (void)dev_combines;
+    (void)n_combines;
+    return KAIROS_OK;
+}
+
+// a5 launch (after the attention kernels of the step; programmatic dependent launch on the preceding kernel)
+int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream) {
     if (n_combines > 0) {
+        const uint8_t* partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
+        __nv_bfloat16* out_dec = reinterpret_cast<__nv_bfloat16*>(a.out_dec);
+        __nv_bfloat16* out_chunk = reinterpret_cast<__nv_bfloat16*>(a.out_chunk);
+        float* lse_dec = a.lse_dec;
+        float* lse_chunk = a.lse_chunk;
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(unsigned(n_combines), kCombineSlices, 1);
         cfg.blockDim = dim3(kCombineThreads, 1, 1);
@@ -708,10 +705,8 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        const uint8_t* cparts = p.partials;
-        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, cparts, p.out_dec, p.out_chunk, p.lse_dec, p.lse_chunk));
+        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, partials, out_dec, out_chunk, lse_dec, lse_chunk));
         KAIROS_CUDA_TRY(cudaGetLastError());
-        *kernels_launched = 2;
     }
     return KAIROS_OK;
 }

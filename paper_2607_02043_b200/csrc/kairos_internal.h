@@ -55,15 +55,19 @@ struct CombineItem {
 struct Plan {
     std::vector<WorkItem> items;       // execution order (longest first)
     std::vector<CombineItem> combines;
+    std::vector<WorkItem> pair_items;  // chunk tiles of 8 tokens for the 2-CTA pair kernel (empty: chunk runs as gen-1 tiles)
+    int32_t n_pairs = 0;               // clusters the pair kernel is launched with (SMs 2*n_pairs are taken from the decode grid)
     int32_t n_decode_items = 0;
     int32_t n_chunk_items = 0;
     int32_t n_partial_slots = 0;
 };
 
 // Host planner (a0): pure integer code, no CUDA.  `target_ctas` = resident CTAs the launch will have.
-// chunk_tile_tokens = query tokens per chunk tile.  See plan.cpp.
+// chunk_tile_tokens = query tokens per chunk tile.  pair_mode: 0 = chunk as gen-1 tiles in the same queue, -1 = let the
+// planner decide whether (and on how many SM pairs) the chunk runs on the pair kernel, n > 0 = force n pairs.  See plan.cpp.
 void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len,
-                int32_t target_ctas, int32_t chunk_tile_tokens, Plan* plan);
+                int32_t target_ctas, int32_t chunk_tile_tokens, Plan* plan, int32_t pair_mode = 0,
+                int32_t pair_tile_tokens = 8);
 
 constexpr size_t kPartialSlotBytes = size_t(kHeads) * kLatent * 4 + size_t(kHeads) * 2 * 4;  // o[16][512] f32 + (m,l)[16]
 
@@ -89,6 +93,10 @@ struct kairos_ctx {
     int impl = 1;                 // 0 = simple CUDA-core kernel (debug cross-check), 1 = tcgen05 path
     CUtensorMap pool_map;         // TMA descriptor of the pool (filled when impl needs it)
     bool has_pool_map = false;
+    CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
+    cudaStream_t aux_stream = nullptr;  // the pair kernel runs beside the decode kernel on this stream (event fork / join)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int force_pairs = -1;         // KAIROS_PAIRS env: -1 auto, 0 never use the pair kernel, n > 0 use n pairs
     static constexpr int kStagingSlots = 4;
     kairos::StagingSlot staging[kStagingSlots];
     int staging_next = 0;
@@ -133,7 +141,15 @@ int launch_attn_simple(kairos_ctx* ctx, const StepArgs& a, const int32_t* dev_le
 int umma_chunk_tile_tokens();
 int umma_resident_ctas(const kairos_ctx* ctx);
 int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
-                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched);
+                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched,
+                     int max_ctas);
+int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream);
 int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
+
+// impl 1, chunk tiles on 2-CTA clusters (attn_pair.cu)
+int pair_tile_tokens();
+int pair_init(kairos_ctx* ctx);
+int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,
+                     cudaStream_t stream);
 
 }  // namespace kairos

@@ -15,14 +15,72 @@ constexpr int kChunkCostNum = 3;       // cost of one chunk tile-page relative t
 constexpr int kChunkCostDen = 4;       // (tensor-bound tile-page vs HBM-bound decode page; measured)
 
 inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b); }
+
+// Cost model of the static SM partition between the pair kernel (chunk) and the decode grid, in SM cycles (measured on
+// B200): one 8-token tile x 64-key page on a pair; one decode page on one CTA; the HBM floor per page.
+constexpr int64_t kPairPageCycles = 1400;
+constexpr int64_t kDecPageCycles = 3000;
+constexpr int64_t kDecPageHbmCycles = 22;
+
+void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t ctas,
+                  int32_t pair_mode, int32_t T2, Plan* plan) {
+    if (pair_mode == 0 || chunk_len <= 0 || ctas < 2) return;
+    const int32_t n_tiles = ceil_div(chunk_len, T2);
+    int64_t pair_pages = 0;
+    for (int32_t t = 0; t < n_tiles; ++t)
+        pair_pages += ceil_div(int64_t(prefix_len) + std::min(chunk_len, (t + 1) * T2), kPage);
+    int64_t dec_pages = 0;
+    for (int32_t i = 0; i < n_dec; ++i) dec_pages += ceil_div(dec_ctx_lens[i], kPage);
+    const int32_t max_pairs = std::min(n_tiles, n_dec > 0 ? (ctas - 1) / 2 : ctas / 2);
+    if (max_pairs < 1) return;
+    int32_t n_p;
+    if (pair_mode > 0) {
+        n_p = std::min(pair_mode, max_pairs);
+    } else {
+        if (pair_pages < 4 * int64_t(ctas / 2)) return;  // small chunk: gen-1 tiles ride in the decode queue
+        if (n_dec == 0) {
+            n_p = max_pairs;
+        } else {
+            int64_t best = -1;
+            n_p = 1;
+            for (int32_t c = 1; c <= max_pairs; ++c) {
+                const int64_t tc = pair_pages * kPairPageCycles / c;
+                const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmCycles);
+                const int64_t t = std::max(tc, td);
+                if (best < 0 || t < best) { best = t; n_p = c; }
+            }
+        }
+    }
+    plan->n_pairs = n_p;
+    for (int32_t t = 0; t < n_tiles; ++t) {
+        WorkItem w{};
+        w.kind = 1;
+        w.q_index = t * T2;
+        w.n_q = std::min(chunk_len, (t + 1) * T2) - t * T2;
+        w.page_begin = 0;
+        w.page_end = ceil_div(int64_t(prefix_len) + w.q_index + w.n_q, kPage);
+        w.n_keys = prefix_len + w.q_index + 1;
+        w.partial_slot = -1;
+        w.cost = w.page_end;
+        plan->pair_items.push_back(w);
+    }
+    std::stable_sort(plan->pair_items.begin(), plan->pair_items.end(), [](const WorkItem& a, const WorkItem& b) { return a.cost > b.cost; });
+}
 }  // namespace
 
 void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len,
-                int32_t target_ctas, int32_t T, Plan* plan) {
+                int32_t target_ctas, int32_t T, Plan* plan, int32_t pair_mode, int32_t T2) {
     plan->items.clear();
     plan->combines.clear();
+    plan->pair_items.clear();
+    plan->n_pairs = 0;
     plan->n_decode_items = plan->n_chunk_items = plan->n_partial_slots = 0;
     if (target_ctas < 1) target_ctas = 1;
+    choose_pairs(dec_ctx_lens, n_dec, chunk_len, prefix_len, target_ctas, pair_mode, T2, plan);
+    if (plan->n_pairs > 0) {  // the chunk runs on its own SM pairs: the queue below holds decode splits only
+        chunk_len = 0;
+        target_ctas = std::max(1, target_ctas - 2 * plan->n_pairs);
+    }
 
     // ---- total cost, in units of 4*decode-page
     int64_t dec_pages = 0;

@@ -52,7 +52,7 @@ _lib.kairos_mixed_step_host.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i
 _lib.kairos_mixed_step_host.restype = _c.c_int
 _lib.kairos_step_latency_table.argtypes = [_vp, _vp, _i32, _vp, _i32, _vp, _i32, _i32, _i32, _i32, _i32, _vp, _vp, _vp]
 _lib.kairos_step_latency_table.restype = _c.c_int
-_lib.kairos_plan_dump.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp, _i32, _vp, _vp]
+_lib.kairos_plan_dump.argtypes = [_vp, _i32, _i32, _i32, _i32, _i32, _vp, _i32, _vp, _vp, _vp]
 _lib.kairos_plan_dump.restype = _c.c_int
 _lib.kairos_last_plan_info.argtypes = [_vp, _vp, _i32]
 _lib.kairos_last_plan_info.restype = _c.c_int
@@ -218,16 +218,19 @@ class Kairos:
         return dict(zip(keys, (int(x) for x in info)))
 
 
-def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ctas: int = 148):
-    """Host planner alone (kairos_plan_dump): (items int32 [n, 8] in queue order, n_partial_slots). No GPU needed."""
+def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ctas: int = 148, pair_mode: int = 0,
+              with_pairs: bool = False):
+    """Host planner alone (kairos_plan_dump): (items int32 [n, 8], n_partial_slots[, n_pairs]). No GPU needed."""
     lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
-    n, slots = _c.c_int32(0), _c.c_int32(0)
+    n, slots, pairs = _c.c_int32(0), _c.c_int32(0), _c.c_int32(0)
     lp = lens.ctypes.data_as(_vp) if lens.size else None
-    _check(_lib.kairos_plan_dump(lp, int(lens.size), int(chunk_len), int(prefix_len), int(n_ctas), None, 0,
-                                 _c.byref(n), _c.byref(slots)))
+    args = (lp, int(lens.size), int(chunk_len), int(prefix_len), int(n_ctas), int(pair_mode))
+    _check(_lib.kairos_plan_dump(*args, None, 0, _c.byref(n), _c.byref(slots), _c.byref(pairs)))
     items = np.zeros((int(n.value), 8), dtype=np.int32)
-    _check(_lib.kairos_plan_dump(lp, int(lens.size), int(chunk_len), int(prefix_len), int(n_ctas),
-                                 items.ctypes.data_as(_vp), int(n.value), _c.byref(n), _c.byref(slots)))
+    _check(_lib.kairos_plan_dump(*args, items.ctypes.data_as(_vp), int(n.value), _c.byref(n), _c.byref(slots),
+                                 _c.byref(pairs)))
+    if with_pairs:
+        return items, int(slots.value), int(pairs.value)
     return items, int(slots.value)
 
 
