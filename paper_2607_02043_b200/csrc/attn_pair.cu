@@ -30,10 +30,12 @@ constexpr int kPairTileTokens = 8;
 constexpr int kPairThreads = 192;            // warp 0 TMA producer (+ queue on rank 0), warp 1 MMA issuer, warps 2-5 softmax / epilogue
 constexpr int kKStage = kPage * kTokenBytes;  // 73,728: K page, all 576 dims (S-CTA)
 constexpr int kVStage = kPage * kLatent * 2;  // 65,536: latent part only (O-CTA)
-constexpr int kStages = 3;
+constexpr int kStages = 3;                    // V stages of the O-CTA
+constexpr int kStagesK = 2;                   // K stages of the S-CTA (the rest of its shared memory stages P for the bulk copy)
+constexpr int kOffPStage = kStagesK * kKStage; // S-CTA: local P staging, 2 x 16 KB
 constexpr int kPBytes = 128 * 128;            // P[128 rows][64 keys] bf16, SWIZZLE_128B K-major
 constexpr int kOffP = kStages * kVStage;      // O-CTA: P buffers after the V stages
-constexpr int kOffSmallS = kStages * kKStage;               // 221,184
+constexpr int kOffSmallS = kStagesK * kKStage + 2 * kPBytes + 1024;  // P staging + alpha staging
 constexpr int kOffSmallO = kStages * kVStage + 2 * kPBytes;  // 229,376
 constexpr int kPairSmallBytes = 2048;
 constexpr int kPairSmem = (kOffSmallO > kOffSmallS ? kOffSmallO : kOffSmallS) + kPairSmallBytes + 1024;
@@ -58,13 +60,19 @@ struct PairSmall {
     uint64_t item_full[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
-    uint32_t flag[2];      // O-CTA: page g needs an O rescale (written by the S-CTA)
-    float alpha[2][128];   // O-CTA: rescale factors of page g
+    alignas(16) float alpha[2][128];  // O-CTA: per-row O rescale factors of page g (bulk-copied with P; 1 = none)
     float linv[128];       // O-CTA: 1 / l per row at the end of the item
 };
 static_assert(sizeof(PairSmall) <= kPairSmallBytes, "PairSmall does not fit");
 
+#ifdef KAIROS_TRACE
+#define PTRACE(ev, g) do { if (blockIdx.x < 2 && (g) < 64) p.trace[(ev) * 64 + (g)] = clock64(); } while (0)
+#else
+#define PTRACE(ev, g) do { } while (0)
+#endif
+
 struct PairParams {
+    unsigned long long* trace;
     const WorkItem* items;
     int32_t n_items;
     int32_t* counter;      // queue head of the pair kernel
@@ -102,24 +110,11 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi) {
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
-__device__ __forceinline__ bool softmax_or(bool pred) {  // bar.red.or over the 128 softmax threads (named barrier 3)
-    uint32_t r;
-    asm volatile(
-        "{\n\t.reg .pred p, q;\n\t"
-        "setp.ne.u32 p, %1, 0;\n\t"
-        "bar.red.or.pred q, 3, 128, p;\n\t"
-        "selp.u32 %0, 1, 0, q;\n\t}"
-        : "=r"(r)
-        : "r"(uint32_t(pred))
-        : "memory");
-    return r != 0;
-}
-
 // ------------------------------------------------------------------------------------------------------------
 // S-CTA, softmax warps (128 threads, thread = query row `row` = TMEM lane).  peer_* are shared::cluster addresses in
 // the O-CTA.  g counts pages over the whole kernel (S buffer / P buffer = g & 1), `it` counts items.
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint32_t peer_small, uint32_t peer_p, const WorkItem& w,
+__device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, uint32_t peer_small, uint32_t peer_p, const WorkItem& w,
                                                 const PairParams& p, uint32_t tmem, int row, int q4, int lane, uint32_t& g,
                                                 uint32_t it) {
     const int tok = row >> 4, head = row & 15;
@@ -152,6 +147,7 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint32_t peer_sma
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
         mbar_wait(&sm->s_full[b], ph);
+        if (row == 0) PTRACE(2, g);
         tc_fence_after();
         float x[64];
         tmem_ld32(tmem + lane_base + kColS2 + b * 64, reinterpret_cast<uint32_t*>(x));
@@ -160,6 +156,7 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint32_t peer_sma
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->s_empty[b]);
+        if (row == 0) PTRACE(3, g);
 
         const int key0 = (w.page_begin + pg) * kPage;
         const bool boundary = key0 + kPage > w.n_keys;  // some row of the tile does not see every key of this page
@@ -179,7 +176,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint32_t peer_sma
         }
         // thresholded running max: the reference moves only when the page's max exceeds it by more than 2^8
         const bool need = tm - m_ref > kRescaleThreshold2;
-        const bool any = softmax_or(need);
         float alpha = 1.f;
         if (need) {
             alpha = ex2f(m_ref - tm);  // 0 on the first visible page (m_ref = -1e30)
@@ -194,39 +190,59 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint32_t peer_sma
         }
         l += sum;
         // ---- P row (bf16, 128 B) -> O-CTA shared memory, K-major SWIZZLE_128B: row r at r*128, 16-B chunk c at c ^ (r & 7)
+        if (row == 0) PTRACE(4, g);
         mbar_wait_cluster(&sm->p_empty[b], ph ^ 1);
-        const uint32_t prow = peer_p + b * kPBytes + uint32_t(row) * 128u;
+        if (row == 0) PTRACE(5, g);
+        // local staging (K-major SWIZZLE_128B: row r at r*128, 16-B chunk c at c ^ (r & 7)), then one 4 KB bulk copy per
+        // warp into the O-CTA's P buffer, completing on its p_full mbarrier (DSMEM moves ~20 B/clk: asynchronous, so the
+        // softmax threads do not wait for it)
+        uint8_t* prow = pstage + b * kPBytes + row * 128;
 #pragma unroll
-        for (int c = 0; c < 8; ++c)
-            st_cluster_v4(prow + (uint32_t(c ^ (row & 7)) << 4), pack2(x[8 * c + 0], x[8 * c + 1]), pack2(x[8 * c + 2], x[8 * c + 3]),
-                          pack2(x[8 * c + 4], x[8 * c + 5]), pack2(x[8 * c + 6], x[8 * c + 7]));
-        const bool rescale = any && pg > 0;  // on the first page O is overwritten (accumulate = 0): nothing to rescale
-        if (rescale) st_cluster_b32(peer_small + uint32_t(offsetof(PairSmall, alpha)) + (b * 128 + row) * 4, __float_as_uint(alpha));
-        if (row == 0) st_cluster_b32(peer_small + uint32_t(offsetof(PairSmall, flag)) + b * 4, rescale ? 1u : 0u);
-        fence_proxy_async_all();
-        asm volatile("fence.acq_rel.cluster;" ::: "memory");
+        for (int c = 0; c < 8; ++c) {
+            uint4 v;
+            v.x = pack2(x[8 * c + 0], x[8 * c + 1]);
+            v.y = pack2(x[8 * c + 2], x[8 * c + 3]);
+            v.z = pack2(x[8 * c + 4], x[8 * c + 5]);
+            v.w = pack2(x[8 * c + 6], x[8 * c + 7]);
+            *reinterpret_cast<uint4*>(prow + ((c ^ (row & 7)) << 4)) = v;
+        }
+        // rescale factor of this row for the O-CTA (1 = leave O alone; on the first page O is overwritten, accumulate = 0):
+        // staged next to P and bulk-copied too, so the per-page path has no generic-proxy remote store at all
+        reinterpret_cast<float*>(pstage + 2 * kPBytes)[b * 128 + row] = pg > 0 ? alpha : 1.f;
+        fence_proxy_async_smem();
         __syncwarp();
-        if (lane == 0) mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, p_full)) + b * 8);
+        if (lane == 0) {
+            const uint32_t bar = peer_small + uint32_t(offsetof(PairSmall, p_full)) + b * 8;
+            asm volatile("mbarrier.arrive.expect_tx.relaxed.cluster.shared::cluster.b64 _, [%0], %1;" ::"r"(bar), "r"(4096u + 128u) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(peer_p + b * kPBytes + uint32_t(q4) * 4096u), "r"(smem_u32(pstage + b * kPBytes + q4 * 4096)), "r"(4096u), "r"(bar)
+                         : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(peer_small + uint32_t(offsetof(PairSmall, alpha)) + (b * 128 + q4 * 32) * 4),
+                           "r"(smem_u32(pstage + 2 * kPBytes + (b * 128 + q4 * 32) * 4)), "r"(128u), "r"(bar)
+                         : "memory");
+        }
+        if (row == 0) PTRACE(6, g);
     }
     // ---- end of item: 1 / l to the O-CTA's epilogue; lse from here
     mbar_wait_cluster(&sm->fin_empty, (it & 1) ^ 1);
     st_cluster_b32(peer_small + uint32_t(offsetof(PairSmall, linv)) + row * 4, __float_as_uint(1.f / l));
-    asm volatile("fence.acq_rel.cluster;" ::: "memory");
-    __syncwarp();
-    if (lane == 0) mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, fin_full)));
+    mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, fin_full)));
     if (tok < w.n_q && p.lse_chunk) p.lse_chunk[size_t(w.q_index + tok) * kHeads + head] = (m_ref + log2f(l)) * kLn2b;
 }
 
 // S-CTA, MMA warp (converged; one elected lane issues)
-__device__ __forceinline__ void sc_mma_item(PairSmall* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t& g, uint32_t it) {
+__device__ __forceinline__ void sc_mma_item(PairSmall* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t& g, uint32_t it,
+                                            const PairParams& p) {
     constexpr uint32_t idesc = make_idesc_bf16(128, 64, 0, 0);
     constexpr uint32_t hi = smem_desc_hi(1024);
     mbar_wait(&sm->q_ready, it & 1);
     tc_fence_after();
     for (int pg = 0; pg < npages; ++pg, ++g) {
-        const uint32_t st = g % kStages, sph = (g / kStages) & 1, b = g & 1, bph = (g >> 1) & 1;
+        const uint32_t st = g % kStagesK, sph = (g / kStagesK) & 1, b = g & 1, bph = (g >> 1) & 1;
         mbar_wait(&sm->kv_full[st], sph);
         mbar_wait(&sm->s_empty[b], bph ^ 1);
+        PTRACE(0, g);
         tc_fence_after();
         const uint32_t kb_lo = smem_desc_lo(kv_base + st * kKStage, 16);
 #pragma unroll
@@ -237,6 +253,7 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, uint32_t tmem, uint32
                                   idesc, (c | j) != 0);
         umma_commit_elect(&sm->s_full[b]);
         umma_commit_elect(&sm->kv_empty[st]);
+        PTRACE(1, g);
     }
     umma_commit_elect(&sm->q_free);
 }
@@ -252,11 +269,11 @@ __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_sm
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
         mbar_wait_cluster(&sm->p_full[b], ph);
-        if (*reinterpret_cast<volatile uint32_t*>(&sm->flag[b]) != 0u) {
+        const float a = *reinterpret_cast<volatile float*>(&sm->alpha[b][row]);
+        if (__any_sync(0xffffffffu, a != 1.f)) {  // warp-uniform: tcgen05.ld / st are warp-collective
             // a row's reference max moved: every PV issued so far must have landed before O is rescaled
             mbar_wait(&sm->pv_done[(g - 1) & 1], ((g - 1) >> 1) & 1);
             tc_fence_after();
-            const float a = *reinterpret_cast<volatile float*>(&sm->alpha[b][row]);
 #pragma unroll 1
             for (int c = 0; c < 16; ++c) {
                 uint32_t r[32];
@@ -308,15 +325,17 @@ __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_sm
 
 // O-CTA, MMA warp
 __device__ __forceinline__ void oc_mma_item(PairSmall* sm, uint32_t peer_small, uint32_t tmem, uint32_t v_base, uint32_t p_base,
-                                            int npages, uint32_t& g, uint32_t it) {
+                                            int npages, uint32_t& g, uint32_t it, const PairParams& p) {
     constexpr uint32_t idesc = make_idesc_bf16(128, 256, 0, 1);  // A = P K-major, B = V page MN-major
     constexpr uint32_t hi = smem_desc_hi(1024);
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t st = g % kStages, sph = (g / kStages) & 1, b = g & 1, bph = (g >> 1) & 1;
         mbar_wait(&sm->corr_done[b], bph);
+        PTRACE(7, g);
         mbar_wait(&sm->v_full[st], sph);
         if (pg == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O
-        fence_proxy_async_all();  // P arrived through the generic proxy of the peer's threads
+        PTRACE(8, g);
+        fence_proxy_async_smem();  // P arrived through the generic proxy of the peer's threads
         tc_fence_after();
         const uint32_t pa_lo = smem_desc_lo(p_base + b * kPBytes, 16);
         const uint32_t vb_lo = smem_desc_lo(v_base + st * kVStage, 8192);
@@ -330,6 +349,7 @@ __device__ __forceinline__ void oc_mma_item(PairSmall* sm, uint32_t peer_small, 
         umma_commit_elect(&sm->pv_done[b]);
         umma_commit_elect_addr(peer_small + uint32_t(offsetof(PairSmall, p_empty)) + b * 8);
         if (pg == npages - 1) umma_commit_elect(&sm->o_full);
+        PTRACE(9, g);
     }
 }
 
@@ -365,10 +385,9 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
         mbar_init(&sm->q_ready, 4);
         mbar_init(&sm->q_free, 1);
         mbar_init(&sm->fin_empty, 4);
-        mbar_init(&sm->fin_full, 4);
+        mbar_init(&sm->fin_full, 128);
         mbar_init(&sm->o_full, 1);
         mbar_init(&sm->o_empty, 4);
-        sm->flag[0] = sm->flag[1] = 0u;
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) prefetch_tensormap(rank == 0 ? &pool_map_k : &pool_map_v);
@@ -413,7 +432,8 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
-                        const uint32_t st = g % kStages, sph = (g / kStages) & 1;
+                        const uint32_t ns = rank == 0 ? kStagesK : kStages;
+                        const uint32_t st = g % ns, sph = (g / ns) & 1;
                         if (rank == 0) {
                             mbar_wait(&sm->kv_empty[st], sph ^ 1);
                             mbar_arrive_expect_tx(&sm->kv_full[st], kKStage);
@@ -450,10 +470,10 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             const WorkItem w = load_item2(p.items + idx);
             const int npages = w.page_end - w.page_begin;
             if (warp == 1) {
-                if (rank == 0) sc_mma_item(sm, tmem, smem_u32(base), npages, g, it);
-                else oc_mma_item(sm, peer_small, tmem, smem_u32(base), smem_u32(base + kOffP), npages, g, it);
+                if (rank == 0) sc_mma_item(sm, tmem, smem_u32(base), npages, g, it, p);
+                else oc_mma_item(sm, peer_small, tmem, smem_u32(base), smem_u32(base + kOffP), npages, g, it, p);
             } else {
-                if (rank == 0) sc_softmax_item(sm, peer_small, peer_p, w, p, tmem, row, q4, lane, g, it);
+                if (rank == 0) sc_softmax_item(sm, base + kOffPStage, peer_small, peer_p, w, p, tmem, row, q4, lane, g, it);
                 else oc_epilogue_item(sm, peer_small, w, p, tmem, row, q4, lane, g, it);
             }
         }
@@ -507,6 +527,7 @@ int pair_init(kairos_ctx* ctx) {
 int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,
                      cudaStream_t stream) {
     PairParams p;
+    p.trace = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + ctx->cfg.workspace_bytes - 8192);  // KAIROS_TRACE builds only
     p.items = dev_items;
     p.n_items = n_items;
     p.counter = reinterpret_cast<int32_t*>(ctx->cfg.workspace) + 2;

@@ -18,7 +18,7 @@ inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b);
 
 // Cost model of the static SM partition between the pair kernel (chunk) and the decode grid, in SM cycles (measured on
 // B200): one 8-token tile x 64-key page on a pair; one decode page on one CTA; the HBM floor per page.
-constexpr int64_t kPairPageCycles = 1400;
+constexpr int64_t kPairPageCycles = 1650;
 constexpr int64_t kDecPageCycles = 3000;
 constexpr int64_t kDecPageHbmCycles = 22;
 
