@@ -35,7 +35,9 @@ constexpr int kStagesK = 2;                   // K stages of the S-CTA (the rest
 constexpr int kOffPStage = kStagesK * kKStage; // S-CTA: local P staging, 2 x 16 KB
 constexpr int kPBytes = 128 * 128;            // P[128 rows][64 keys] bf16, SWIZZLE_128B K-major
 constexpr int kOffP = kStages * kVStage;      // O-CTA: P buffers after the V stages
-constexpr int kOffSmallS = kStagesK * kKStage + 2 * kPBytes + 1024;  // P staging + alpha staging
+constexpr int kOffQStage = kStagesK * kKStage + 2 * kPBytes + 2048;  // S-CTA: two 16 KB TMA landing buffers for Q chunks (1024-aligned)
+static_assert(kOffQStage % 1024 == 0, "SWIZZLE_128B tiles need 1024-byte alignment");
+constexpr int kOffSmallS = kOffQStage + 2 * 16384;  // P staging + alpha staging (1 KB) + linv staging (512 B)
 constexpr int kOffSmallO = kStages * kVStage + 2 * kPBytes;  // 229,376
 constexpr int kPairSmallBytes = 2048;
 constexpr int kPairSmem = (kOffSmallO > kOffSmallS ? kOffSmallO : kOffSmallS) + kPairSmallBytes + 1024;
@@ -47,13 +49,24 @@ constexpr float kRescaleThreshold2 = 8.0f;
 constexpr float kLn2b = 0.6931471805599453f;
 constexpr float kMinusHuge2 = -1.0e30f;
 
+// S-CTA only (lives in its otherwise unused shared memory at kOffSmallS): one barrier pair per slot of the K ring (a group
+// of chunks of one page); a slot is refilled as soon as its MMAs retire.
+constexpr int kGroupChunks = 3;  // chunks per ring slot (24 KB): an mbarrier wait costs the issuing warp ~100 cycles even when
+                                 // complete, so per-chunk slots (9 waits per page) made the MMA warp issue-bound
+constexpr int kGroups = 9 / kGroupChunks;
+struct ScRing {
+    uint64_t kv_full[kStagesK * kGroups], kv_empty[kStagesK * kGroups];
+};
+static_assert(kOffSmallS + int(sizeof(ScRing)) <= kOffSmallO, "ScRing overlaps the shared small struct");
+
 // One struct for both ranks (same offsets in both CTAs, so mapa of a local address names the peer's copy).
 struct PairSmall {
     // S-CTA
-    uint64_t kv_full[kStages], kv_empty[kStages], s_full[2], s_empty[2], q_ready, q_free;
+    uint64_t s_full[2], s_empty[2], q_ready, q_free;
     uint64_t p_empty[2];   // arrived by the O-CTA's tcgen05.commit when PV(g) has consumed P buffer g & 1
     uint64_t fin_empty;    // arrived by the O-CTA's epilogue warps: linv[] may be overwritten
     uint64_t item_empty[2];
+    uint64_t qst_full[2];  // Q chunk landed in staging buffer (TMA)
     // O-CTA
     uint64_t v_full[kStages], v_empty[kStages], p_full[2], corr_done[2], pv_done[2], o_full, o_empty, fin_full;
     // both
@@ -61,7 +74,7 @@ struct PairSmall {
     int32_t item_ring[2];
     uint32_t tmem_base;
     alignas(16) float alpha[2][128];  // O-CTA: per-row O rescale factors of page g (bulk-copied with P; 1 = none)
-    float linv[128];       // O-CTA: 1 / l per row at the end of the item
+    alignas(16) float linv[128];      // O-CTA: 1 / l per row at the end of the item (bulk-copied)
 };
 static_assert(sizeof(PairSmall) <= kPairSmallBytes, "PairSmall does not fit");
 
@@ -100,6 +113,15 @@ __device__ __forceinline__ void tma_load_box3(void* smem_dst, const CUtensorMap*
           "l"(policy)
         : "memory");
 }
+__device__ __forceinline__ void tma_load_chunk(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t row, int32_t chunk,
+                                               uint64_t policy) {  // box (64 elems, 64 rows, kGroupChunks chunks)
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5}], [%2], %6;"
+        ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(0), "r"(row), "r"(chunk),
+          "l"(policy)
+        : "memory");
+}
 __device__ __forceinline__ float ex2f(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -114,33 +136,75 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi) {
 // S-CTA, softmax warps (128 threads, thread = query row `row` = TMEM lane).  peer_* are shared::cluster addresses in
 // the O-CTA.  g counts pages over the whole kernel (S buffer / P buffer = g & 1), `it` counts items.
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, uint32_t peer_small, uint32_t peer_p, const WorkItem& w,
-                                                const PairParams& p, uint32_t tmem, int row, int q4, int lane, uint32_t& g,
-                                                uint32_t it) {
-    const int tok = row >> 4, head = row & 15;
+// S-CTA: Q tile of item `it` -> TMEM (the 128 row-owning threads).  Waits for the S-MMAs of item it - 1 (q_free).
+__device__ __forceinline__ void sc_load_q(PairSmall* sm, const WorkItem& w, const PairParams& p, const CUtensorMap* qmap, uint32_t tmem,
+                                          int row, int q4, int lane, uint32_t& qcount, uint32_t it) {
     const uint32_t lane_base = uint32_t(q4 * 32) << 16;
-    // ---- Q row -> TMEM (A operand of S = Q K^T): 576 bf16 = 288 columns
+    uint8_t* qst = reinterpret_cast<uint8_t*>(sm) - kOffSmallO + kOffQStage;
+    const int row0 = w.q_index * kHeads;
+    if (row == 0) {  // the first two Q chunks start moving before the previous item's S-MMAs have retired
+        for (int c = 0; c < 2; ++c) {
+            mbar_arrive_expect_tx(&sm->qst_full[c], 16384);
+            tma_load_2d(qst + c * 16384, qmap, &sm->qst_full[c], c * 64, row0, kEvictFirst);
+        }
+    }
+    if (row == 0) PTRACE(10, it * 4 + 0);
     mbar_wait(&sm->q_free, (it & 1) ^ 1);  // previous item's S-MMAs have retired
     tc_fence_after();
+    if (row == 0) PTRACE(10, it * 4 + 1);
     {
-        const uint4* src = reinterpret_cast<const uint4*>(p.q_chunk + (size_t(w.q_index) * kHeads + row) * kDim);
-        const bool live = tok < w.n_q;
-#pragma unroll
-        for (int i = 0; i < 9; ++i) {
+        // Q tile [128 rows x 576] -> TMEM through two 16 KB staging buffers: one TMA box (64 dims x 128 rows, SWIZZLE_128B,
+        // rows past the chunk's end zero-filled) per 64-dim chunk; each thread then reads its own row's 128 B (conflict
+        // free) and stores 32 TMEM columns.  (Per-thread global loads of a row cost ~10k cycles: 32 lines per LDG.)
+#pragma unroll 1
+        for (int c = 0; c < 9; ++c) {
+            const uint32_t qb = c & 1;
+            mbar_wait(&sm->qst_full[qb], (qcount >> qb) & 1);  // qcount: one phase-parity bit per staging buffer
+            qcount ^= 1u << qb;
+            const uint8_t* src = qst + qb * 16384 + row * 128;
             uint32_t r[32];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const uint4 v = live ? __ldg(src + i * 8 + j) : make_uint4(0u, 0u, 0u, 0u);
+                const uint4 v = *reinterpret_cast<const uint4*>(src + ((j ^ (row & 7)) << 4));
                 r[4 * j + 0] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
             }
-            tmem_st32(tmem + lane_base + kColQ + 32 * i, r);
+            tmem_st32(tmem + lane_base + kColQ + 32 * c, r);
+            if (c + 2 < 9) {
+                asm volatile("bar.sync 3, 128;" ::: "memory");  // every row has read this buffer
+                if (row == 0) {
+                    mbar_arrive_expect_tx(&sm->qst_full[qb], 16384);
+                    tma_load_2d(qst + qb * 16384, qmap, &sm->qst_full[qb], (c + 2) * 64, row0, kEvictFirst);
+                }
+            }
         }
         tmem_wait_st();
     }
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->q_ready);
+    if (row == 0) PTRACE(10, it * 4 + 2);
 
+}
+
+__device__ __forceinline__ WorkItem sc_fetch_item(PairSmall* sm, const PairParams& p, int lane, uint32_t it, int* idx_out) {
+    const uint32_t slot = it & 1, iph = (it >> 1) & 1;
+    mbar_wait(&sm->item_full[slot], iph);
+    const int idx = *reinterpret_cast<volatile int32_t*>(&sm->item_ring[slot]);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm->item_empty[slot]);
+    *idx_out = idx;
+    WorkItem w{};
+    if (idx >= 0) w = load_item2(p.items + idx);
+    return w;
+}
+
+// Processes item `it` (its Q is already in TMEM).  Before the softmax of the LAST page -- all S-MMAs of the item have
+// retired by then -- it fetches item it + 1 and loads that item's Q, so the MMA warp restarts while this item drains.
+__device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, uint32_t peer_small, uint32_t peer_p, const WorkItem& w,
+                                                const PairParams& p, const CUtensorMap* qmap, uint32_t tmem, int row, int q4, int lane,
+                                                uint32_t& g, uint32_t& qcount, uint32_t it, WorkItem* next, int* next_idx) {
+    const int tok = row >> 4, head = row & 15;
+    const uint32_t lane_base = uint32_t(q4 * 32) << 16;
     float m_ref = kMinusHuge2, l = 0.f;
     const int npages = w.page_end - w.page_begin;
     const int vis = w.n_keys + tok;  // keys visible to this row: positions < vis
@@ -148,6 +212,10 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
         mbar_wait(&sm->s_full[b], ph);
         if (row == 0) PTRACE(2, g);
+        if (pg == npages - 1) {  // every S-MMA of this item has retired: Q may be replaced
+            *next = sc_fetch_item(sm, p, lane, it + 1, next_idx);
+            if (*next_idx >= 0) sc_load_q(sm, *next, p, qmap, tmem, row, q4, lane, qcount, it + 1);
+        }
         tc_fence_after();
         float x[64];
         tmem_ld32(tmem + lane_base + kColS2 + b * 64, reinterpret_cast<uint32_t*>(x));
@@ -226,13 +294,25 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
     }
     // ---- end of item: 1 / l to the O-CTA's epilogue; lse from here
     mbar_wait_cluster(&sm->fin_empty, (it & 1) ^ 1);
-    st_cluster_b32(peer_small + uint32_t(offsetof(PairSmall, linv)) + row * 4, __float_as_uint(1.f / l));
-    mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, fin_full)));
+    {  // staged locally and bulk-copied like P (a release.cluster arrive per thread costs ~3000 cycles)
+        float* lst = reinterpret_cast<float*>(pstage + 2 * kPBytes + 1024);
+        lst[row] = 1.f / l;
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+            const uint32_t bar = peer_small + uint32_t(offsetof(PairSmall, fin_full));
+            asm volatile("mbarrier.arrive.expect_tx.relaxed.cluster.shared::cluster.b64 _, [%0], %1;" ::"r"(bar), "r"(128u) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(peer_small + uint32_t(offsetof(PairSmall, linv)) + q4 * 128), "r"(smem_u32(lst + q4 * 32)), "r"(128u), "r"(bar)
+                         : "memory");
+        }
+    }
     if (tok < w.n_q && p.lse_chunk) p.lse_chunk[size_t(w.q_index + tok) * kHeads + head] = (m_ref + log2f(l)) * kLn2b;
+    if (row == 0) PTRACE(10, it * 4 + 3);
 }
 
 // S-CTA, MMA warp (converged; one elected lane issues)
-__device__ __forceinline__ void sc_mma_item(PairSmall* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t& g, uint32_t it,
+__device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_t tmem, uint32_t kv_base, int npages, uint32_t& g, uint32_t it,
                                             const PairParams& p) {
     constexpr uint32_t idesc = make_idesc_bf16(128, 64, 0, 0);
     constexpr uint32_t hi = smem_desc_hi(1024);
@@ -240,19 +320,24 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, uint32_t tmem, uint32
     tc_fence_after();
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t st = g % kStagesK, sph = (g / kStagesK) & 1, b = g & 1, bph = (g >> 1) & 1;
-        mbar_wait(&sm->kv_full[st], sph);
         mbar_wait(&sm->s_empty[b], bph ^ 1);
         PTRACE(0, g);
-        tc_fence_after();
         const uint32_t kb_lo = smem_desc_lo(kv_base + st * kKStage, 16);
 #pragma unroll
-        for (uint32_t c = 0; c < 9; ++c)
+        for (uint32_t gr = 0; gr < kGroups; ++gr) {
+            mbar_wait(&ring->kv_full[st * kGroups + gr], sph);
+            tc_fence_after();
 #pragma unroll
-            for (uint32_t j = 0; j < 4; ++j)
-                umma_bf16_ts_lohi(tmem + kColS2 + b * 64, tmem + kColQ + (c * 4 + j) * 8, kb_lo + ((c * 8192 + j * 32) >> 4), hi,
-                                  idesc, (c | j) != 0);
+            for (uint32_t cc = 0; cc < kGroupChunks; ++cc) {
+                const uint32_t c = gr * kGroupChunks + cc;
+#pragma unroll
+                for (uint32_t j = 0; j < 4; ++j)
+                    umma_bf16_ts_lohi(tmem + kColS2 + b * 64, tmem + kColQ + (c * 4 + j) * 8, kb_lo + ((c * 8192 + j * 32) >> 4), hi,
+                                      idesc, (c | j) != 0);
+            }
+            umma_commit_elect(&ring->kv_empty[st * kGroups + gr]);
+        }
         umma_commit_elect(&sm->s_full[b]);
-        umma_commit_elect(&sm->kv_empty[st]);
         PTRACE(1, g);
     }
     umma_commit_elect(&sm->q_free);
@@ -295,23 +380,46 @@ __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_sm
     tc_fence_after();
     const float linv = *reinterpret_cast<volatile float*>(&sm->linv[row]);
     {
-        const bool live = tok < w.n_q;  // ragged last tile: dead rows still take part in the warp-collective tcgen05.ld
-        uint4* dst = reinterpret_cast<uint4*>(p.out_chunk + (size_t(w.q_index + (live ? tok : 0)) * kHeads + head) * kLatent);
+        // Each thread owns one output row; writing 16 B per row per instruction would touch 32 cache lines per store
+        // (measured: ~14k cycles per tile).  A 4x4 transpose of 16-B units inside every lane quad makes each store
+        // instruction write 64 contiguous bytes per row, 8 rows per instruction.
+        const int qd = lane & 3;
+        const int rbase = row - qd;  // first row of this quad
+        __nv_bfloat16* obase = p.out_chunk + (size_t(w.q_index) * kHeads) * kLatent;
 #pragma unroll 1
         for (int c = 0; c < 16; ++c) {
             uint32_t r[32];
             tmem_ld32(tmem + lane_base + c * 32, r);
             tmem_wait_ld();
-            if (live) {
+            uint4 e[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    uint4 v;
-                    v.x = pack2(__uint_as_float(r[8 * j + 0]) * linv, __uint_as_float(r[8 * j + 1]) * linv);
-                    v.y = pack2(__uint_as_float(r[8 * j + 2]) * linv, __uint_as_float(r[8 * j + 3]) * linv);
-                    v.z = pack2(__uint_as_float(r[8 * j + 4]) * linv, __uint_as_float(r[8 * j + 5]) * linv);
-                    v.w = pack2(__uint_as_float(r[8 * j + 6]) * linv, __uint_as_float(r[8 * j + 7]) * linv);
-                    dst[c * 4 + j] = v;
+            for (int j = 0; j < 4; ++j) {
+                e[j].x = pack2(__uint_as_float(r[8 * j + 0]) * linv, __uint_as_float(r[8 * j + 1]) * linv);
+                e[j].y = pack2(__uint_as_float(r[8 * j + 2]) * linv, __uint_as_float(r[8 * j + 3]) * linv);
+                e[j].z = pack2(__uint_as_float(r[8 * j + 4]) * linv, __uint_as_float(r[8 * j + 5]) * linv);
+                e[j].w = pack2(__uint_as_float(r[8 * j + 6]) * linv, __uint_as_float(r[8 * j + 7]) * linv);
+            }
+#pragma unroll
+            for (int m = 1; m <= 2; m <<= 1) {
+                const bool up = (qd & m) != 0;
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    if (a & m) continue;
+                    const uint4 snd = up ? e[a] : e[a ^ m];
+                    uint4 rcv;
+                    rcv.x = __shfl_xor_sync(0xffffffffu, snd.x, m);
+                    rcv.y = __shfl_xor_sync(0xffffffffu, snd.y, m);
+                    rcv.z = __shfl_xor_sync(0xffffffffu, snd.z, m);
+                    rcv.w = __shfl_xor_sync(0xffffffffu, snd.w, m);
+                    if (up) e[a] = rcv; else e[a ^ m] = rcv;
                 }
+            }
+            // e[i] now holds 16-B unit `qd` of row rbase + i
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int rr = rbase + i;
+                if ((rr >> 4) < w.n_q)
+                    *reinterpret_cast<uint4*>(obase + size_t(rr) * kLatent + c * 32 + qd * 8) = e[i];
             }
         }
     }
@@ -356,19 +464,22 @@ __device__ __forceinline__ void oc_mma_item(PairSmall* sm, uint32_t peer_small, 
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kPairThreads, 1)
 kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const __grid_constant__ CUtensorMap pool_map_v,
-                         const PairParams p) {
+                         const __grid_constant__ CUtensorMap q_map, const PairParams p) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t rank = cluster_ctarank();  // 0 = S-CTA, 1 = O-CTA
     PairSmall* sm = reinterpret_cast<PairSmall*>(base + kOffSmallO);  // same offset on both ranks (beyond both layouts)
+    ScRing* ring = reinterpret_cast<ScRing*>(base + kOffSmallS);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t peer_small = mapa_shared(smem_u32(sm), rank ^ 1);
     const uint32_t peer_p = mapa_shared(smem_u32(base + kOffP), 1);  // P buffers live in the O-CTA
 
     if (threadIdx.x == 0) {
+        for (int i = 0; i < kStagesK * kGroups; ++i) {
+            mbar_init(&ring->kv_full[i], 1);
+            mbar_init(&ring->kv_empty[i], 1);
+        }
         for (int i = 0; i < kStages; ++i) {
-            mbar_init(&sm->kv_full[i], 1);
-            mbar_init(&sm->kv_empty[i], 1);
             mbar_init(&sm->v_full[i], 1);
             mbar_init(&sm->v_empty[i], 1);
         }
@@ -382,15 +493,18 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             mbar_init(&sm->item_full[i], 1);
             mbar_init(&sm->item_empty[i], 11);  // S-CTA: MMA warp + 4 softmax warps; O-CTA: producer + MMA + 4 epilogue warps
         }
+        mbar_init(&sm->qst_full[0], 1);
+        mbar_init(&sm->qst_full[1], 1);
         mbar_init(&sm->q_ready, 4);
         mbar_init(&sm->q_free, 1);
         mbar_init(&sm->fin_empty, 4);
-        mbar_init(&sm->fin_full, 128);
+        mbar_init(&sm->fin_full, 4);
         mbar_init(&sm->o_full, 1);
         mbar_init(&sm->o_empty, 4);
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) prefetch_tensormap(rank == 0 ? &pool_map_k : &pool_map_v);
+    if (warp == 2 && lane == 0 && rank == 0) prefetch_tensormap(&q_map);
     if (warp == 1) tmem_alloc(&sm->tmem_base, 512);
     tc_fence_before();
     __syncthreads();
@@ -424,6 +538,10 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             }
             if (idx < 0) break;
             const WorkItem w = load_item2(p.items + idx);
+            if (rank == 0 && lane == 0) {  // the tile's Q rows are contiguous: bring them into L2 one item ahead of their use
+                const uint32_t qbytes = uint32_t(w.n_q) * kHeads * kTokenBytes;
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.q_chunk + size_t(w.q_index) * kHeads * kDim), "r"(qbytes) : "memory");
+            }
             const int32_t* pt = p.chunk_pt + w.page_begin;
             const int npages = w.page_end - w.page_begin;
             for (int i = 0; i < npages; i += 32) {
@@ -435,9 +553,12 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
                         const uint32_t ns = rank == 0 ? kStagesK : kStages;
                         const uint32_t st = g % ns, sph = (g / ns) & 1;
                         if (rank == 0) {
-                            mbar_wait(&sm->kv_empty[st], sph ^ 1);
-                            mbar_arrive_expect_tx(&sm->kv_full[st], kKStage);
-                            tma_load_box3(base + st * kKStage, &pool_map_k, &sm->kv_full[st], pid * kPage, kEvictLast);
+                            for (int gr = 0; gr < kGroups; ++gr) {
+                                mbar_wait(&ring->kv_empty[st * kGroups + gr], sph ^ 1);
+                                mbar_arrive_expect_tx(&ring->kv_full[st * kGroups + gr], kGroupChunks * 8192);
+                                tma_load_chunk(base + st * kKStage + gr * kGroupChunks * 8192, &pool_map_k, &ring->kv_full[st * kGroups + gr],
+                                               pid * kPage, gr * kGroupChunks, kEvictLast);
+                            }
                         } else {
                             mbar_wait(&sm->v_empty[st], sph ^ 1);
                             mbar_arrive_expect_tx(&sm->v_full[st], kVStage);
@@ -451,30 +572,43 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
         // ================= consumers: MMA warp (1) and the four row-owning warps (2-5)
         const int q4 = warp & 3;  // TMEM lane quadrant this warp may touch
         const int row = q4 * 32 + lane;
-        uint32_t g = 0;
-        for (uint32_t it = 0;; ++it) {
-            const uint32_t slot = it & 1, iph = (it >> 1) & 1;
+        uint32_t g = 0, qcount = 0;
+        if (rank == 0 && warp >= 2) {
+            // S-CTA row-owning warps: item fetch and Q load run one item ahead of the softmax
             int idx;
-            if (rank == 0) {
-                mbar_wait(&sm->item_full[slot], iph);
-                idx = *reinterpret_cast<volatile int32_t*>(&sm->item_ring[slot]);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&sm->item_empty[slot]);
-            } else {
-                mbar_wait_cluster(&sm->item_full[slot], iph);
-                idx = *reinterpret_cast<volatile int32_t*>(&sm->item_ring[slot]);
-                __syncwarp();
-                if (lane == 0) mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, item_empty)) + slot * 8);
+            WorkItem w = sc_fetch_item(sm, p, lane, 0, &idx);
+            if (idx >= 0) sc_load_q(sm, w, p, &q_map, tmem, row, q4, lane, qcount, 0);
+            for (uint32_t it = 0; idx >= 0; ++it) {
+                WorkItem nxt{};
+                int nidx = -1;
+                sc_softmax_item(sm, base + kOffPStage, peer_small, peer_p, w, p, &q_map, tmem, row, q4, lane, g, qcount, it, &nxt, &nidx);
+                w = nxt;
+                idx = nidx;
             }
-            if (idx < 0) break;
-            const WorkItem w = load_item2(p.items + idx);
-            const int npages = w.page_end - w.page_begin;
-            if (warp == 1) {
-                if (rank == 0) sc_mma_item(sm, tmem, smem_u32(base), npages, g, it, p);
-                else oc_mma_item(sm, peer_small, tmem, smem_u32(base), smem_u32(base + kOffP), npages, g, it, p);
-            } else {
-                if (rank == 0) sc_softmax_item(sm, base + kOffPStage, peer_small, peer_p, w, p, tmem, row, q4, lane, g, it);
-                else oc_epilogue_item(sm, peer_small, w, p, tmem, row, q4, lane, g, it);
+        } else {
+            for (uint32_t it = 0;; ++it) {
+                const uint32_t slot = it & 1, iph = (it >> 1) & 1;
+                int idx;
+                if (rank == 0) {
+                    mbar_wait(&sm->item_full[slot], iph);
+                    idx = *reinterpret_cast<volatile int32_t*>(&sm->item_ring[slot]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&sm->item_empty[slot]);
+                } else {
+                    mbar_wait_cluster(&sm->item_full[slot], iph);
+                    idx = *reinterpret_cast<volatile int32_t*>(&sm->item_ring[slot]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_remote(peer_small + uint32_t(offsetof(PairSmall, item_empty)) + slot * 8);
+                }
+                if (idx < 0) break;
+                const WorkItem w = load_item2(p.items + idx);
+                const int npages = w.page_end - w.page_begin;
+                if (warp == 1) {
+                    if (rank == 0) sc_mma_item(sm, ring, tmem, smem_u32(base), npages, g, it, p);
+                    else oc_mma_item(sm, peer_small, tmem, smem_u32(base), smem_u32(base + kOffP), npages, g, it, p);
+                } else {
+                    oc_epilogue_item(sm, peer_small, w, p, tmem, row, q4, lane, g, it);
+                }
             }
         }
     }
@@ -499,6 +633,11 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
 
 int pair_tile_tokens() { return kPairTileTokens; }
 
+typedef CUresult (*EncodeTiledFn2)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn2 g_encode2 = nullptr;
+
 int pair_init(kairos_ctx* ctx) {
     typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -507,6 +646,7 @@ int pair_init(kairos_ctx* ctx) {
     cudaDriverEntryPointQueryResult q;
     KAIROS_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
     if (!fn || q != cudaDriverEntryPointSuccess) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    g_encode2 = reinterpret_cast<EncodeTiledFn2>(fn);
     // latent part of a page: pool viewed as [chunk 9][row num_pages*64][64 elems], box = 8 chunks x 64 rows x 64 elems
     cuuint64_t dims[3] = {64, cuuint64_t(ctx->cfg.num_pages) * kPage, 9};
     cuuint64_t strides[2] = {cuuint64_t(kTokenBytes), 128};
@@ -516,6 +656,11 @@ int pair_init(kairos_ctx* ctx) {
                                                      box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool, latent box) failed: " + std::to_string(int(r)));
+    cuuint32_t box1[3] = {64, 64, kGroupChunks};  // a group of 64-dim chunks of a page: the S-CTA's K ring is refilled group by group
+    r = reinterpret_cast<EncodeTiledFn>(fn)(&ctx->pool_map_c, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->cfg.pool, dims, strides, box1, es,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool, chunk box) failed: " + std::to_string(int(r)));
     KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_chunk_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
     KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking));
     KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
@@ -538,7 +683,18 @@ int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.lse_chunk = a.lse_chunk;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
     n_pairs = std::max(1, std::min(n_pairs, n_items));
-    kairos_chunk_pair_kernel<<<2 * n_pairs, kPairThreads, kPairSmem, stream>>>(ctx->pool_map, ctx->pool_map_v, p);
+    CUtensorMap q_map;  // q_chunk as [C*16 rows][576], box = 64 dims x 128 rows (one tile, one 64-dim chunk)
+    {
+        cuuint64_t dims[2] = {cuuint64_t(kDim), cuuint64_t(a.chunk_len) * kHeads};
+        cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
+        cuuint32_t box[2] = {64, 128};
+        cuuint32_t es[2] = {1, 1};
+        CUresult r = g_encode2(&q_map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(a.q_chunk), dims, strides, box, es,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q tile) failed: " + std::to_string(int(r)));
+    }
+    kairos_chunk_pair_kernel<<<2 * n_pairs, kPairThreads, kPairSmem, stream>>>(ctx->pool_map_c, ctx->pool_map_v, q_map, p);
     KAIROS_CUDA_TRY(cudaGetLastError());
     return KAIROS_OK;
 }

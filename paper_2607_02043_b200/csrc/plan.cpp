@@ -16,11 +16,16 @@ constexpr int kChunkCostDen = 4;       // (tensor-bound tile-page vs HBM-bound d
 
 inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b); }
 
-// Cost model of the static SM partition between the pair kernel (chunk) and the decode grid, in SM cycles (measured on
-// B200): one 8-token tile x 64-key page on a pair; one decode page on one CTA; the HBM floor per page.
-constexpr int64_t kPairPageCycles = 1650;
+// Cost model of the static SM partition between the pair kernel (chunk) and the decode grid, in nominal SM cycles
+// (1.965 GHz), calibrated on B200 (profiles/r01_bench_gen2.md): one 8-token tile x 64-key page on a pair (at the clocks the
+// chip sustains under tensor load), the fixed cost of a tile (Q load, pipeline fill, epilogue), one decode page on one CTA
+// (latency-bound, two pages in flight), the HBM floor per decode page with every SM streaming, and the same 8-token
+// tile-page done as two gen-1 tiles (what the pair path has to beat).
+constexpr int64_t kPairPageCycles = 2200;
+constexpr int64_t kPairItemCycles = 25000;
 constexpr int64_t kDecPageCycles = 3000;
-constexpr int64_t kDecPageHbmCycles = 22;
+constexpr int64_t kDecPageHbmSmCycles = 4260;
+constexpr int64_t kGen1PairPageSmCycles = 7570;
 
 void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t ctas,
                   int32_t pair_mode, int32_t T2, Plan* plan) {
@@ -37,18 +42,22 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
     if (pair_mode > 0) {
         n_p = std::min(pair_mode, max_pairs);
     } else {
-        if (pair_pages < 4 * int64_t(ctas / 2)) return;  // small chunk: gen-1 tiles ride in the decode queue
+        const int64_t work_c = pair_pages * kPairPageCycles + int64_t(n_tiles) * kPairItemCycles;
         if (n_dec == 0) {
             n_p = max_pairs;
+            if (work_c / n_p > pair_pages * kGen1PairPageSmCycles / ctas) return;  // few short tiles: gen-1 tiles use every SM
         } else {
             int64_t best = -1;
             n_p = 1;
             for (int32_t c = 1; c <= max_pairs; ++c) {
-                const int64_t tc = pair_pages * kPairPageCycles / c;
-                const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmCycles);
+                const int64_t tc = work_c / c;
+                const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmSmCycles / ctas);
                 const int64_t t = std::max(tc, td);
                 if (best < 0 || t < best) { best = t; n_p = c; }
             }
+            // one queue for everything (gen-1 tiles ride in the decode grid) unless the partition is clearly faster
+            const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
+            if (best * 10 > t_gen1 * 9) return;
         }
     }
     plan->n_pairs = n_p;

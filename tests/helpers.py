@@ -28,12 +28,15 @@ def oracle_pool_after_append(inp: W.MixedStepInputs) -> np.ndarray:
 class GpuRun:
     """Uploads the inputs, appends the chunk, runs kairos_mixed_step.  Keeps device tensors for reuse."""
 
-    def __init__(self, inp: W.MixedStepInputs, impl: str = "umma", workspace_bytes=None):
+    def __init__(self, inp: W.MixedStepInputs, impl: str = "umma", workspace_bytes=None, pairs=None):
         import torch
         from paper_2607_02043_b200 import kairos as K
         self.K, self.torch, self.inp = K, torch, inp
         old = os.environ.get("KAIROS_IMPL")
+        old_pairs = os.environ.get("KAIROS_PAIRS")
         os.environ["KAIROS_IMPL"] = impl
+        if pairs is not None:  # force the chunk onto `pairs` 2-CTA clusters (0 = never), read at kairos_create
+            os.environ["KAIROS_PAIRS"] = str(pairs)
         try:
             self.pool = K.bf16_tensor(inp.pool)
             ws = K.workspace_bytes(max(inp.n_dec, 1), max(inp.chunk_len, 1)) if workspace_bytes is None else workspace_bytes
@@ -44,6 +47,11 @@ class GpuRun:
                 os.environ.pop("KAIROS_IMPL", None)
             else:
                 os.environ["KAIROS_IMPL"] = old
+            if pairs is not None:
+                if old_pairs is None:
+                    os.environ.pop("KAIROS_PAIRS", None)
+                else:
+                    os.environ["KAIROS_PAIRS"] = old_pairs
         dev = "cuda"
         self.q_dec = K.bf16_tensor(inp.q_dec)
         self.q_chunk = K.bf16_tensor(inp.q_chunk)

@@ -18,9 +18,9 @@ pytestmark = pytest.mark.gpu
 IMPLS = ["umma", "simple"]
 
 
-def _full_compare(inp, impl, check_append=True):
+def _full_compare(inp, impl, check_append=True, pairs=None):
     from oracle import oracle
-    run = Hp.GpuRun(inp, impl)
+    run = Hp.GpuRun(inp, impl, pairs=pairs)
     run.append()
     pool_np = Hp.oracle_pool_after_append(inp)
     if check_append:
@@ -113,6 +113,29 @@ EDGE = [
 def test_edge_cases(name, kw, impl):
     inp = W.make_inputs(name, 100 + len(name), q_scale=0.5, extra_pages=3, **kw)
     _full_compare(inp, impl)
+
+
+# ------------------------------------------------------------------ the chunk on 2-CTA clusters (attn_pair.cu), forced
+# The planner only moves the chunk to the pair kernel for large chunks (configs[2], [3] at C >= 2048, [4]); here it is
+# forced so that every row of the small cases -- ragged tiles, prefixes that end inside a page, one tile on one pair,
+# more tiles than pairs, the thresholded rescale path with unscaled q -- is compared with the oracle.
+@pytest.mark.parametrize("pairs", [1, 3])
+@pytest.mark.parametrize("q_scale", [0.1, 1.0])
+def test_config0_on_pair_kernel(pairs, q_scale):
+    run, _, _ = _full_compare(W.make_config(0, q_scale=q_scale), "umma", pairs=pairs)
+    assert run.ctx.last_plan_info()["kernels"] == 2  # pair grid + decode grid, no combine at this size
+
+
+@pytest.mark.parametrize("name,kw", [e for e in EDGE if e[1]["chunk_len"] > 0], ids=[e[0] for e in EDGE if e[1]["chunk_len"] > 0])
+def test_edge_cases_on_pair_kernel(name, kw):
+    inp = W.make_inputs(name, 100 + len(name), q_scale=0.5, extra_pages=3, **kw)
+    _full_compare(inp, "umma", pairs=2)
+
+
+def test_pair_kernel_rescale_path_and_long_tiles():
+    """Scores with a steep positional trend force running-max updates page after page (the O-CTA's rescale path)."""
+    inp = W.make_inputs("pair_rescale", 77, [300], 40, 1500, q_scale=2.0)
+    _full_compare(inp, "umma", pairs=2)
 
 
 def test_empty_step_is_noop_and_errors_are_host_side():

@@ -15,11 +15,17 @@ SLOT_BYTES = 16 * 512 * 4 + 16 * 2 * 4
 KIND, QI, PB, PE, NKEYS, NQ, SLOT, COST = range(8)
 
 
-def _check_plan(lens, C, P, n_ctas=148):
+def _check_plan(lens, C, P, n_ctas=148, pair_mode=0):
     lens = np.asarray(lens, dtype=np.int32)
-    items, n_slots = K.plan_dump(lens, C, P, n_ctas)
+    items, n_slots, n_pairs = K.plan_dump(lens, C, P, n_ctas, pair_mode=pair_mode, with_pairs=True)
     dec = items[items[:, KIND] == 0]
-    chk = items[items[:, KIND] == 1]
+    chk = items[items[:, KIND] >= 1]
+    if n_pairs > 0:  # the chunk runs on the cluster kernel: whole 8-token tiles, no KV split, clusters fit beside the decode grid
+        assert (chk[:, KIND] == 2).all() and (chk[:, SLOT] == -1).all() and (chk[:, PB] == 0).all()
+        assert 1 <= n_pairs <= min(len(chk), n_ctas // 2) and (len(lens) == 0 or 2 * n_pairs < n_ctas)
+        assert (np.diff(chk[:, COST]) <= 0).all()
+    else:
+        assert (chk[:, KIND] == 1).all()
     # ---- decode coverage
     for i, L in enumerate(lens):
         pages = (int(L) + PAGE - 1) // PAGE
@@ -87,6 +93,23 @@ def test_plan_edge_shapes(lens, C, P):
     _check_plan(lens, C, P)
     _check_plan(lens, C, P, n_ctas=1)
     _check_plan(lens, C, P, n_ctas=7)
+
+
+@pytest.mark.parametrize("pair_mode", [-1, 1, 5, 74])
+@pytest.mark.parametrize("lens,C,P", [([], 8, 0), ([100], 13, 61), ([2048] * 256, 2048, 0), ([2048] * 256, 8192, 0),
+                                      ([32768] * 32, 4096, 28672), ([], 8192, 0), ([64] * 4, 64, 128), ([300] * 7, 129, 4000)])
+def test_plan_with_pair_kernel(lens, C, P, pair_mode):
+    _check_plan(lens, C, P, pair_mode=pair_mode)
+    _check_plan(lens, C, P, n_ctas=7, pair_mode=pair_mode)
+
+
+def test_planner_picks_the_pair_kernel_for_large_chunks_only():
+    n = lambda lens, C, P: K.plan_dump(lens, C, P, 148, pair_mode=-1, with_pairs=True)[2]
+    assert n([64, 128, 200, 256], 64, 128) == 0          # configs[0]
+    assert n([2048] * 256, 512, 0) == 0                  # small chunk rides in the decode queue as gen-1 tiles
+    assert n([2048] * 256, 8192, 0) > 40                 # tensor-bound: most SM pairs go to the chunk
+    assert n([32768] * 32, 4096, 28672) > 40             # configs[4]
+    assert n([], 8192, 0) == 74
 
 
 def test_plan_depends_only_on_lengths_and_is_deterministic():
