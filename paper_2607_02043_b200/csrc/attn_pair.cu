@@ -348,7 +348,6 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_
 // ------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_small, const WorkItem& w, const PairParams& p,
                                                  uint32_t tmem, int row, int q4, int lane, uint32_t& g, uint32_t it) {
-    const int tok = row >> 4, head = row & 15;
     const uint32_t lane_base = uint32_t(q4 * 32) << 16;
     const int npages = w.page_end - w.page_begin;
     for (int pg = 0; pg < npages; ++pg, ++g) {

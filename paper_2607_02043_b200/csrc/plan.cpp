@@ -21,8 +21,8 @@ inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b);
 // chip sustains under tensor load), the fixed cost of a tile (Q load, pipeline fill, epilogue), one decode page on one CTA
 // (latency-bound, two pages in flight), the HBM floor per decode page with every SM streaming, and the same 8-token
 // tile-page done as two gen-1 tiles (what the pair path has to beat).
-constexpr int64_t kPairPageCycles = 2200;
-constexpr int64_t kPairItemCycles = 25000;
+constexpr int64_t kPairPageCycles = 1750;
+constexpr int64_t kPairItemCycles = 32000;
 constexpr int64_t kDecPageCycles = 3000;
 constexpr int64_t kDecPageHbmSmCycles = 4260;
 constexpr int64_t kGen1PairPageSmCycles = 7570;
@@ -57,7 +57,7 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
             }
             // one queue for everything (gen-1 tiles ride in the decode grid) unless the partition is clearly faster
             const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
-            if (best * 10 > t_gen1 * 9) return;
+            if (best * 10 > t_gen1 * 8) return;
         }
     }
     plan->n_pairs = n_p;
