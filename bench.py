@@ -2,7 +2,7 @@
 """bench.py -- one JSON line per run for the mixed-step MLA attention path (BASELINE.json `metric`).
 
 A "step" = one pass of the whole hot path over one synthetic batch:
-kairos_append_latent(chunk) + kairos_mixed_step (host planner, persistent tcgen05 kernel, LSE combine).
+kairos_append_latent(chunk) + kairos_mixed_step (host planner, persistent tcgen05 kernels, LSE combine).
 Workload at N=1: BASELINE.json configs[1] ("decode-node steady state": 64 lognormal decodes + one 512-token chunk),
 seeded synthetic inputs standing in for the paper's proprietary traces.  N>1: one replica per GPU
 (requests shard by sequence with no data-path collective: "replicas only"), value aggregated over ranks.
@@ -275,20 +275,22 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (kairos_mixed_kernel): algorithmic bytes / flops per launch over its
-    # live CUDA-event duration inside the second timed region
+    # ---- roofline of the attention kernels of the step (kairos_mixed_kernel, plus the concurrent kairos_chunk_pair_kernel
+    # when the planner moves the chunk onto SM pairs): algorithmic bytes / flops per step over the live CUDA-event
+    # duration of that bracket inside the second timed region
     kern_avg_us = kern_us / max(kern_n, 1)
     t_hbm_us = alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
     t_tc_us = alg_flops / (peaks["bf16_tflops"] * 1e12) * 1e6
     bound = "hbm" if t_hbm_us >= t_tc_us else "tensor"
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = None  # DRAM bytes of one launch of the dominant kernel from the committed ncu capture of this configuration
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")
     if os.path.exists(tpath):
-        try:
-            with open(tpath) as f:
-                traffic = json.load(f).get(f"config{args.config}" + (f"_C{args.chunk}" if args.chunk is not None else ""))
-        except Exception:
-            traffic = None
+        key = f"config{args.config}" + (f"_C{args.chunk}" if args.chunk is not None else "")
+        with open(tpath) as f:
+            for line in f.read().splitlines()[1:]:
+                k, _, v = line.split(",")
+                if k == key:
+                    traffic = int(v)
     if bound == "hbm":
         achieved = alg_bytes / (kern_avg_us * 1e-6) / 1e9
         roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
@@ -297,7 +299,9 @@ def main():
         achieved = alg_flops / (kern_avg_us * 1e-6) / 1e12
         roof = {"bound": "tensor", "achieved": achieved, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": achieved / peaks["bf16_tflops"], "traffic": traffic}
-    roof.update({"kernel": "kairos_mixed_kernel", "kernel_us": kern_avg_us, "launches_timed": kern_n,
+    kname = ("kairos_chunk_pair_kernel (chunk, %d 2-CTA clusters) + kairos_mixed_kernel (decode splits), concurrent grids"
+             % info["chunk_pairs"]) if info.get("chunk_pairs", 0) > 0 else "kairos_mixed_kernel"
+    roof.update({"kernel": kname, "kernel_us": kern_avg_us, "launches_timed": kern_n,
                  "peak_source": peaks["source"], "algorithmic_bytes": alg_bytes, "algorithmic_flops": alg_flops,
                  "step_roofline_us": max(t_hbm_us, t_tc_us),
                  "step_frac_of_roofline": max(t_hbm_us, t_tc_us) / (ms_max * 1e3 / args.steps),
@@ -316,7 +320,7 @@ def main():
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": workload_label(args.config, inp), "parallelism": f"replicas x{world} (no collective)",
                    "l2": f"inputs rotate over {replicas} disjoint pool/query copies ({replicas * step_touch / 2**20:.0f} MiB > 2x L2)",
-                   "step": "kairos_append_latent(chunk) + kairos_mixed_step (planner H2D + persistent kernel + combine)",
+                   "step": "kairos_append_latent(chunk) + kairos_mixed_step (planner H2D + persistent attention kernel(s) + combine)",
                    "plan": info, "library": K.version()},
         "clocks": clocks,
         "e2e": {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

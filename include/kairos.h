@@ -185,7 +185,8 @@ int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_l
 
 /* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
  * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched
- * by that call, [5] = workspace bytes used.  n = number of int64 slots available in info. */
+ * by that call, [5] = workspace bytes used, [6] = 2-CTA clusters the chunk ran on (0 = the chunk ran as tiles of the
+ * decode grid's queue).  n = number of int64 slots available in info (at most 7 are written). */
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
 
 /*

@@ -177,6 +177,7 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     ctx->last_info[3] = std::min<int64_t>(umma_resident_ctas(ctx), int64_t(plan.items.size()));
     ctx->last_info[4] = kernels;
     ctx->last_info[5] = int64_t(ws_needed);
+    ctx->last_info[6] = plan.n_pairs;
     return KAIROS_OK;
 }
 
@@ -398,7 +399,7 @@ int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_l
 
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n) {
     if (!ctx || !info || n < 0) return fail(KAIROS_ERR_INVALID_ARG, "NULL argument");
-    for (int32_t i = 0; i < n && i < 6; ++i) info[i] = ctx->last_info[i];
+    for (int32_t i = 0; i < n && i < 7; ++i) info[i] = ctx->last_info[i];
     return KAIROS_OK;
 }
 

@@ -103,7 +103,7 @@ struct kairos_ctx {
     int staging_next = 0;
     kairos::HostStage host_stage;
     kairos::Plan plan;            // reused per call
-    int64_t last_info[6] = {0, 0, 0, 0, 0, 0};
+    int64_t last_info[7] = {0, 0, 0, 0, 0, 0, 0};
     bool profile = false;         // bracket the main kernel with events (kairos_profile_enable)
     std::vector<cudaEvent_t> prof_events;  // pairs: [2i] start, [2i+1] stop
     size_t prof_used = 0;         // events in use since the last kairos_profile_read

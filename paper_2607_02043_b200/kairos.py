@@ -212,9 +212,9 @@ class Kairos:
         return float(us.value), int(n.value)
 
     def last_plan_info(self) -> dict:
-        info = (_c.c_int64 * 6)()
-        _check(_lib.kairos_last_plan_info(self._h, info, 6))
-        keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes"]
+        info = (_c.c_int64 * 7)()
+        _check(_lib.kairos_last_plan_info(self._h, info, 7))
+        keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes", "chunk_pairs"]
         return dict(zip(keys, (int(x) for x in info)))
 
 
