@@ -4,13 +4,14 @@
 // tensor peak (profiles/r01_mma_issue_probe.txt).
 //
 //   rank 0, "S-CTA":  S[128 q rows x 64 keys] = Q[128 x 576] . K_page^T     tcgen05.mma M=128 N=64, A = Q held in TMEM
-//                     (bf16, 288 columns, loaded once per tile), B = the K page in SMEM (K-major, TMA, 3 stages);
-//                     4 softmax warps own one query row per thread (row max / sum are thread-local), write
-//                     P = exp2(S*c - m) as bf16 straight into the O-CTA's shared memory (DSMEM) and arrive on its
-//                     mbarrier.
+//                     (bf16, 288 columns, loaded once per tile through TMA staging), B = the K page in SMEM (K-major,
+//                     TMA, 2 stages refilled in 3 groups); 4 softmax warps own one query row per thread (row max / sum
+//                     are thread-local); P = exp2(S*c - m) as bf16 and the per-row rescale factors are staged in local
+//                     shared memory and moved to the O-CTA by cp.async.bulk (shared::cta -> shared::cluster), which
+//                     completes on the O-CTA's mbarrier.
 //   rank 1, "O-CTA":  O[128 x 512] += P[128 x 64] . V_page[64 x 512]        tcgen05.mma M=128 N=256 x2, A = P (SMEM,
 //                     K-major), B = the latent page as stored (MN-major, TMA, 3 stages), fp32 accumulators = all
-//                     512 TMEM columns; its 4 epilogue warps rescale O on the (rare, thresholded) running-max updates
+//                     512 TMEM columns; its 4 row-owning warps rescale O on the (rare, thresholded) running-max updates
 //                     and write O / l as bf16.
 //
 // Rows of a tile: r = 16 * (token in tile) + head.  Work items come from a queue shared by all pairs (rank 0 pops and
