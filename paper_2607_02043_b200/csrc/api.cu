@@ -229,6 +229,7 @@ int kairos_create(const kairos_config* cfg, kairos_ctx** out) {
             return rc;
         }
         if (const char* fp = std::getenv("KAIROS_PAIRS")) ctx->force_pairs = std::atoi(fp);  // debug / sweeps: 0 = gen-1 chunk tiles only
+        if (const char* fd = std::getenv("KAIROS_DEC_ONLY")) ctx->force_dec_only = std::atoi(fd);
     }
     *out = ctx;
     return KAIROS_OK;

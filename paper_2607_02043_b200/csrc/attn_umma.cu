@@ -31,18 +31,50 @@ constexpr int kSoftmaxWarps = 8;                 // 2 per TMEM lane quadrant: ea
 constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
 constexpr int kThreads = 64 + kSoftmaxThreads;    // warp 0 producer, warp 1 MMA issuer, warps 2-9 softmax
 constexpr int kChunkTileTokens = 4;
-constexpr int kStageBytes = kPage * kTokenBytes;  // 73,728: one page
-constexpr int kQBytes = 64 * kTokenBytes;         // 73,728: up to 64 query rows
+// one page = 73,728 B = 9 slots of 8 KB ([64 tokens][128 B], SWIZZLE_128B)
+constexpr int kSlotBytes = 8192;
+// Shared memory: the Q tile, then a ring of 8 KB slots that pages stream through (9 consecutive slots per page, refilled
+// as pages retire, so that more than two pages' worth of loads can be in flight), then the barriers / statistics.
+// DEC = true is the decode-only instantiation: two 16-row Q buffers (36 KB) leave room for 22 slots (2.44 pages in flight);
+// the mixed instantiation holds a 64-row Q tile (72 KB) and 18 slots.  Decode items alternate between two 18 KB Q
+// buffers at the start of the Q region (item parity), so that the next item's Q is loaded while the current item still
+// streams its pages; a chunk tile takes the whole region (both buffers).
+template <bool DEC>
+struct Geo {
+    static constexpr int kQBytes = (DEC ? 2 * 16 : 64) * kTokenBytes;  // two decode Q buffers, or one 64-row chunk tile
+    static constexpr int kSlots = DEC ? 22 : 18;  // even: a pair of latent slots (one M=128 V^T operand) never straddles the wrap
+    static constexpr int kOffKV = kQBytes;
+    static constexpr int kOffSmall = kOffKV + kSlots * kSlotBytes;
+    static constexpr int kSmemBytes = kOffSmall + 3072 + 1024;  // Small + alignment slack
+    static_assert(kQBytes % 1024 == 0 && kSlots % 2 == 0, "ring must stay 1024-B aligned and even");
+    static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
+};
 constexpr int kOffQ = 0;
-constexpr int kOffKV = kQBytes;
-// P^T [64 keys][<=64 rows] bf16 (8 KB) lives in the RoPE chunk (chunk 8) of its own KV stage: that chunk is only
-// read by the S MMAs, which have completed before the softmax of the page starts, and the stage is not reloaded
-// until the PV MMAs that read P^T have completed.  One P^T per stage = free double buffering, no extra SMEM.
-constexpr int kOffPInStage = 8 * 8192;
-constexpr int kOffSmall = kOffKV + 2 * kStageBytes;  // 221,184
-constexpr int kSmallBytes = 2048;
-constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;  // + alignment slack
-static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
+constexpr int kDecQBytes = 16 * kTokenBytes;  // 18,432: one decode Q buffer
+constexpr int kSmallBytes = 3072;
+constexpr int kPageRing = 4;  // full / empty barriers per page in flight (at most 4 pages have slots in the ring at once)
+
+// Where page number g (counted per CTA since launch) sits in a ring of R slots: it takes slots s .. s+8 (mod R), s = 9g mod R.
+// The 8 latent slots start at the even one of {s, s+1} so that slot pairs (one 128-dim V^T block) are contiguous; the RoPE
+// slot is the remaining one (before the latent slots when s is odd, after them when s is even).  P^T [64 keys][<=64 rows]
+// bf16 (8 KB) is written into the page's RoPE slot: that slot is only read by the S MMAs, which have completed before the
+// softmax of the page starts, and the page's slots are not reloaded until the PV MMAs that read P^T have completed.
+struct PageSlots {
+    uint32_t pair[4];  // first slot of latent chunks (2b, 2b+1)
+    uint32_t rope;
+    uint32_t odd;      // s is odd: the RoPE slot comes first in ring order
+};
+template <int R>
+__device__ __forceinline__ PageSlots page_slots(uint32_t g) {
+    PageSlots ps;
+    const uint32_t s = (g * 9u) % uint32_t(R);
+    ps.odd = s & 1u;
+    const uint32_t e = s + ps.odd;
+    ps.rope = ps.odd ? s : (s + 8u) % uint32_t(R);
+#pragma unroll
+    for (uint32_t b = 0; b < 4; ++b) ps.pair[b] = (e + 2u * b) % uint32_t(R);
+    return ps;
+}
 
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64
@@ -52,7 +84,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
 
 struct Small {
-    uint64_t q_full, q_empty, kv_full[2], kv_empty[2], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kPageRing], kv_empty[kPageRing], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -66,7 +98,11 @@ static_assert(sizeof(Small) <= kSmallBytes, "Small does not fit");
 
 #ifdef KAIROS_TRACE
 #define KTRACE(ev, g) do { if (blockIdx.x == 0 && (g) < 64) p.trace[(ev) * 64 + (g)] = clock64(); } while (0)
+// per-CTA statistics (globaltimer ns) 16 KB below the CTA-0 timeline: [cta][0 start, 1 end, 2 pages, 3 items]
+#define KSTAT(k, v) do { (p.trace - 2048)[blockIdx.x * 4 + (k)] = (v); } while (0)
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 #else
+#define KSTAT(k, v) do { } while (0)
 #define KTRACE(ev, g) do { } while (0)
 #endif
 
@@ -95,12 +131,13 @@ __device__ __forceinline__ WorkItem load_item(const WorkItem* p) {
     return w;
 }
 
-__device__ __forceinline__ void tma_load_page(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t row, uint64_t policy) {
-    // 3-D box (64 elems, 64 rows, 9 chunks) of the pool viewed as [chunk][row][64]: lands as [9][64][128 B]
+__device__ __forceinline__ void tma_load_chunks(uint32_t smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t row, int32_t chunk,
+                                                uint64_t policy) {
+    // 3-D box (64 elems, 64 rows, 1 or 2 chunks) of the pool viewed as [chunk][row][64]: lands as [chunks][64][128 B]
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
         " [%0], [%1, {%3, %4, %5}], [%2], %6;"
-        ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(0), "r"(row), "r"(0),
+        ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(0), "r"(row), "r"(chunk),
           "l"(policy)
         : "memory");
 }
@@ -143,7 +180,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 // 8 warps: warp sw works on TMEM lane quadrant sw & 3 (16 of its lanes hold the M=64 accumulator rows = keys) and on
 // the column half sw >> 2 (N/2 query rows).
 // ------------------------------------------------------------------------------------------------------------
-template <int N>
+template <int N, int R>
 __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkItem& w, const KParams& p, uint32_t tmem,
                                              int sw, int lane, uint32_t& g, uint32_t it) {
     constexpr int NC = N / 2;            // columns of this warp
@@ -236,7 +273,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
             x[c] = pv;
         }
         if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
-            uint8_t* ps = kv + b * kStageBytes + kOffPInStage;
+            uint8_t* ps = kv + page_slots<R>(g).rope * kSlotBytes;
 #pragma unroll
             for (int j = 0; j < NC / 8; ++j) {
                 uint4 v;
@@ -319,14 +356,15 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
 // MMA issue for one work item (whole warp, converged).  S(s) may run one page ahead of PV; PV has priority as soon
 // as its P^T is ready, because its completion releases the KV stage to the TMA producer.
 // ------------------------------------------------------------------------------------------------------------
-template <int N>
+template <int N, int R>
 __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base,
-                                         int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p) {
+                                         int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p,
+                                         uint32_t qbuf, uint32_t qfull_parity) {
     constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
     constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
     const uint32_t qb_lo = smem_desc_lo(q_base, 16);
-    mbar_wait(&sm->q_full, it & 1);
+    mbar_wait(&sm->q_full[qbuf], qfull_parity);
     int s_next = 0, pv_next = 0;
     uint32_t spins = 0;
     while (pv_next < npages) {
@@ -339,16 +377,19 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                 if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
                 KTRACE(3, gg);
                 tc_fence_after();
-                const uint32_t st = pst, a0 = kv_base + st * kStageBytes;
-                const uint32_t va_lo = smem_desc_lo(a0, 8192), pb_lo = smem_desc_lo(a0 + kOffPInStage, 8192);
+                const PageSlots ps = page_slots<R>(gg);
+                const uint32_t st = gg & (kPageRing - 1);
+                const uint32_t pb_lo = smem_desc_lo(kv_base + ps.rope * kSlotBytes, 8192);
 #pragma unroll
-                for (uint32_t b4 = 0; b4 < 4; ++b4)
+                for (uint32_t b4 = 0; b4 < 4; ++b4) {
+                    const uint32_t va_lo = smem_desc_lo(kv_base + ps.pair[b4] * kSlotBytes, 8192);
 #pragma unroll
                     for (uint32_t ks = 0; ks < 4; ++ks)
-                        umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + (((2 * b4) * 8192 + ks * 2048) >> 4), desc_hi,
+                        umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + ((ks * 2048) >> 4), desc_hi,
                                           pb_lo + ((ks * 2048) >> 4), desc_hi, idesc_o, (pv_next > 0 || ks > 0));
+                }
                 umma_commit_elect(&sm->kv_empty[st]);
-                umma_commit_elect(&sm->pv_done[st]);
+                umma_commit_elect(&sm->pv_done[pst]);
                 if (pv_next == npages - 1) umma_commit_elect(&sm->o_full);
                 KTRACE(4, gg);
                 ++pv_next;
@@ -359,20 +400,26 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
         if (s_next < npages && s_next <= pv_next + 1) {
             const uint32_t gg = g0 + s_next;
             const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
-            if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[st], ph))) {
+            if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[gg & (kPageRing - 1)], (gg / kPageRing) & 1))) {
                 KTRACE(1, gg);
-                mbar_wait(&sm->s_empty[st], ph ^ 1);
+                mbar_wait(&sm->s_empty[st], ph ^ 1);  // the softmax warps have read this S^T buffer (tcgen05.ld)
                 tc_fence_after();
-                const uint32_t ka_lo = smem_desc_lo(kv_base + st * kStageBytes, 16);
+                const PageSlots ps = page_slots<R>(gg);
 #pragma unroll
-                for (uint32_t c = 0; c < 9; ++c)
+                for (uint32_t c = 0; c < 9; ++c) {
+                    const uint32_t slot = c < 8 ? ps.pair[c >> 1] + (c & 1) : ps.rope;
+                    const uint32_t ka_lo = smem_desc_lo(kv_base + slot * kSlotBytes, 16);
 #pragma unroll
                     for (uint32_t j = 0; j < 4; ++j)
-                        umma_bf16_ss_lohi(tmem + kColS + st * 64, ka_lo + ((c * 8192 + j * 32) >> 4), desc_hi,
+                        umma_bf16_ss_lohi(tmem + kColS + st * 64, ka_lo + ((j * 32) >> 4), desc_hi,
                                           qb_lo + ((c * N * 128 + j * 32) >> 4), desc_hi, idesc_s, (c | j) != 0);
+                }
                 umma_commit_elect(&sm->s_full[st]);
                 ++s_next;
-                if (s_next == npages) umma_commit_elect(&sm->q_empty);  // Q tile free once every S-MMA retires
+                if (s_next == npages) {  // Q buffer(s) free once every S-MMA retires
+                    umma_commit_elect(&sm->q_empty[qbuf]);
+                    if (N == 64) umma_commit_elect(&sm->q_empty[1]);
+                }
                 KTRACE(2, gg);
                 spins = 0;
                 continue;
@@ -383,21 +430,32 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
 }
 
 // ------------------------------------------------------------------------------------------------------------
+template <bool DEC>
 __global__ void __launch_bounds__(kThreads, 1)
-kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_constant__ CUtensorMap qd_map,
-                    const __grid_constant__ CUtensorMap qc_map, const KParams p) {
+kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_constant__ CUtensorMap pool_map1,
+                    const __grid_constant__ CUtensorMap qd_map, const __grid_constant__ CUtensorMap qc_map, const KParams p) {
+    using G = Geo<DEC>;
+    constexpr int R = G::kSlots;
+    constexpr int kOffKV = G::kOffKV;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    Small* sm = reinterpret_cast<Small*>(base + kOffSmall);
+    Small* sm = reinterpret_cast<Small*>(base + G::kOffSmall);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) KTRACE(10, 0);
+#ifdef KAIROS_TRACE
+    if (threadIdx.x == 0) KSTAT(0, gtime());
+#endif
 
     if (threadIdx.x == 0) {
-        mbar_init(&sm->q_full, 1);
-        mbar_init(&sm->q_empty, 1);
         for (int i = 0; i < 2; ++i) {
+            mbar_init(&sm->q_full[i], 1);
+            mbar_init(&sm->q_empty[i], 1);
+        }
+        for (int i = 0; i < kPageRing; ++i) {
             mbar_init(&sm->kv_full[i], 1);
             mbar_init(&sm->kv_empty[i], 1);
+        }
+        for (int i = 0; i < 2; ++i) {
             mbar_init(&sm->s_full[i], 1);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
@@ -410,7 +468,8 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) {
-        prefetch_tensormap(&pool_map);
+        prefetch_tensormap(&pool_map2);
+        prefetch_tensormap(&pool_map1);
         prefetch_tensormap(&qd_map);
         prefetch_tensormap(&qc_map);
     }
@@ -424,11 +483,17 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
 
     if (warp == 0) {
         // ================= producer: pop work items, TMA-load Q tiles and KV pages =================
-        uint32_t g = 0;
+        uint32_t g = 0;        // pages issued so far
+        uint32_t g_acked = 0;  // pages whose slots have been taken back (kv_empty observed)
+        int free_slots = R;
+        uint32_t q_use0 = 0, q_use1 = 0;  // how many items have used each Q buffer (a chunk tile uses both)
+        const uint32_t kv_u32 = smem_u32(base + kOffKV);
         for (uint32_t it = 0;; ++it) {
-            int idx = 0;
-            if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
+            int idx = int(blockIdx.x);  // the first item is static (grid <= n_items): no queue round trip before the first load
+            if (it > 0) {
+                if (lane == 0) idx = atomicAdd(&p.counters[0], 1) + int(gridDim.x);
+                idx = __shfl_sync(0xffffffffu, idx, 0);
+            }
             if (idx >= p.n_items) idx = -1;
             if (lane == 0 && it == 0) KTRACE(10, 2);
             if (lane == 0) {
@@ -436,17 +501,25 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
                 sm->item_ring[it & 1] = idx;
                 mbar_arrive(&sm->item_full[it & 1]);
             }
+#ifdef KAIROS_TRACE
+            if (idx < 0 && lane == 0) { KSTAT(2, (unsigned long long)g); KSTAT(3, (unsigned long long)it); }
+#endif
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
-            const int N = w.kind ? 64 : 16;
+            const int N = (!DEC && w.kind) ? 64 : 16;
             if (lane == 0 && it == 0) KTRACE(10, 3);
+            const bool is_chunk = !DEC && w.kind;
+            const int qb = is_chunk ? 0 : int(it & 1);
             if (lane == 0) {
-                mbar_wait(&sm->q_empty, (it & 1) ^ 1);
-                mbar_arrive_expect_tx(&sm->q_full, uint32_t(9 * N * 128));
-                const CUtensorMap* qm = w.kind ? &qc_map : &qd_map;
+                mbar_wait(&sm->q_empty[qb], ((qb ? q_use1 : q_use0) & 1) ^ 1);
+                if (is_chunk) mbar_wait(&sm->q_empty[1], (q_use1 & 1) ^ 1);
+                mbar_arrive_expect_tx(&sm->q_full[qb], uint32_t(9 * N * 128));
+                const CUtensorMap* qm = is_chunk ? &qc_map : &qd_map;
                 for (int c = 0; c < 9; ++c)
-                    tma_load_2d(base + kOffQ + c * N * 128, qm, &sm->q_full, c * 64, w.q_index * kHeads, kEvictFirst);
+                    tma_load_2d(base + kOffQ + qb * kDecQBytes + c * N * 128, qm, &sm->q_full[qb], c * 64, w.q_index * kHeads, kEvictFirst);
             }
+            if (qb == 0) ++q_use0;
+            if (qb == 1 || is_chunk) ++q_use1;
             const int32_t* pt = (w.kind ? p.chunk_pt : p.dec_pt + size_t(w.q_index) * p.dec_stride) + w.page_begin;
             const uint64_t policy = w.kind ? kEvictLast : kEvictFirst;  // chunk KV is re-read by every tile
             const int npages = w.page_end - w.page_begin;
@@ -457,11 +530,31 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
-                        const int st = g & 1;
-                        mbar_wait(&sm->kv_empty[st], ((g >> 1) & 1) ^ 1);
+                        const PageSlots ps = page_slots<R>(g);
+                        uint64_t* full = &sm->kv_full[g & (kPageRing - 1)];
+                        const int row = pid * kPage;
+                        // take slots in ring order; pages retire in order, 9 slots each
+                        auto reserve = [&](int n) {
+                            while (free_slots < n) {
+                                mbar_wait(&sm->kv_empty[g_acked & (kPageRing - 1)], (g_acked / kPageRing) & 1);
+                                ++g_acked;
+                                free_slots += 9;
+                            }
+                            free_slots -= n;
+                        };
+                        reserve(ps.odd ? 1 : 2);
                         KTRACE(0, g);
-                        mbar_arrive_expect_tx(&sm->kv_full[st], kStageBytes);
-                        tma_load_page(base + kOffKV + st * kStageBytes, &pool_map, &sm->kv_full[st], pid * kPage, policy);
+                        mbar_arrive_expect_tx(full, 9 * kSlotBytes);
+                        if (ps.odd) tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, full, row, 8, policy);
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) {
+                            if (b > 0 || ps.odd) reserve(2);
+                            tma_load_chunks(kv_u32 + ps.pair[b] * kSlotBytes, &pool_map2, full, row, 2 * b, policy);
+                        }
+                        if (!ps.odd) {
+                            reserve(1);
+                            tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, full, row, 8, policy);
+                        }
                     }
                 }
             }
@@ -470,6 +563,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
         // ================= MMA issuer: the whole warp runs converged, one elected lane issues =================
         const uint32_t leader = elect_one();
         const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV);
+        uint32_t q_full0 = 0, q_full1 = 0;
         uint32_t g = 0;
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
@@ -481,8 +575,12 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             const WorkItem w = load_item(p.items + idx);
             const int kind = __shfl_sync(0xffffffffu, w.kind, 0);
             const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
-            if (kind) mma_item<64>(sm, tmem, q_base, kv_base, npages, g, it, leader, p);
-            else mma_item<16>(sm, tmem, q_base, kv_base, npages, g, it, leader, p);
+            // Q buffer bookkeeping mirrors the producer's: q_full[b] completes once per item that loads into buffer b
+            const uint32_t qb = (!DEC && kind) ? 0u : (it & 1u);
+            const uint32_t qpar = (qb ? q_full1 : q_full0) & 1u;
+            if (qb) ++q_full1; else ++q_full0;
+            if (!DEC && kind) mma_item<64, R>(sm, tmem, q_base, kv_base, npages, g, it, leader, p, 0, qpar);
+            else mma_item<16, R>(sm, tmem, q_base + qb * kDecQBytes, kv_base, npages, g, it, leader, p, qb, qpar);
             g += npages;
         }
     } else {
@@ -497,8 +595,8 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
-            if (w.kind) softmax_item<64>(sm, kv, w, p, tmem, sw, lane, g, it);
-            else softmax_item<16>(sm, kv, w, p, tmem, sw, lane, g, it);
+            if (!DEC && w.kind) softmax_item<64, R>(sm, kv, w, p, tmem, sw, lane, g, it);
+            else softmax_item<16, R>(sm, kv, w, p, tmem, sw, lane, g, it);
         }
     }
 
@@ -506,6 +604,9 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map, const __grid_c
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x == 0) KTRACE(10, 7);
+#ifdef KAIROS_TRACE
+    if (threadIdx.x == 0) KSTAT(1, gtime());
+#endif
     if (warp == 1) tmem_dealloc(tmem, kTmemCols);
     if (threadIdx.x == 0) {
         __threadfence();
@@ -651,7 +752,16 @@ int umma_init(kairos_ctx* ctx) {
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed: " + std::to_string(int(r)));
     ctx->has_pool_map = true;
-    KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    // the ring is filled by boxes of 2 latent chunks (16 KB) and 1 RoPE chunk (8 KB)
+    for (int n = 1; n <= 2; ++n) {
+        cuuint32_t boxn[3] = {64, 64, cuuint32_t(n)};
+        r = g_encode(n == 2 ? &ctx->pool_map2 : &ctx->pool_map1, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ctx->cfg.pool, dims, strides, boxn,
+                     es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool chunks) failed: " + std::to_string(int(r)));
+    }
+    KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<false>::kSmemBytes));
+    KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<true>::kSmemBytes));
     KAIROS_CUDA_TRY(cudaMemset(ctx->cfg.workspace, 0, 256));  // work-queue counters
     return KAIROS_OK;
 }
@@ -679,7 +789,13 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
     const int grid = std::max(1, std::min(n_items, std::min(max_ctas, umma_resident_ctas(ctx))));
-    kairos_mixed_kernel<<<grid, kThreads, kSmemBytes, stream>>>(ctx->pool_map, qd_map, qc_map, p);
+    // decode-only queues (no chunk, or the chunk is on the pair grid) take the instantiation with the deeper page ring
+    bool dec_only = a.chunk_len == 0 || ctx->plan.n_chunk_items == 0;
+    if (ctx->force_dec_only >= 0) dec_only = dec_only && ctx->force_dec_only != 0;
+    if (dec_only)
+        kairos_mixed_kernel<true><<<grid, kThreads, Geo<true>::kSmemBytes, stream>>>(ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p);
+    else
+        kairos_mixed_kernel<false><<<grid, kThreads, Geo<false>::kSmemBytes, stream>>>(ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p);
     KAIROS_CUDA_TRY(cudaGetLastError());
     *kernels_launched = 1;
     (void)dev_combines;

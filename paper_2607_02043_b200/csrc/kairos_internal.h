@@ -93,6 +93,8 @@ struct kairos_ctx {
     int impl = 1;                 // 0 = simple CUDA-core kernel (debug cross-check), 1 = tcgen05 path
     CUtensorMap pool_map;         // TMA descriptor of the pool (filled when impl needs it)
     bool has_pool_map = false;
+    CUtensorMap pool_map2, pool_map1;  // boxes of 2 latent chunks / 1 chunk of a page: the slot ring of kairos_mixed_kernel
+    int force_dec_only = -1;      // KAIROS_DEC_ONLY env (sweeps): 0 = never use the decode-only instantiation
     CUtensorMap pool_map_c;       // one 64-dim chunk of a page (8 KB box): K ring of the pair kernel's S-CTA
     CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
     cudaStream_t aux_stream = nullptr;  // the pair kernel runs beside the decode kernel on this stream (event fork / join)
