@@ -118,8 +118,18 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     std::memcpy(st->host, plan.items.data(), items_bytes);
     if (comb_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + comb_off, plan.combines.data(), comb_bytes);
     if (pair_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + pair_off, plan.pair_items.data(), pair_bytes);
-    KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, stream));
-    KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
+    // The work list goes to the device on the library's copy stream, so that it overlaps whatever the caller's stream is
+    // still running (the append of this step, the previous step's tail); the caller's stream then waits for it.  The
+    // slot's device buffer is not overwritten before the kernels of its previous use have read it (`consumed`).
+    if (ctx->copy_stream) {
+        if (st->consumed) KAIROS_CUDA_TRY(cudaStreamWaitEvent(ctx->copy_stream, st->consumed, 0));
+        KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        KAIROS_CUDA_TRY(cudaEventRecord(st->done, ctx->copy_stream));
+        KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, st->done, 0));
+    } else {
+        KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, stream));
+        KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
+    }
     auto T3 = now();
     int kernels = 0;
     // Roofline leg of bench.py: one pair of events around the attention kernels of the step (the decode grid and, when
@@ -141,20 +151,32 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     const WorkItem* dev_pair = reinterpret_cast<const WorkItem*>(static_cast<uint8_t*>(st->dev) + pair_off);
     const int n_pairs = plan.n_pairs;
     const bool have_queue = !plan.items.empty();
-    if (n_pairs > 0 && have_queue) {  // pair grid first (it needs whole SM pairs), decode grid beside it
-        KAIROS_CUDA_TRY(cudaEventRecord(ctx->ev_fork, stream));
-        KAIROS_CUDA_TRY(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_fork, 0));
-        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, ctx->aux_stream)) return rc;
-        KAIROS_CUDA_TRY(cudaEventRecord(ctx->ev_join, ctx->aux_stream));
+    const WorkItem* dev_items = reinterpret_cast<const WorkItem*>(st->dev);
+    const CombineItem* dev_comb = reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off);
+    if (n_pairs > 0 && have_queue) {
+        // The two grids share the SMs in time (plan.cpp::choose_pairs).  dec_ctas > 0: the decode grid goes first, as 2-CTA
+        // clusters on dec_ctas SMs (whole TPCs), then one chunk cluster per SM pair -- those that do not fit yet start when
+        // the decode CTAs exit.  dec_ctas == 0: the clusters take every SM pair and the decode CTAs follow as SMs free up.
+        // Both kernels go to the caller's stream; the second one is launched with programmatic stream serialisation and
+        // starts once every CTA of the first is resident (both trigger launch_dependents on entry), so the order in
+        // which the grids take SMs is the launch order.
+        if (plan.dec_ctas > 0) {
+            if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
+                                          &kernels, plan.dec_ctas, /*as_clusters=*/true, /*pdl=*/false))
+                return rc;
+            if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/true)) return rc;
+        } else {
+            if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/false)) return rc;
+            if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
+                                          &kernels, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/true))
+                return rc;
+        }
     } else if (n_pairs > 0) {
-        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream)) return rc;
-    }
-    if (have_queue) {
-        if (int rc = launch_attn_umma(ctx, a, reinterpret_cast<const WorkItem*>(st->dev), int32_t(plan.items.size()),
-                                      reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
-                                      int32_t(plan.combines.size()), stream, &kernels, umma_resident_ctas(ctx) - 2 * n_pairs))
+        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/false)) return rc;
+    } else if (have_queue) {
+        if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
+                                      &kernels, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/false))
             return rc;
-        if (n_pairs > 0) KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, ctx->ev_join, 0));
     }
     if (n_pairs > 0) ++kernels;
     if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
@@ -163,6 +185,10 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
                                     int32_t(plan.combines.size()), stream))
             return rc;
         ++kernels;
+    }
+    if (ctx->copy_stream) {
+        if (!st->consumed) KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&st->consumed, cudaEventDisableTiming));
+        KAIROS_CUDA_TRY(cudaEventRecord(st->consumed, stream));
     }
     if (dbg) {
         auto T4 = now();
@@ -174,7 +200,7 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     ctx->last_info[0] = int64_t(plan.items.size());
     ctx->last_info[1] = plan.n_decode_items;
     ctx->last_info[2] = plan.n_chunk_items + int64_t(plan.pair_items.size());
-    ctx->last_info[3] = std::min<int64_t>(umma_resident_ctas(ctx), int64_t(plan.items.size()));
+    ctx->last_info[3] = std::min<int64_t>(plan.n_pairs > 0 && plan.dec_ctas > 0 ? plan.dec_ctas : umma_resident_ctas(ctx), int64_t(plan.items.size()));
     ctx->last_info[4] = kernels;
     ctx->last_info[5] = int64_t(ws_needed);
     ctx->last_info[6] = plan.n_pairs;
@@ -228,6 +254,7 @@ int kairos_create(const kairos_config* cfg, kairos_ctx** out) {
             delete ctx;
             return rc;
         }
+        if (!std::getenv("KAIROS_NO_COPY_STREAM")) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         if (const char* fp = std::getenv("KAIROS_PAIRS")) ctx->force_pairs = std::atoi(fp);  // debug / sweeps: 0 = gen-1 chunk tiles only
         if (const char* fd = std::getenv("KAIROS_DEC_ONLY")) ctx->force_dec_only = std::atoi(fd);
     }
@@ -243,10 +270,12 @@ int kairos_destroy(kairos_ctx* ctx) {
         if (s.host) cudaFreeHost(s.host);
         if (s.dev) cudaFree(s.dev);
         if (s.done) cudaEventDestroy(s.done);
+        if (s.consumed) cudaEventDestroy(s.consumed);
     }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
     for (auto e : ctx->prof_events) cudaEventDestroy(e);
     if (ctx->aux_stream) cudaStreamDestroy(ctx->aux_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete ctx;

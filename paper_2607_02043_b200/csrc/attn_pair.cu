@@ -199,8 +199,7 @@ __device__ __forceinline__ WorkItem sc_fetch_item(PairSmall* sm, const PairParam
     return w;
 }
 
-// Processes item `it` (its Q is already in TMEM).  Before the softmax of the LAST page -- all S-MMAs of the item have
-// retired by then -- it fetches item it + 1 and loads that item's Q, so the MMA warp restarts while this item drains.
+// Processes item `it` (its Q is already in TMEM), then fetches item it + 1 and loads that item's Q.
 __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, uint32_t peer_small, uint32_t peer_p, const WorkItem& w,
                                                 const PairParams& p, const CUtensorMap* qmap, uint32_t tmem, int row, int q4, int lane,
                                                 uint32_t& g, uint32_t& qcount, uint32_t it, WorkItem* next, int* next_idx) {
@@ -213,10 +212,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
         mbar_wait(&sm->s_full[b], ph);
         if (row == 0) PTRACE(2, g);
-        if (pg == npages - 1) {  // every S-MMA of this item has retired: Q may be replaced
-            *next = sc_fetch_item(sm, p, lane, it + 1, next_idx);
-            if (*next_idx >= 0) sc_load_q(sm, *next, p, qmap, tmem, row, q4, lane, qcount, it + 1);
-        }
         tc_fence_after();
         float x[64];
         tmem_ld32(tmem + lane_base + kColS2 + b * 64, reinterpret_cast<uint32_t*>(x));
@@ -310,6 +305,11 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
     }
     if (tok < w.n_q && p.lse_chunk) p.lse_chunk[size_t(w.q_index + tok) * kHeads + head] = (m_ref + log2f(l)) * kLn2b;
     if (row == 0) PTRACE(10, it * 4 + 3);
+    // Every S-MMA of this item has retired (its last s_full was consumed above): Q may be replaced.  The next item's Q is
+    // loaded only now, after the last P and 1/l have left, so that the ~7k-cycle load overlaps the O-CTA's last PV and its
+    // epilogue (which otherwise stall the next item's first pages) instead of delaying them.
+    *next = sc_fetch_item(sm, p, lane, it + 1, next_idx);
+    if (*next_idx >= 0) sc_load_q(sm, *next, p, qmap, tmem, row, q4, lane, qcount, it + 1);
 }
 
 // S-CTA, MMA warp (converged; one elected lane issues)
@@ -386,11 +386,8 @@ __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_sm
         const int qd = lane & 3;
         const int rbase = row - qd;  // first row of this quad
         __nv_bfloat16* obase = p.out_chunk + (size_t(w.q_index) * kHeads) * kLatent;
-#pragma unroll 1
-        for (int c = 0; c < 16; ++c) {
-            uint32_t r[32];
-            tmem_ld32(tmem + lane_base + c * 32, r);
-            tmem_wait_ld();
+        // the tcgen05.ld of block c + 1 is in flight while block c is converted, transposed and stored
+        auto emit = [&](const uint32_t (&r)[32], int c) {
             uint4 e[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -421,6 +418,17 @@ __device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_sm
                 if ((rr >> 4) < w.n_q)
                     *reinterpret_cast<uint4*>(obase + size_t(rr) * kLatent + c * 32 + qd * 8) = e[i];
             }
+        };
+        uint32_t ra[32], rb[32];
+        tmem_ld32(tmem + lane_base, ra);
+#pragma unroll 1
+        for (int c = 0; c < 16; c += 2) {
+            tmem_wait_ld();
+            tmem_ld32(tmem + lane_base + (c + 1) * 32, rb);
+            emit(ra, c);
+            tmem_wait_ld();
+            if (c + 2 < 16) tmem_ld32(tmem + lane_base + (c + 2) * 32, ra);
+            emit(rb, c + 1);
         }
     }
     tc_fence_before();
@@ -503,6 +511,7 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
         mbar_init(&sm->o_empty, 4);
         fence_barrier_init();
     }
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // a decode grid queued behind this kernel may take SMs as clusters finish
     if (warp == 0 && lane == 0) prefetch_tensormap(rank == 0 ? &pool_map_k : &pool_map_v);
     if (warp == 2 && lane == 0 && rank == 0) prefetch_tensormap(&q_map);
     if (warp == 1) tmem_alloc(&sm->tmem_base, 512);
@@ -670,7 +679,7 @@ int pair_init(kairos_ctx* ctx) {
 
 // Launches n_pairs 2-CTA clusters over the chunk-tile items (kind 1, 8-token tiles, no KV split) on `stream`.
 int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,
-                     cudaStream_t stream) {
+                     cudaStream_t stream, bool pdl) {
     PairParams p;
     p.trace = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + ctx->cfg.workspace_bytes - 8192);  // KAIROS_TRACE builds only
     p.items = dev_items;
@@ -694,7 +703,20 @@ int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q tile) failed: " + std::to_string(int(r)));
     }
-    kairos_chunk_pair_kernel<<<2 * n_pairs, kPairThreads, kPairSmem, stream>>>(ctx->pool_map_c, ctx->pool_map_v, q_map, p);
+    // pdl: launched right behind the decode grid on the same stream with programmatic stream serialisation, so that the
+    // clusters start as soon as every decode CTA is resident (that kernel triggers launch_dependents at its start) and
+    // run beside it; neither kernel reads what the other writes, so this kernel has no griddepcontrol.wait.
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(unsigned(2 * n_pairs), 1, 1);
+    cfg.blockDim = dim3(kPairThreads, 1, 1);
+    cfg.dynamicSmemBytes = kPairSmem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_chunk_pair_kernel, ctx->pool_map_c, ctx->pool_map_v, q_map, p));
     KAIROS_CUDA_TRY(cudaGetLastError());
     return KAIROS_OK;
 }

@@ -120,6 +120,7 @@ struct KParams {
     float* lse_chunk;
     uint8_t* partials;
     float scale_log2;
+    int32_t static_first;  // 1: CTA b starts with item b and the queue hands out items from gridDim.x on
 };
 
 __device__ __forceinline__ WorkItem load_item(const WorkItem* p) {
@@ -490,8 +491,8 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
         const uint32_t kv_u32 = smem_u32(base + kOffKV);
         for (uint32_t it = 0;; ++it) {
             int idx = int(blockIdx.x);  // the first item is static (grid <= n_items): no queue round trip before the first load
-            if (it > 0) {
-                if (lane == 0) idx = atomicAdd(&p.counters[0], 1) + int(gridDim.x);
+            if (it > 0 || !p.static_first) {
+                if (lane == 0) idx = atomicAdd(&p.counters[0], 1) + (p.static_first ? int(gridDim.x) : 0);
                 idx = __shfl_sync(0xffffffffu, idx, 0);
             }
             if (idx >= p.n_items) idx = -1;
@@ -767,7 +768,8 @@ int umma_init(kairos_ctx* ctx) {
 }
 
 int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
-                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched, int max_ctas) {
+                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched, int max_ctas,
+                     bool as_clusters, bool pdl) {
     CUtensorMap qd_map = ctx->pool_map, qc_map = ctx->pool_map;  // placeholders when a side is empty (never dereferenced)
     if (a.n_dec > 0)
         if (int rc = encode_rows_map(&qd_map, a.q_dec, uint64_t(a.n_dec) * kHeads, 16)) return rc;
@@ -788,14 +790,41 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.lse_chunk = a.lse_chunk;
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
-    const int grid = std::max(1, std::min(n_items, std::min(max_ctas, umma_resident_ctas(ctx))));
+    int grid = std::max(1, std::min(n_items, std::min(max_ctas, umma_resident_ctas(ctx))));
+    // beside the pair kernel the grid is launched as 2-CTA clusters (nothing in the kernel uses the cluster): it then
+    // occupies whole TPCs, which the chunk clusters need, and the first item comes from the queue (a CTA that becomes
+    // resident late must not be holding a statically assigned item)
+    const bool with_pairs = ctx->plan.n_pairs > 0;
+    if (as_clusters) grid = std::max(2, std::min(max_ctas, umma_resident_ctas(ctx)) & ~1);
+    p.static_first = with_pairs ? 0 : 1;
     // decode-only queues (no chunk, or the chunk is on the pair grid) take the instantiation with the deeper page ring
     bool dec_only = a.chunk_len == 0 || ctx->plan.n_chunk_items == 0;
     if (ctx->force_dec_only >= 0) dec_only = dec_only && ctx->force_dec_only != 0;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(unsigned(grid), 1, 1);
+    cfg.blockDim = dim3(kThreads, 1, 1);
+    cfg.dynamicSmemBytes = dec_only ? Geo<true>::kSmemBytes : Geo<false>::kSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[2];
+    int n_attr = 0;
+    if (as_clusters) {
+        attr[n_attr].id = cudaLaunchAttributeClusterDimension;
+        attr[n_attr].val.clusterDim.x = 2;
+        attr[n_attr].val.clusterDim.y = 1;
+        attr[n_attr].val.clusterDim.z = 1;
+        ++n_attr;
+    }
+    if (pdl) {  // queued behind the pair kernel: CTAs become resident as clusters finish (this kernel never waits on it)
+        attr[n_attr].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n_attr].val.programmaticStreamSerializationAllowed = 1;
+        ++n_attr;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = n_attr;
     if (dec_only)
-        kairos_mixed_kernel<true><<<grid, kThreads, Geo<true>::kSmemBytes, stream>>>(ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p);
+        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_mixed_kernel<true>, ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p));
     else
-        kairos_mixed_kernel<false><<<grid, kThreads, Geo<false>::kSmemBytes, stream>>>(ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p);
+        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_mixed_kernel<false>, ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p));
     KAIROS_CUDA_TRY(cudaGetLastError());
     *kernels_launched = 1;
     (void)dev_combines;
@@ -820,7 +849,8 @@ int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_co
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
-        cfg.numAttrs = 1;
+        // with two attention kernels in flight (pair + decode grids) the combine is an ordinary launch: it must follow both
+        cfg.numAttrs = ctx->plan.n_pairs > 0 ? 0 : 1;
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, partials, out_dec, out_chunk, lse_dec, lse_chunk));
         KAIROS_CUDA_TRY(cudaGetLastError());
     }

@@ -56,7 +56,8 @@ struct Plan {
     std::vector<WorkItem> items;       // execution order (longest first)
     std::vector<CombineItem> combines;
     std::vector<WorkItem> pair_items;  // chunk tiles of 8 tokens for the 2-CTA pair kernel (empty: chunk runs as gen-1 tiles)
-    int32_t n_pairs = 0;               // clusters the pair kernel is launched with (SMs 2*n_pairs are taken from the decode grid)
+    int32_t n_pairs = 0;               // clusters the pair kernel is launched with (one per SM pair, at most one per tile)
+    int32_t dec_ctas = 0;              // with n_pairs > 0: CTAs of the decode grid launched BEFORE the clusters (even); 0 = one per SM, behind them
     int32_t n_decode_items = 0;
     int32_t n_chunk_items = 0;
     int32_t n_partial_slots = 0;
@@ -77,6 +78,7 @@ struct StagingSlot {
     void* dev = nullptr;
     size_t bytes = 0;
     cudaEvent_t done = nullptr;  // recorded after the H2D copy out of `host`
+    cudaEvent_t consumed = nullptr;  // recorded on the caller's stream after the kernels that read `dev` (plan copies only)
     bool used = false;
 };
 
@@ -97,6 +99,7 @@ struct kairos_ctx {
     int force_dec_only = -1;      // KAIROS_DEC_ONLY env (sweeps): 0 = never use the decode-only instantiation
     CUtensorMap pool_map_c;       // one 64-dim chunk of a page (8 KB box): K ring of the pair kernel's S-CTA
     CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
+    cudaStream_t copy_stream = nullptr; // the plan's H2D copy runs here, beside whatever precedes the step on the caller's stream
     cudaStream_t aux_stream = nullptr;  // the pair kernel runs beside the decode kernel on this stream (event fork / join)
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int force_pairs = -1;         // KAIROS_PAIRS env: -1 auto, 0 never use the pair kernel, n > 0 use n pairs
@@ -145,7 +148,7 @@ int umma_chunk_tile_tokens();
 int umma_resident_ctas(const kairos_ctx* ctx);
 int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
                      const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched,
-                     int max_ctas);
+                     int max_ctas, bool as_clusters, bool pdl);
 int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream);
 int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
 
@@ -153,6 +156,6 @@ int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
 int pair_tile_tokens();
 int pair_init(kairos_ctx* ctx);
 int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,
-                     cudaStream_t stream);
+                     cudaStream_t stream, bool pdl);
 
 }  // namespace kairos

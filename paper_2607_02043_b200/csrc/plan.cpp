@@ -16,17 +16,22 @@ constexpr int kChunkCostDen = 4;       // (tensor-bound tile-page vs HBM-bound d
 
 inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b); }
 
-// Cost model of the static SM partition between the pair kernel (chunk) and the decode grid, in nominal SM cycles
-// (1.965 GHz), calibrated on B200 (profiles/r01_bench_gen2.md): one 8-token tile x 64-key page on a pair (at the clocks the
-// chip sustains under tensor load), the fixed cost of a tile (Q load, pipeline fill, epilogue), one decode page on one CTA
-// (latency-bound, two pages in flight), the HBM floor per decode page with every SM streaming, and the same 8-token
-// tile-page done as two gen-1 tiles (what the pair path has to beat).
-constexpr int64_t kPairPageCycles = 1750;
-constexpr int64_t kPairItemCycles = 32000;
-constexpr int64_t kDecPageCycles = 3000;
+// Cost model of the SM sharing between the pair kernel (chunk) and the decode grid, in nominal SM cycles (1.965 GHz),
+// calibrated on B200 (profiles/r01_bench_gen3.md): one 8-token tile x 64-key page on a pair (at the clocks the chip
+// sustains under tensor load), the fixed cost of a tile (Q load, pipeline fill, epilogue), one decode page on one CTA
+// when HBM is not the limit, the HBM floor per decode page with every SM streaming, and the same 8-token tile-page done
+// as two gen-1 tiles (what the pair path has to beat).
+constexpr int64_t kPairPageCycles = 1800;
+constexpr int64_t kPairItemCycles = 27000;
+constexpr int64_t kDecPageCycles = 2600;
 constexpr int64_t kDecPageHbmSmCycles = 4260;
 constexpr int64_t kGen1PairPageSmCycles = 7570;
 
+// When the chunk runs on the pair kernel, clusters are launched for EVERY SM pair (up to one per tile) and the two grids
+// share the SMs in time: the decode grid is launched first on `dec_ctas` SMs (as 2-CTA clusters, so that it occupies whole
+// TPCs), the clusters that do not fit beside it become resident when the decode CTAs exit and join the tile queue
+// then.  dec_ctas = 0 means the decode grid is launched behind the pair grid with one CTA per SM and fills the SMs the
+// clusters leave as they finish (the chunk is so much larger than the decode work that a static share would idle).
 void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len, int32_t ctas,
                   int32_t pair_mode, int32_t T2, Plan* plan) {
     if (pair_mode == 0 || chunk_len <= 0 || ctas < 2) return;
@@ -36,30 +41,39 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
         pair_pages += ceil_div(int64_t(prefix_len) + std::min(chunk_len, (t + 1) * T2), kPage);
     int64_t dec_pages = 0;
     for (int32_t i = 0; i < n_dec; ++i) dec_pages += ceil_div(dec_ctx_lens[i], kPage);
-    const int32_t max_pairs = std::min(n_tiles, n_dec > 0 ? (ctas - 1) / 2 : ctas / 2);
+    const int32_t max_pairs = std::min(n_tiles, ctas / 2);
     if (max_pairs < 1) return;
-    int32_t n_p;
-    if (pair_mode > 0) {
-        n_p = std::min(pair_mode, max_pairs);
-    } else {
-        const int64_t work_c = pair_pages * kPairPageCycles + int64_t(n_tiles) * kPairItemCycles;
-        if (n_dec == 0) {
-            n_p = max_pairs;
-            if (work_c / n_p > pair_pages * kGen1PairPageSmCycles / ctas) return;  // few short tiles: gen-1 tiles use every SM
-        } else {
-            int64_t best = -1;
-            n_p = 1;
-            for (int32_t c = 1; c <= max_pairs; ++c) {
-                const int64_t tc = work_c / c;
-                const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmSmCycles / ctas);
-                const int64_t t = std::max(tc, td);
-                if (best < 0 || t < best) { best = t; n_p = c; }
-            }
-            // one queue for everything (gen-1 tiles ride in the decode grid) unless the partition is clearly faster
-            const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
-            if (best * 10 > t_gen1 * 8) return;
+    const int64_t work_c = pair_pages * kPairPageCycles + int64_t(n_tiles) * kPairItemCycles;
+    int32_t dec_ctas = 0;
+    if (n_dec > 0) {
+        // c = clusters resident while the decode grid runs on ctas - 2c SMs; afterwards all max_pairs clusters run
+        auto total = [&](int32_t c) {
+            const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmSmCycles / ctas);
+            return td + std::max<int64_t>(0, work_c - int64_t(c) * td) / max_pairs;
+        };
+        int32_t c_lo = 0, c_hi = std::min(max_pairs, (ctas - 2) / 2);
+        if (pair_mode > 0) c_lo = c_hi = std::min(pair_mode, c_hi);
+        int64_t best = -1;
+        int32_t best_c = 0;
+        for (int32_t c = c_lo; c <= c_hi; ++c) {
+            // c = 0 stands for "decode behind the clusters": chunk on every pair, then the decode pages at the HBM rate
+            const int64_t t = c == 0 ? work_c / max_pairs + dec_pages * kDecPageHbmSmCycles / ctas : total(c);
+            if (best < 0 || t < best) { best = t; best_c = c; }
         }
+        if (pair_mode < 0) {
+            // one queue for everything (gen-1 tiles ride in the decode grid) unless sharing is clearly faster
+            const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
+            if (best * 10 > t_gen1 * 9) return;
+            // a chunk that dwarfs the decode work: a static share idles (tile quantisation, contention) more than the overlap
+            // gains; measured on configs[2] and [4] (profiles/r01_bench_gen3.md): the decode CTAs fill the clusters' tail instead
+            if (work_c / max_pairs >= 4 * (dec_pages * kDecPageHbmSmCycles / ctas)) best_c = 0;
+        }
+        dec_ctas = best_c == 0 || pair_mode >= max_pairs ? 0 : ctas - 2 * best_c;
+    } else if (pair_mode < 0) {
+        if (work_c / max_pairs > pair_pages * kGen1PairPageSmCycles / ctas) return;  // few short tiles: gen-1 tiles use every SM
     }
+    const int32_t n_p = (n_dec == 0 && pair_mode > 0) ? std::min(pair_mode, max_pairs) : max_pairs;
+    plan->dec_ctas = dec_ctas;
     plan->n_pairs = n_p;
     for (int32_t t = 0; t < n_tiles; ++t) {
         WorkItem w{};
@@ -83,12 +97,13 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
     plan->combines.clear();
     plan->pair_items.clear();
     plan->n_pairs = 0;
+    plan->dec_ctas = 0;
     plan->n_decode_items = plan->n_chunk_items = plan->n_partial_slots = 0;
     if (target_ctas < 1) target_ctas = 1;
     choose_pairs(dec_ctx_lens, n_dec, chunk_len, prefix_len, target_ctas, pair_mode, T2, plan);
-    if (plan->n_pairs > 0) {  // the chunk runs on its own SM pairs: the queue below holds decode splits only
+    if (plan->n_pairs > 0) {  // the chunk runs on SM pairs: the queue below holds decode splits only
         chunk_len = 0;
-        target_ctas = std::max(1, target_ctas - 2 * plan->n_pairs);
+        if (plan->dec_ctas > 0) target_ctas = plan->dec_ctas;
     }
 
     // ---- total cost, in units of 4*decode-page

@@ -22,7 +22,7 @@ def _check_plan(lens, C, P, n_ctas=148, pair_mode=0):
     chk = items[items[:, KIND] >= 1]
     if n_pairs > 0:  # the chunk runs on the cluster kernel: whole 8-token tiles, no KV split, clusters fit beside the decode grid
         assert (chk[:, KIND] == 2).all() and (chk[:, SLOT] == -1).all() and (chk[:, PB] == 0).all()
-        assert 1 <= n_pairs <= min(len(chk), n_ctas // 2) and (len(lens) == 0 or 2 * n_pairs < n_ctas)
+        assert 1 <= n_pairs <= min(len(chk), n_ctas // 2) and 2 * n_pairs <= n_ctas
         assert (np.diff(chk[:, COST]) <= 0).all()
     else:
         assert (chk[:, KIND] == 1).all()
