@@ -306,6 +306,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         if (lane == (c & 15)) sm->red[w4][cbase + c] = v;
     }
     named_sync(1);
+    if (tid_s == 0 && it == 0) KTRACE(11, 0);
     const bool is_final = w.partial_slot < 0;
     if (tid_s < N) {
         const float L = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
@@ -325,25 +326,35 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         }
     }
     named_sync(2);
+    if (tid_s == 0 && it == 0) KTRACE(11, 1);
+    // TMEM reads run at 64 B/clk per SM and each tcgen05.ld round trip costs several hundred cycles: the loads of block
+    // b4 + 1 are in flight while block b4 is converted and stored
+    uint32_t rr[2][NC];
+    auto load_block = [&](int b4, uint32_t* r) {
+#pragma unroll
+        for (int c0 = 0; c0 < NC; c0 += W) tmem_ldw<W>(tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + cbase + c0), r + c0);
+    };
+    load_block(0, rr[0]);
 #pragma unroll
     for (int b4 = 0; b4 < 4; ++b4) {
+        if (tid_s == 0 && it == 0) KTRACE(11, 2 + b4);
+        tmem_wait_ld();
+        if (b4 < 3) load_block(b4 + 1, rr[(b4 + 1) & 1]);
+        const uint32_t* r = rr[b4 & 1];
         const int d = b4 * 128 + w4 * 32 + lane;
 #pragma unroll
         for (int c0 = 0; c0 < NC; c0 += W) {
             const int col = cbase + c0;
             const int tok = col >> 4;
             if (tok >= w.n_q) continue;  // ragged chunk tail (uniform across the warp)
-            uint32_t r[W];
-            tmem_ldw<W>(tmem_addr(tmem, w4 * 32, kColO + b4 * 64 + col), r);
-            tmem_wait_ld();
             if (is_final) {
                 __nv_bfloat16* o = (w.kind ? p.out_chunk : p.out_dec) + (size_t(w.q_index + tok) * kHeads + (col & 15)) * kLatent + d;
 #pragma unroll
-                for (int i = 0; i < W; ++i) o[i * kLatent] = __float2bfloat16_rn(__uint_as_float(r[i]) * sm->linv[col + i]);
+                for (int i = 0; i < W; ++i) o[i * kLatent] = __float2bfloat16_rn(__uint_as_float(r[c0 + i]) * sm->linv[col + i]);
             } else {
                 float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot + tok) * kPartialSlotBytes) + (col & 15) * kLatent + d;
 #pragma unroll
-                for (int i = 0; i < W; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[i]));
+                for (int i = 0; i < W; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[c0 + i]));
             }
         }
     }

@@ -11,8 +11,14 @@ namespace kairos {
 
 namespace {
 constexpr int kMinSplitPages = 4;      // never cut a KV range into pieces shorter than this
-constexpr int kChunkCostNum = 3;       // cost of one chunk tile-page relative to one decode page = 3/4
-constexpr int kChunkCostDen = 4;       // (tensor-bound tile-page vs HBM-bound decode page; measured)
+// Item costs in units of a quarter decode page (~550 SM cycles), from the CTA timelines under profiles/: a gen-1 chunk
+// tile-page (N = 64 softmax on the critical path) costs ~1.5 decode pages, and every item carries a fixed cost
+// (Q load, pipeline fill, epilogue: ~3k cycles for a decode split, ~9k for a chunk tile).  Only the ORDER of the queue
+// (longest first) and the chunk / decode interleave depend on the fixed parts.
+constexpr int kChunkCostNum = 6;
+constexpr int kChunkCostDen = 4;
+constexpr int kDecItemFixedCost = 5;
+constexpr int kChunkItemFixedCost = 16;
 
 inline int32_t ceil_div(int64_t a, int64_t b) { return int32_t((a + b - 1) / b); }
 
@@ -183,7 +189,7 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
                 w.n_keys = dec_ctx_lens[i];
                 w.n_q = 1;
                 w.partial_slot = n_splits > 1 ? first_slot + s : -1;
-                w.cost = (w.page_end - w.page_begin) * kChunkCostDen;
+                w.cost = (w.page_end - w.page_begin) * kChunkCostDen + kDecItemFixedCost;
                 dec_items.push_back(w);
             }
         }
@@ -220,7 +226,7 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
             w.n_keys = prefix_len + q0 + 1;
             w.n_q = nq;
             w.partial_slot = n_splits > 1 ? first_slot + s * T : -1;
-            w.cost = (w.page_end - w.page_begin) * kChunkCostNum;
+            w.cost = (w.page_end - w.page_begin) * kChunkCostNum + kChunkItemFixedCost;
             chunk_items.push_back(w);
         }
     }
