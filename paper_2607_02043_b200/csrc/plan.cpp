@@ -32,6 +32,7 @@ constexpr int64_t kPairItemCycles = 27000;
 constexpr int64_t kDecPageCycles = 2600;
 constexpr int64_t kDecPageHbmSmCycles = 4260;
 constexpr int64_t kGen1PairPageSmCycles = 7570;
+constexpr int64_t kKernelFloorCycles = 25000;  // launch, first loads, first chain, epilogue of a persistent kernel (~12.7 us)
 
 // When the chunk runs on the pair kernel, clusters are launched for EVERY SM pair (up to one per tile) and the two grids
 // share the SMs in time: the decode grid is launched first on `dec_ctas` SMs (as 2-CTA clusters, so that it occupies whole
@@ -51,34 +52,58 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
     if (max_pairs < 1) return;
     const int64_t work_c = pair_pages * kPairPageCycles + int64_t(n_tiles) * kPairItemCycles;
     int32_t dec_ctas = 0;
-    if (n_dec > 0) {
-        // c = clusters resident while the decode grid runs on ctas - 2c SMs; afterwards all max_pairs clusters run
-        auto total = [&](int32_t c) {
-            const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), dec_pages * kDecPageHbmSmCycles / ctas);
+    int32_t n_p = max_pairs;
+    if (pair_mode < -1) {
+        // forced (sweeps): -(n + 1) = n clusters first, the decode grid on every SM behind them
+        n_p = std::min(-pair_mode - 1, max_pairs);
+    } else if (n_dec > 0) {
+        const int64_t td_all = dec_pages * kDecPageHbmSmCycles / ctas;  // decode alone, every SM streaming
+        // (A) decode first on ctas - 2c SMs, c clusters beside it, every cluster afterwards
+        auto t_dec_first = [&](int32_t c) {
+            const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), td_all);
             return td + std::max<int64_t>(0, work_c - int64_t(c) * td) / max_pairs;
         };
-        int32_t c_lo = 0, c_hi = std::min(max_pairs, (ctas - 2) / 2);
-        if (pair_mode > 0) c_lo = c_hi = std::min(pair_mode, c_hi);
+        // (B) n clusters first, the decode grid (one CTA per SM) behind them: it takes the other SMs at once and the
+        // clusters' SMs as they finish; n = max_pairs means the decode CTAs only fill the clusters' tail
+        auto t_pairs_first = [&](int32_t n) {
+            const int64_t tiles_each = ceil_div(n_tiles, n);
+            const int64_t tc = std::max(work_c / n, tiles_each * (work_c / n_tiles));
+            const int64_t done = std::min<int64_t>({dec_pages, tc * (ctas - 2 * n) / kDecPageCycles, tc * ctas / kDecPageHbmSmCycles});
+            return tc + (dec_pages - done) * kDecPageHbmSmCycles / ctas;
+        };
         int64_t best = -1;
-        int32_t best_c = 0;
-        for (int32_t c = c_lo; c <= c_hi; ++c) {
-            // c = 0 stands for "decode behind the clusters": chunk on every pair, then the decode pages at the HBM rate
-            const int64_t t = c == 0 ? work_c / max_pairs + dec_pages * kDecPageHbmSmCycles / ctas : total(c);
-            if (best < 0 || t < best) { best = t; best_c = c; }
-        }
-        if (pair_mode < 0) {
+        int32_t best_c = 0, best_n = 0;  // exactly one of them ends up > 0
+        if (pair_mode > 0) {
+            best_c = std::min({pair_mode, max_pairs, (ctas - 2) / 2});
+            if (pair_mode >= max_pairs) { best_c = 0; best_n = max_pairs; }
+        } else if (ceil_div(work_c, (td_all + kKernelFloorCycles) * 8 / 10) <= std::min(max_pairs, 48)) {
+            // a chunk that is small beside the decode work (measured, profiles/r01_bench_gen3.md: configs[3] C <= 1024): just
+            // enough clusters to finish it a little before the decodes would, launched first; the decode grid (the
+            // decode-only instantiation with the deeper ring) streams on the other SMs and inherits theirs
+            best_n = std::max(std::min(8, max_pairs), ceil_div(work_c, (td_all + kKernelFloorCycles) * 8 / 10));
+        } else {
+            for (int32_t c = 1; c <= std::min(max_pairs, (ctas - 2) / 2); ++c) {
+                const int64_t t = t_dec_first(c);
+                if (best < 0 || t < best) { best = t; best_c = c; best_n = 0; }
+            }
+            for (int32_t n = 1; n <= max_pairs; ++n) {
+                const int64_t t = t_pairs_first(n);
+                if (best < 0 || t < best) { best = t; best_c = 0; best_n = n; }
+            }
             // one queue for everything (gen-1 tiles ride in the decode grid) unless sharing is clearly faster
             const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
             if (best * 10 > t_gen1 * 9) return;
             // a chunk that dwarfs the decode work: a static share idles (tile quantisation, contention) more than the overlap
             // gains; measured on configs[2] and [4] (profiles/r01_bench_gen3.md): the decode CTAs fill the clusters' tail instead
-            if (work_c / max_pairs >= 4 * (dec_pages * kDecPageHbmSmCycles / ctas)) best_c = 0;
+            if (work_c / max_pairs >= 4 * td_all) { best_c = 0; best_n = max_pairs; }
         }
-        dec_ctas = best_c == 0 || pair_mode >= max_pairs ? 0 : ctas - 2 * best_c;
+        if (best_c > 0) dec_ctas = ctas - 2 * best_c;
+        else n_p = best_n;
     } else if (pair_mode < 0) {
         if (work_c / max_pairs > pair_pages * kGen1PairPageSmCycles / ctas) return;  // few short tiles: gen-1 tiles use every SM
+    } else {
+        n_p = std::min(pair_mode, max_pairs);
     }
-    const int32_t n_p = (n_dec == 0 && pair_mode > 0) ? std::min(pair_mode, max_pairs) : max_pairs;
     plan->dec_ctas = dec_ctas;
     plan->n_pairs = n_p;
     for (int32_t t = 0; t < n_tiles; ++t) {

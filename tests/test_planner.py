@@ -103,10 +103,10 @@ def test_plan_with_pair_kernel(lens, C, P, pair_mode):
     _check_plan(lens, C, P, n_ctas=7, pair_mode=pair_mode)
 
 
-def test_planner_picks_the_pair_kernel_for_large_chunks_only():
+def test_planner_policy_for_the_pair_kernel():
     n = lambda lens, C, P: K.plan_dump(lens, C, P, 148, pair_mode=-1, with_pairs=True)[2]
     assert n([64, 128, 200, 256], 64, 128) == 0          # configs[0]
-    assert n([2048] * 256, 512, 0) == 0                  # small chunk rides in the decode queue as gen-1 tiles
+    assert 8 <= n([2048] * 256, 512, 0) <= 16            # small chunk beside many decodes: a few clusters first, decode grid behind
     assert n([2048] * 256, 8192, 0) > 40                 # tensor-bound: most SM pairs go to the chunk
     assert n([32768] * 32, 4096, 28672) > 40             # configs[4]
     assert n([], 8192, 0) == 74
