@@ -170,8 +170,10 @@ int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int32_t nB, co
  * kairos_workspace_bytes bound.
  *   dec_ctx_lens   HOST int32 [n_dec] (each >= 1)
  *   pair_mode      0 = the chunk runs as 4-token tiles in the same queue as the decode splits; -1 = the planner
- *                  decides whether the chunk runs as 8-token tiles on 2-CTA clusters beside the decode grid (and on
- *                  how many), as kairos_mixed_step does; n > 0 = force n clusters
+ *                  decides whether the chunk runs as 8-token tiles on 2-CTA clusters that share the SMs in time with
+ *                  the decode grid, and in which order the two grids are launched, as kairos_mixed_step does
+ *                  (DESIGN.md 6.2); n > 0 = the decode grid first, beside n resident clusters (n >= every SM pair:
+ *                  the clusters first); -(n + 1) = n clusters first, the decode grid on every SM behind them
  *   items_out      HOST int32 [max_items][8]: kind (0 decode split / 1 chunk tile in the queue / 2 chunk tile of the
  *                  cluster kernel), q_index (request index or first chunk token), page_begin, page_end, n_keys, n_q,
  *                  partial_slot (-1 = final output), cost; queue order, then the cluster kernel's items.  May be NULL.

@@ -274,10 +274,7 @@ int kairos_destroy(kairos_ctx* ctx) {
     }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
     for (auto e : ctx->prof_events) cudaEventDestroy(e);
-    if (ctx->aux_stream) cudaStreamDestroy(ctx->aux_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
-    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete ctx;
     return KAIROS_OK;
 }

@@ -671,9 +671,6 @@ int pair_init(kairos_ctx* ctx) {
                                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool, chunk box) failed: " + std::to_string(int(r)));
     KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_chunk_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
-    KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking));
-    KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
-    KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
     return KAIROS_OK;
 }
 

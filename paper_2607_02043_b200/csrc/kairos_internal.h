@@ -100,9 +100,8 @@ struct kairos_ctx {
     CUtensorMap pool_map_c;       // one 64-dim chunk of a page (8 KB box): K ring of the pair kernel's S-CTA
     CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
     cudaStream_t copy_stream = nullptr; // the plan's H2D copy runs here, beside whatever precedes the step on the caller's stream
-    cudaStream_t aux_stream = nullptr;  // the pair kernel runs beside the decode kernel on this stream (event fork / join)
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    int force_pairs = -1;         // KAIROS_PAIRS env: -1 auto, 0 never use the pair kernel, n > 0 use n pairs
+    int force_pairs = -1;         // KAIROS_PAIRS env (sweeps): -1 auto, 0 never use the pair kernel, n > 0 decode grid first beside n
+                                  // clusters, -(n + 1) n clusters first (plan.cpp::choose_pairs)
     static constexpr int kStagingSlots = 4;
     kairos::StagingSlot staging[kStagingSlots];
     int staging_next = 0;
