@@ -251,11 +251,28 @@ def _sampled_compare(inp, n_dec_samples=8, n_chunk_samples=24):
     return Hp.assert_attention_close(g, r, inp.name + " (sampled rows)")
 
 
+# The three orders in which the decode grid and the chunk clusters share the SMs, and the chunk as gen-1
+# tiles of the decode queue, each on every row of configs[1]: KAIROS_PAIRS n > 0 = decode grid first (as 2-CTA clusters)
+# beside n chunk clusters, -(n + 1) = n chunk clusters first with the full decode grid behind them, 0 = one queue.
+@pytest.mark.parametrize("pairs", [0, 20, -17, 74])
+def test_config1_every_row_in_every_launch_order(pairs):
+    run, _, _ = _full_compare(W.make_config(1), "umma", pairs=pairs)
+    info = run.ctx.last_plan_info()
+    assert (info["chunk_pairs"] == 0) == (pairs == 0)
+
+
+@pytest.mark.parametrize("name,kw", [e for e in EDGE if e[1]["chunk_len"] > 0 and len(e[1]["dec_ctx_lens"]) > 0],
+                         ids=[e[0] for e in EDGE if e[1]["chunk_len"] > 0 and len(e[1]["dec_ctx_lens"]) > 0])
+def test_edge_cases_clusters_first(name, kw):
+    inp = W.make_inputs(name, 100 + len(name), q_scale=0.5, extra_pages=3, **kw)
+    _full_compare(inp, "umma", pairs=-3)
+
+
 def test_config2_heavy_tail_sampled_rows():
     _sampled_compare(W.make_config(2))
 
 
-@pytest.mark.parametrize("C", [0, 512, 8192])
+@pytest.mark.parametrize("C", [0, 512, 2048, 8192])
 def test_config3_chunk_sweep_sampled_rows(C):
     _sampled_compare(W.make_config(3, chunk_len=C))
 
