@@ -625,6 +625,9 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
     // ---- teardown: neither CTA may exit while its peer can still touch its shared memory
     tc_fence_before();
     __syncthreads();
+    // launched behind the decode grid with programmatic stream serialisation: wait for that grid before exiting, so that this
+    // grid's completion implies the decode grid's for everything that follows in the stream (no-op for an ordinary launch)
+    if (threadIdx.x == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
     cluster_arrive();
     cluster_wait();
     if (warp == 1) tmem_dealloc(tmem, 512);
@@ -702,7 +705,7 @@ int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     }
     // pdl: launched right behind the decode grid on the same stream with programmatic stream serialisation, so that the
     // clusters start as soon as every decode CTA is resident (that kernel triggers launch_dependents at its start) and
-    // run beside it; neither kernel reads what the other writes, so this kernel has no griddepcontrol.wait.
+    // run beside it; neither kernel reads what the other writes, so this kernel only executes griddepcontrol.wait before it exits.
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(unsigned(2 * n_pairs), 1, 1);
     cfg.blockDim = dim3(kPairThreads, 1, 1);

@@ -615,6 +615,10 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
     // ---- teardown
     tc_fence_before();
     __syncthreads();
+    // When this grid was launched behind the pair kernel with programmatic stream serialisation it never waited for it; it
+    // does so before it exits, so that "this grid has completed" implies "the pair grid has completed" for everything that
+    // follows in the stream (the combine, the caller's consumers of out_chunk).  No-op for an ordinary launch.
+    if (threadIdx.x == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
     if (threadIdx.x == 0) KTRACE(10, 7);
 #ifdef KAIROS_TRACE
     if (threadIdx.x == 0) KSTAT(1, gtime());
@@ -860,8 +864,8 @@ int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_co
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
-        // with two attention kernels in flight (pair + decode grids) the combine is an ordinary launch: it must follow both
-        cfg.numAttrs = ctx->plan.n_pairs > 0 ? 0 : 1;
+        // with two attention kernels in flight the second one waits for the first before it exits, so following it is enough
+        cfg.numAttrs = 1;
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, partials, out_dec, out_chunk, lse_dec, lse_chunk));
         KAIROS_CUDA_TRY(cudaGetLastError());
     }
