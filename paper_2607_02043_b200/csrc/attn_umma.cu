@@ -411,10 +411,13 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
         }
         if (s_next < npages && s_next <= pv_next + 1) {
             const uint32_t gg = g0 + s_next;
-            const uint32_t st = gg & 1, ph = (gg >> 1) & 1;
+            const uint32_t st = gg & 1;
             if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[gg & (kPageRing - 1)], (gg / kPageRing) & 1))) {
                 KTRACE(1, gg);
-                mbar_wait(&sm->s_empty[st], ph ^ 1);  // the softmax warps have read this S^T buffer (tcgen05.ld)
+                // No wait on s_empty: S(g) reuses the S^T buffer of page g - 2, whose PV has been issued (s_next <= pv_next + 1,
+                // and an item returns only after its last PV), i.e. p_full(g - 2) was observed, and every softmax warp arrives
+                // on s_empty (after its tcgen05.ld of S^T) before it arrives on p_full.  A completed mbarrier wait still costs
+                // this warp ~100 cycles, and it is the serial resource of the page chain.
                 tc_fence_after();
                 const PageSlots ps = page_slots<R>(gg);
 #pragma unroll
