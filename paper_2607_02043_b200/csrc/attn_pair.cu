@@ -324,10 +324,10 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_
         mbar_wait(&sm->s_empty[b], bph ^ 1);
         PTRACE(0, g);
         const uint32_t kb_lo = smem_desc_lo(kv_base + st * kKStage, 16);
+        mbar_wait(&ring->kv_full[st * kGroups], sph);
+        tc_fence_after();
 #pragma unroll
         for (uint32_t gr = 0; gr < kGroups; ++gr) {
-            mbar_wait(&ring->kv_full[st * kGroups + gr], sph);
-            tc_fence_after();
 #pragma unroll
             for (uint32_t cc = 0; cc < kGroupChunks; ++cc) {
                 const uint32_t c = gr * kGroupChunks + cc;
@@ -562,10 +562,12 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
                         const uint32_t ns = rank == 0 ? kStagesK : kStages;
                         const uint32_t st = g % ns, sph = (g / ns) & 1;
                         if (rank == 0) {
+                            // one full barrier per page (a completed mbarrier wait costs the MMA warp ~100 cycles), one empty
+                            // barrier per group of chunks (a group is refilled as soon as its MMAs retire)
                             for (int gr = 0; gr < kGroups; ++gr) {
                                 mbar_wait(&ring->kv_empty[st * kGroups + gr], sph ^ 1);
-                                mbar_arrive_expect_tx(&ring->kv_full[st * kGroups + gr], kGroupChunks * 8192);
-                                tma_load_chunk(base + st * kKStage + gr * kGroupChunks * 8192, &pool_map_k, &ring->kv_full[st * kGroups + gr],
+                                if (gr == 0) mbar_arrive_expect_tx(&ring->kv_full[st * kGroups], kKStage);
+                                tma_load_chunk(base + st * kKStage + gr * kGroupChunks * 8192, &pool_map_k, &ring->kv_full[st * kGroups],
                                                pid * kPage, gr * kGroupChunks, kEvictLast);
                             }
                         } else {
