@@ -8,13 +8,16 @@
 //   P^T = exp2(S^T*c - m)  (column statistics across the 64 key lanes, lazy max update)
 //   O^T[512 x N]     += V^T[512 x 64] . P^T[64 x N]          tcgen05.mma M=128 x4, MN-major A = the SAME smem page
 //
-//   N = 16 query rows (1 decode token x 16 heads) or 64 (4 chunk tokens x 16 heads).  The page tile is loaded once
-//   by one 3-D TMA (SWIZZLE_128B, [9 chunks][64 tokens][128 B]) and serves as K (K-major) and as V (MN-major).
-//   Accumulators live in TMEM: S^T double-buffered (2 x 64 columns), O^T 4 x 64 columns, fp32.
+//   N = 16 query rows (1 decode token x 16 heads) or 64 (4 chunk tokens x 16 heads).  A page is loaded once by five TMA
+//   boxes (4 pairs of latent chunks + the RoPE chunk, SWIZZLE_128B, 8 KB slots of [64 tokens][128 B]) into a ring of
+//   slots and serves as K (K-major) and as V (MN-major).  Accumulators live in TMEM: S^T double-buffered (2 x 64 columns),
+//   O^T 4 x 64 columns, fp32.
 //
-// Warp roles (192 threads): warp 0 = TMA producer + work-queue pop, warp 1 = MMA issuer (one lane) + TMEM owner,
-// warps 2-5 = softmax / correction / epilogue (one TMEM lane quadrant each).
-// Descriptor encodings were validated on B200 by profiles/r01_tcgen05_probe.txt.
+// Warp roles (320 threads): warp 0 = TMA producer + work-queue pop, warp 1 = MMA issuer (one elected lane) + TMEM owner,
+// warps 2-9 = softmax / correction / epilogue (two per TMEM lane quadrant, half of the query columns each).
+// Two instantiations: <false> holds a 64-row chunk Q tile and 18 slots, <true> (queues without chunk tiles) two 16-row decode
+// Q buffers and 22 slots.  Descriptor encodings were validated on B200 by profiles/r01_tcgen05_probe.txt; DESIGN.md 6.1 has
+// the measurements behind the structure.
 #include <cuda_bf16.h>
 
 #include <algorithm>
