@@ -13,6 +13,11 @@ __global__ void __launch_bounds__(256) append_kernel(uint4* __restrict__ pool, c
                                                      const uint4* __restrict__ k_rope,
                                                      const int32_t* __restrict__ page_table, int32_t n_tokens,
                                                      int32_t start_pos) {
+    // Launched with programmatic stream serialisation: the grid may become resident while the previous kernel of the stream
+    // (typically the previous step's combine or attention kernel, which trigger launch_dependents on entry) is still
+    // running, and waits here until that kernel has completed and flushed -- the launch latency is hidden, the order is not
+    // relaxed (the previous step may still be reading the pages this step overwrites).
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int64_t total = int64_t(n_tokens) * kVecPerToken;
     for (int64_t i = blockIdx.x * int64_t(blockDim.x) + threadIdx.x; i < total; i += int64_t(gridDim.x) * blockDim.x) {
         const int32_t j = int32_t(i / kVecPerToken);
@@ -64,9 +69,18 @@ inline int grid_for(int64_t vecs, int sm_count) {
 
 int launch_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                   int32_t start_pos, cudaStream_t stream) {
-    append_kernel<<<grid_for(int64_t(n_tokens) * kVecPerToken, ctx->sm_count), 256, 0, stream>>>(
-        reinterpret_cast<uint4*>(ctx->cfg.pool), reinterpret_cast<const uint4*>(latent),
-        reinterpret_cast<const uint4*>(k_rope), page_table, n_tokens, start_pos);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(unsigned(grid_for(int64_t(n_tokens) * kVecPerToken, ctx->sm_count)), 1, 1);
+    cfg.blockDim = dim3(256, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, append_kernel, reinterpret_cast<uint4*>(ctx->cfg.pool), reinterpret_cast<const uint4*>(latent),
+                                       reinterpret_cast<const uint4*>(k_rope), page_table, n_tokens, start_pos));
     KAIROS_CUDA_TRY(cudaGetLastError());
     return KAIROS_OK;
 }

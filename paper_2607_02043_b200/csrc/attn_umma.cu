@@ -652,6 +652,7 @@ __global__ void __launch_bounds__(kCombineThreads) combine_kernel(const CombineI
                                                       __nv_bfloat16* __restrict__ out_dec, __nv_bfloat16* __restrict__ out_chunk,
                                                       float* __restrict__ lse_dec, float* __restrict__ lse_chunk) {
     constexpr int kMaxK = 64;  // splits whose weights are staged in shared memory per pass
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the next step's append may pre-launch (it waits for this grid)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const CombineItem ci = items[blockIdx.x];
     const int kind = ci.kind_stride & 0xff, stride = ci.kind_stride >> 8;
