@@ -32,7 +32,11 @@
  * Asynchrony: kairos_append_latent and kairos_mixed_step enqueue on `cuda_stream` (a cudaStream_t cast to
  * void*; NULL = legacy default stream) and return without synchronising.  Host arrays (dec_ctx_lens) are
  * read before the call returns.  Calls on one context must be issued from one thread at a time and on
- * one stream at a time (the plan buffers are reused per call, ordered by that stream).
+ * one stream at a time (the plan buffers are reused per call, ordered by that stream).  Stream order is
+ * what the caller sees: a later operation on `cuda_stream` observes every output of an earlier call.  Inside
+ * that order the library overlaps its own work: the step's work list is copied on a stream of the context,
+ * and kernels are launched with programmatic stream serialisation (a grid may become resident while its
+ * predecessor drains, and waits for it on the device before touching anything the predecessor may still use).
  *
  * Errors: every call returns 0 (KAIROS_OK) or a negative kairos_status.  Argument errors are detected on
  * the host before anything is enqueued.  Page ids are trusted (not range-checked on the device).
