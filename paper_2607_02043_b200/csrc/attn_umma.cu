@@ -82,6 +82,10 @@ __device__ __forceinline__ PageSlots page_slots(uint32_t g) {
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64
 constexpr uint32_t kColO = 128;  // O^T blocks at 128 + 64*b
+#ifndef KAIROS_S_AHEAD
+#define KAIROS_S_AHEAD 1
+#endif
+constexpr int kSAhead = KAIROS_S_AHEAD;  // pages the S MMAs may run ahead of the PV MMAs (S^T is double-buffered: <= 1)
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the max grows by more than 2^8
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
@@ -412,7 +416,7 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                 continue;
             }
         }
-        if (s_next < npages && s_next <= pv_next + 1) {
+        if (s_next < npages && s_next <= pv_next + kSAhead) {
             const uint32_t gg = g0 + s_next;
             const uint32_t st = gg & 1;
             if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[gg & (kPageRing - 1)], (gg / kPageRing) & 1))) {
