@@ -2,21 +2,27 @@
 """bench.py -- one JSON line per run for the mixed-step MLA attention path (BASELINE.json `metric`).
 
 A "step" = one pass of the whole hot path over one synthetic batch:
-kairos_append_latent(chunk) + kairos_mixed_step (host planner, persistent tcgen05 kernels, LSE combine).
-Workload at N=1: BASELINE.json configs[1] ("decode-node steady state": 64 lognormal decodes + one 512-token chunk),
-seeded synthetic inputs standing in for the paper's proprietary traces.  N>1: one replica per GPU
-(requests shard by sequence with no data-path collective: "replicas only"), value aggregated over ranks.
+kairos_append_latent(chunk) + kairos_mixed_step (host planner or cached plan, persistent tcgen05 kernels, LSE combine).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--chunk C] [--impl kairos|reference]
+Headline workload at N=1: BASELINE.json configs[4] ("long-context stress": 32 decodes at 32768 + a 4096-token chunk over
+a 28672-token prefix), the largest single-GPU configuration (BASELINE.json's `metric` names no config).  The same run
+also times every other gated workload -- configs[1], configs[2], all seven chunk sizes of configs[3] -- and reports them
+in `sweep` (step time, attention-kernel bracket, host enqueue time, fraction of the roofline against the BURST tensor
+peak).  Inputs are seeded synthetic stand-ins for the paper's proprietary traces.  N>1: one replica per
+GPU (requests shard by sequence with no data-path collective: "replicas only"), value aggregated over ranks.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--chunk C] [--no-sweep] [--impl kairos|reference]
   torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-Timing: W >= 3 warm-up steps, then exactly K steps bracketed by barrier + torch.cuda.synchronize, CUDA events on
-the launching stream, max over ranks.  Between steps the inputs rotate over R disjoint copies of the pool / queries
-so that the bytes touched between two uses of a copy exceed 2x the 126 MB L2 (stated in `config.l2`).
+Timing: W >= 3 warm-up steps, then exactly K steps bracketed by barrier + torch.cuda.synchronize, CUDA events on the
+launching stream, max over ranks.  L2: a workload whose step touches more than 2x the 126 MB L2 needs nothing; smaller
+ones rotate over R disjoint copies of the pool / queries so that more than 2x L2 is touched between two uses of a copy
+(stated per point in `l2`).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import sys
@@ -34,6 +40,8 @@ from paper_2607_02043_b200 import workloads as W  # noqa: E402
 L2_BYTES = 126 * 2 ** 20
 METRIC = "mixed_step_mla_attention_us"
 UNIT = "us/step"
+HEADLINE = (4, None)
+SWEEP = [(1, None), (2, None)] + [(3, c) for c in W.SWEEP_CHUNKS] + [(4, None)]
 
 
 def load_peaks():
@@ -47,13 +55,42 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
 
 
+def csrc_sha() -> str:
+    """Hash of the kernel sources: an ncu DRAM-traffic capture under profiles/ is only quoted for the sources it measured."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2607_02043_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(key: str):
+    """DRAM read+write bytes of one launch of the dominant kernel from the committed `ncu --set full` capture of exactly
+    this point (profiles/r02_traffic.csv: key,kernel,dram_bytes,csrc_sha), or (None, why)."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    if not os.path.exists(path):
+        return None, "no ncu capture committed for this point"
+    sha = csrc_sha()
+    with open(path) as f:
+        for line in f.read().splitlines()[1:]:
+            parts = line.split(",")
+            if len(parts) >= 4 and parts[0] == key:
+                if parts[3] != sha:
+                    return None, "capture predates the current kernel sources"
+                return int(parts[2]), parts[1]
+    return None, "no ncu capture committed for this point"
+
+
+def point_key(index: int, chunk) -> str:
+    return f"config{index}" + (f"_C{chunk}" if chunk is not None else "")
+
+
 def make_workload(index: int, chunk, seed_shift: int = 0):
     inp = W.make_config(index, chunk_len=chunk)
-    if seed_shift:  # other replicas: same shapes, different seed (independent batches)
-        kw = dict(q_scale=0.1)
-        if index == 1:
-            inp = W.make_inputs("steady_state", 1 + seed_shift, None, 512, 0, n_dec=64,
-                                lognormal=dict(median=1024, sigma=0.8, lo=64, hi=8192), **kw)
+    if seed_shift and index == 1:  # other replicas: same shapes, different seed (independent batches)
+        inp = W.make_inputs("steady_state", 1 + seed_shift, None, 512, 0, n_dec=64,
+                            lognormal=dict(median=1024, sigma=0.8, lo=64, hi=8192), q_scale=0.1)
     return inp
 
 
@@ -106,32 +143,65 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+# ---------------------------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(inp, budget_pairs: float = 6.0e6):
+    """A bounded sample of the workload for the oracle: every decode and every chunk row when the whole step fits the
+    budget, else evenly spaced decodes / chunk rows; returns (dec_idx, chunk_idx, pairs_in_sample, pairs_total, label)."""
+    L = inp.dec_ctx_lens.astype(np.int64)
+    C, P = inp.chunk_len, inp.prefix_len
+    dec_pairs, chunk_pairs = int(L.sum()), C * P + C * (C + 1) // 2
+    total = dec_pairs + chunk_pairs
+    if total <= budget_pairs:
+        return np.arange(inp.n_dec, dtype=np.int32), np.arange(C, dtype=np.int32), total, total, "every decode and chunk row"
+    fd = min(1.0, budget_pairs / 2 / max(dec_pairs, 1))
+    fc = min(1.0, budget_pairs / 2 / max(chunk_pairs, 1))
+    nd = max(1, int(round(inp.n_dec * fd))) if inp.n_dec else 0
+    nc = max(1, int(round(C * fc))) if C else 0
+    di = np.unique(np.linspace(0, inp.n_dec - 1, nd).astype(np.int32)) if nd else np.zeros(0, np.int32)
+    ci = np.unique(np.linspace(0, C - 1, nc).astype(np.int32)) if nc else np.zeros(0, np.int32)
+    pairs = int(L[di].sum()) + int((P + ci.astype(np.int64) + 1).sum())
+    return di, ci, pairs, total, (f"{len(di)} of {inp.n_dec} decodes and {len(ci)} of {C} chunk rows, evenly spaced; "
+                                  f"time scaled by (query, key) pairs {total}/{pairs}")
+
+
 def oracle_step_seconds(inp, reps: int):
-    """Times the oracle as it stands on the host cores for one full step (append + mixed step)."""
+    """Times the oracle as it stands on the host cores; returns (per-rep seconds scaled to the full step, threads, label)."""
     from oracle import oracle
+    di, ci, pairs, total, label = oracle_sample(inp)
+    full = pairs == total
     ts = []
+    pool = inp.pool.copy()
+    oracle.append(pool, inp.chunk_latent, inp.chunk_k_rope, inp.chunk_page_table, inp.prefix_len)
     for _ in range(reps):
-        pool = inp.pool.copy()
         t0 = time.perf_counter()
-        oracle.append(pool, inp.chunk_latent, inp.chunk_k_rope, inp.chunk_page_table, inp.prefix_len)
-        oracle.mixed_step(pool, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
-                          inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
-        ts.append(time.perf_counter() - t0)
-    return ts, oracle.num_threads()
+        if full:
+            oracle.append(pool, inp.chunk_latent, inp.chunk_k_rope, inp.chunk_page_table, inp.prefix_len)
+            oracle.mixed_step(pool, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
+                              inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+        else:
+            if len(di):
+                oracle.attend_rows(pool, inp.dec_page_tables, inp.dec_table_stride, di, inp.q_dec[di], inp.dec_ctx_lens[di],
+                                   inp.softmax_scale)
+            if len(ci):
+                oracle.attend_rows(pool, inp.chunk_page_table[None, :], inp.chunk_page_table.shape[0],
+                                   np.zeros(len(ci), np.int32), inp.q_chunk[ci], (inp.prefix_len + ci + 1).astype(np.int32),
+                                   inp.softmax_scale)
+        ts.append((time.perf_counter() - t0) * (total / pairs))
+    return ts, oracle.num_threads(), label
 
 
 def run_reference(args, rank: int):
-    """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
+    """--impl reference: the CPU oracle timed on the host cores (rank 0 only), on this arm's config / metric / unit."""
     if rank != 0:
         return
     inp = make_workload(args.config, args.chunk)
-    for _ in range(max(args.warmup, 0)):
-        oracle_step_seconds(inp, 1)
-    ts, cores = oracle_step_seconds(inp, args.steps)
+    steps = min(args.steps, 5)
+    oracle_step_seconds(inp, 1)
+    ts, cores, label = oracle_step_seconds(inp, steps)
     us = float(np.mean(ts)) * 1e6
-    sample = f"full {inp.name} step (append + every decode and chunk row), {args.steps} timed reps"
-    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+    sample = f"{inp.name}: {label}; {steps} timed reps"
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": 1, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_label(args.config, inp), "what": "CPU oracle (oracle/oracle_mla.c) on host cores"},
             "cpu_baseline": {"value": us, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -140,15 +210,110 @@ def run_reference(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------- the GPU arm
+class Point:
+    """One workload resident on the device (R rotating copies) with its timed regions."""
+
+    def __init__(self, index, chunk, rank_seed_shift, dev, K, torch):
+        self.index, self.chunk, self.K, self.torch, self.dev = index, chunk, K, torch, dev
+        inp = self.inp = make_workload(index, chunk, seed_shift=rank_seed_shift)
+        self.alg_bytes, self.alg_flops = inp.algorithmic_bytes(), inp.algorithmic_flops()
+        step_touch = inp.pool.nbytes + inp.q_dec.nbytes + inp.q_chunk.nbytes
+        if step_touch > 2 * L2_BYTES:
+            replicas = 1
+            self.l2 = f"one step touches {step_touch / 2**20:.0f} MiB > 2x L2: no flush needed"
+        else:
+            replicas = int(np.ceil(2.0 * L2_BYTES / max(step_touch, 1))) + 1
+            self.l2 = f"inputs rotate over {replicas} disjoint pool/query copies ({replicas * step_touch / 2**20:.0f} MiB > 2x L2)"
+        self.replicas = replicas
+
+        class Rep:
+            pass
+        self.reps = []
+        for _ in range(replicas):
+            R = Rep()
+            R.pool = K.bf16_tensor(inp.pool, dev)
+            R.ws = torch.empty(K.workspace_bytes(max(inp.n_dec, 1), max(inp.chunk_len, 1)), dtype=torch.uint8, device=dev)
+            R.ctx = K.Kairos(R.pool, R.ws, inp.softmax_scale)
+            R.q_dec = K.bf16_tensor(inp.q_dec, dev)
+            R.q_chunk = K.bf16_tensor(inp.q_chunk, dev)
+            R.dec_pt = torch.from_numpy(inp.dec_page_tables).to(dev)
+            R.chunk_pt = torch.from_numpy(inp.chunk_page_table).to(dev)
+            R.latent = K.bf16_tensor(inp.chunk_latent, dev)
+            R.k_rope = K.bf16_tensor(inp.chunk_k_rope, dev)
+            R.out_dec = torch.empty((inp.n_dec, 16, 512), dtype=torch.bfloat16, device=dev)
+            R.out_chunk = torch.empty((inp.chunk_len, 16, 512), dtype=torch.bfloat16, device=dev)
+            R.lse_dec = torch.empty((inp.n_dec, 16), dtype=torch.float32, device=dev)
+            R.lse_chunk = torch.empty((inp.chunk_len, 16), dtype=torch.float32, device=dev)
+            self.reps.append(R)
+        self.lens = inp.dec_ctx_lens
+
+    def step(self, R):
+        inp = self.inp
+        if inp.chunk_len:
+            R.ctx.append_latent(R.latent, R.k_rope, R.chunk_pt, inp.prefix_len)
+        R.ctx.mixed_step(R.q_dec, R.dec_pt, self.lens, R.q_chunk, R.chunk_pt, inp.chunk_len, inp.prefix_len,
+                         out_dec=R.out_dec, out_chunk=R.out_chunk, lse_dec=R.lse_dec, lse_chunk=R.lse_chunk)
+
+    def warm(self, n):
+        for i in range(max(n, 3) * self.replicas):  # every copy plans, hits its cache and captures its graph before timing
+            self.step(self.reps[i % self.replicas])
+        self.torch.cuda.synchronize()
+        self.info = self.reps[0].ctx.last_plan_info()
+
+    def timed(self, n_steps, barrier, profile=False):
+        """(device ms over n_steps, host seconds spent issuing them, summed attention-bracket us, brackets)."""
+        torch = self.torch
+        for R in self.reps:
+            R.ctx.profile_enable(profile)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        for i in range(n_steps):
+            self.step(self.reps[i % self.replicas])
+        e1.record()
+        host_s = time.perf_counter() - t0
+        barrier()
+        ms = e0.elapsed_time(e1)
+        k_us, k_n = 0.0, 0
+        if profile:
+            for R in self.reps:
+                us, n = R.ctx.profile_read()
+                k_us += us
+                k_n += n
+                R.ctx.profile_enable(False)
+        return ms, host_s, k_us, k_n
+
+    def close(self):
+        for R in self.reps:
+            R.ctx.close()
+        self.reps = []
+        self.torch.cuda.empty_cache()
+
+
+def roofline_entry(pt: Point, us_per_step: float, kern_us: float, peaks) -> dict:
+    t_hbm = pt.alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
+    t_tc_burst = pt.alg_flops / (peaks["bf16_tflops"] * 1e12) * 1e6
+    t_tc_sus = pt.alg_flops / (peaks["bf16_tflops_sustained"] * 1e12) * 1e6
+    bound = "hbm" if t_hbm >= t_tc_burst else "tensor"
+    roof = max(t_hbm, t_tc_burst)
+    return {"bound": bound, "roofline_us": roof, "roofline_us_sustained_tensor_peak": max(t_hbm, t_tc_sus),
+            "frac": roof / us_per_step, "frac_sustained": max(t_hbm, t_tc_sus) / us_per_step,
+            "kernel_frac": roof / kern_us if kern_us > 0 else None}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
-    ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: steady state)")
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=HEADLINE[0], help="BASELINE.json configs index of the headline workload")
     ap.add_argument("--chunk", type=int, default=None, help="chunk size for configs[3]")
     ap.add_argument("--impl", default="kairos", choices=["kairos", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="time the headline workload only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -157,8 +322,6 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
     if args.impl == "reference":
-        if args.steps > 50:
-            args.steps = 20  # bounded: each reference step is a full CPU pass over the workload
         run_reference(args, rank)
         return
 
@@ -174,101 +337,72 @@ def main():
     dev = torch.device("cuda", local_rank)
     peaks = load_peaks()
 
-    inp = make_workload(args.config, args.chunk, seed_shift=R_.replica_seed_shift(rank))
-    alg_bytes, alg_flops = inp.algorithmic_bytes(), inp.algorithmic_flops()
-    pool_bytes = inp.pool.nbytes
-    step_touch = pool_bytes + inp.q_dec.nbytes + inp.q_chunk.nbytes
-    replicas = max(2, int(np.ceil(2.0 * L2_BYTES / max(step_touch, 1))) + 1)
-    free_b, _ = torch.cuda.mem_get_info()
-    replicas = int(min(replicas, max(1, (free_b * 0.6) // max(step_touch * 1.3, 1))))
-
-    class Rep:
-        pass
-    reps = []
-    lens = inp.dec_ctx_lens
-    for r in range(replicas):
-        R = Rep()
-        R.pool = K.bf16_tensor(inp.pool, dev)
-        R.ws = torch.empty(K.workspace_bytes(max(inp.n_dec, 1), max(inp.chunk_len, 1)), dtype=torch.uint8, device=dev)
-        R.ctx = K.Kairos(R.pool, R.ws, inp.softmax_scale)
-        R.q_dec = K.bf16_tensor(inp.q_dec, dev)
-        R.q_chunk = K.bf16_tensor(inp.q_chunk, dev)
-        R.dec_pt = torch.from_numpy(inp.dec_page_tables).to(dev)
-        R.chunk_pt = torch.from_numpy(inp.chunk_page_table).to(dev)
-        R.latent = K.bf16_tensor(inp.chunk_latent, dev)
-        R.k_rope = K.bf16_tensor(inp.chunk_k_rope, dev)
-        R.out_dec = torch.empty((inp.n_dec, 16, 512), dtype=torch.bfloat16, device=dev)
-        R.out_chunk = torch.empty((inp.chunk_len, 16, 512), dtype=torch.bfloat16, device=dev)
-        R.lse_dec = torch.empty((inp.n_dec, 16), dtype=torch.float32, device=dev)
-        R.lse_chunk = torch.empty((inp.chunk_len, 16), dtype=torch.float32, device=dev)
-        reps.append(R)
-
-    def step(R):
-        if inp.chunk_len:
-            R.ctx.append_latent(R.latent, R.k_rope, R.chunk_pt, inp.prefix_len)
-        R.ctx.mixed_step(R.q_dec, R.dec_pt, lens, R.q_chunk, R.chunk_pt, inp.chunk_len, inp.prefix_len,
-                         out_dec=R.out_dec, out_chunk=R.out_chunk, lse_dec=R.lse_dec, lse_chunk=R.lse_chunk)
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed_region(n_steps: int, profile: bool):
-        for R in reps:
-            R.ctx.profile_enable(profile)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        e0.record()
-        for i in range(n_steps):
-            step(reps[i % replicas])
-        e1.record()
-        barrier()
-        ms = e0.elapsed_time(e1)
-        k_us, k_n = 0.0, 0
-        if profile:
-            for R in reps:
-                us, n = R.ctx.profile_read()
-                k_us += us
-                k_n += n
-                R.ctx.profile_enable(False)
-        return ms, k_us, k_n
-
-    # warm-up
-    for i in range(args.warmup):
-        step(reps[i % replicas])
-    barrier()
-    info = reps[0].ctx.last_plan_info()
-
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ms, _, _ = timed_region(args.steps, profile=False)
-    # roofline leg: the same K steps again with the main kernel bracketed by CUDA events on its stream
-    ms_prof, kern_us, kern_n = timed_region(args.steps, profile=True)
+
+    # ---- the other gated workloads (rank 0's own GPU, N = 1 only): same protocol, their own step counts
+    sweep = []
+    headline_key = point_key(args.config, args.chunk)
+    if world == 1 and not args.no_sweep:
+        for (ci, cc) in SWEEP:
+            if point_key(ci, cc) == headline_key:
+                continue
+            pt = Point(ci, cc, 0, dev, K, torch)
+            pt.warm(args.warmup)
+            n = max(args.steps, 30)
+            ms, host_s, _, _ = pt.timed(n, barrier)
+            _, _, k_us, k_n = pt.timed(n, barrier, profile=True)
+            us, kern = ms * 1e3 / n, k_us / max(k_n, 1)
+            e = {"workload": point_key(ci, cc), "B": pt.inp.n_dec, "C": pt.inp.chunk_len, "P": pt.inp.prefix_len,
+                 "step_us": us, "kernel_us": kern, "host_enqueue_us": host_s * 1e6 / n, "steps": n, "l2": pt.l2,
+                 "chunk_pairs": pt.info["chunk_pairs"], "dec_ctas_first": pt.info["dec_ctas_first"],
+                 "kernels_per_step": pt.info["kernels"] + (1 if pt.inp.chunk_len else 0), "graph": pt.info["graph"]}
+            e.update(roofline_entry(pt, us, kern, peaks))
+            sweep.append(e)
+            pt.close()
+            del pt
+
+    # ---- headline workload
+    pt = Point(args.config, args.chunk, R_.replica_seed_shift(rank), dev, K, torch)
+    inp = pt.inp
+    pt.warm(args.warmup)
+    info = pt.info
+    ms, host_s, _, _ = pt.timed(args.steps, barrier)
+    # roofline leg: the same K steps again with the attention kernels bracketed by CUDA events on their stream
+    ms_prof, _, kern_us, kern_n = pt.timed(args.steps, barrier, profile=True)
     clocks = sampler.stop()
 
     ms_max = R_.max_over_ranks(ms, dev)
     us_per_step = R_.whole_job_us_per_step(ms, args.steps, world, dev)  # world replicas advance one step per iteration
 
     # ---- end-to-end leg: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
-    R = reps[0]
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
-    h_qd, h_qc = pin(inp.q_dec), pin(inp.q_chunk)
-    h_dpt, h_cpt = pin(inp.dec_page_tables), pin(inp.chunk_page_table)
-    h_lat, h_rope = pin(inp.chunk_latent), pin(inp.chunk_k_rope)
-    h_od = torch.empty((inp.n_dec, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
-    h_oc = torch.empty((inp.chunk_len, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
-    e2e_steps = max(20, min(args.steps, 200))
-    for _ in range(3):
-        h2d, d2h = R.ctx.mixed_step_host(h_qd, h_dpt, lens, h_qc, h_lat, h_rope, h_cpt, inp.chunk_len, inp.prefix_len, h_od, h_oc)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(e2e_steps):
-        reps[i % replicas].ctx.mixed_step_host(h_qd, h_dpt, lens, h_qc, h_lat, h_rope, h_cpt, inp.chunk_len,
-                                               inp.prefix_len, h_od, h_oc)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_us = R_.max_over_ranks(e2e_s, dev) * 1e6 / (e2e_steps * world)
+    e2e = None
+    if not args.no_e2e:
+        R = pt.reps[0]
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        h_qd, h_qc = pin(inp.q_dec), pin(inp.q_chunk)
+        h_dpt, h_cpt = pin(inp.dec_page_tables), pin(inp.chunk_page_table)
+        h_lat, h_rope = pin(inp.chunk_latent), pin(inp.chunk_k_rope)
+        h_od = torch.empty((inp.n_dec, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+        h_oc = torch.empty((inp.chunk_len, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+        e2e_steps = max(10, min(args.steps, 100))
+        for _ in range(3):
+            h2d, d2h = R.ctx.mixed_step_host(h_qd, h_dpt, pt.lens, h_qc, h_lat, h_rope, h_cpt, inp.chunk_len, inp.prefix_len, h_od, h_oc)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(e2e_steps):
+            pt.reps[i % pt.replicas].ctx.mixed_step_host(h_qd, h_dpt, pt.lens, h_qc, h_lat, h_rope, h_cpt, inp.chunk_len,
+                                                         inp.prefix_len, h_od, h_oc)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        e2e_us = R_.max_over_ranks(e2e_s, dev) * 1e6 / (e2e_steps * world)
+        e2e = {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "api": "kairos_mixed_step_host (pinned host buffers, synchronous)", "steps": e2e_steps}
 
     if rank != 0:
         if world > 1:
@@ -277,63 +411,58 @@ def main():
 
     # ---- roofline of the attention kernels of the step (kairos_mixed_kernel, plus the concurrent kairos_chunk_pair_kernel
     # when the planner moves the chunk onto SM pairs): algorithmic bytes / flops per step over the live CUDA-event
-    # duration of that bracket inside the second timed region
+    # duration of that bracket inside the second timed region.  Tensor peak = the BURST cuBLAS figure of MEASURED_PEAKS.json
+    # (a step lasts milliseconds at full clocks); the fraction against the sustained figure is reported beside it.
     kern_avg_us = kern_us / max(kern_n, 1)
-    t_hbm_us = alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
-    # the kernels are timed inside the long step loop, so the tensor peak is the SUSTAINED cuBLAS figure of MEASURED_PEAKS.json
-    # (the burst figure is for a kernel timed alone); the burst fraction is reported beside it
-    tc_peak = peaks["bf16_tflops_sustained"]
-    t_tc_us = alg_flops / (tc_peak * 1e12) * 1e6
-    bound = "hbm" if t_hbm_us >= t_tc_us else "tensor"
-    traffic = None  # DRAM bytes of one launch of the dominant kernel from the committed ncu capture of this configuration
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if os.path.exists(tpath):
-        key = f"config{args.config}" + (f"_C{args.chunk}" if args.chunk is not None else "")
-        with open(tpath) as f:
-            for line in f.read().splitlines()[1:]:
-                k, _, v = line.split(",")
-                if k == key:
-                    traffic = int(v)
-    if bound == "hbm":
-        achieved = alg_bytes / (kern_avg_us * 1e-6) / 1e9
-        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic}
+    own_us = ms_max * 1e3 / args.steps
+    re = roofline_entry(pt, own_us, kern_avg_us, peaks)
+    traffic, traffic_note = measured_traffic(headline_key)
+    if re["bound"] == "hbm":
+        achieved = pt.alg_bytes / (kern_avg_us * 1e-6) / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"]}
     else:
-        achieved = alg_flops / (kern_avg_us * 1e-6) / 1e12
-        roof = {"bound": "tensor", "achieved": achieved, "peak": tc_peak, "unit": "TFLOP/s",
-                "frac": achieved / tc_peak, "traffic": traffic, "peak_kind": "sustained (kernel timed inside the step loop)",
-                "peak_burst": peaks["bf16_tflops"], "frac_of_burst": achieved / peaks["bf16_tflops"]}
+        achieved = pt.alg_flops / (kern_avg_us * 1e-6) / 1e12
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": achieved / peaks["bf16_tflops"], "peak_kind": "burst",
+                "peak_sustained": peaks["bf16_tflops_sustained"], "frac_sustained": achieved / peaks["bf16_tflops_sustained"]}
     kname = ("kairos_chunk_pair_kernel (chunk, %d 2-CTA clusters) + kairos_mixed_kernel (decode splits), concurrent grids"
              % info["chunk_pairs"]) if info.get("chunk_pairs", 0) > 0 else "kairos_mixed_kernel"
-    roof.update({"kernel": kname, "kernel_us": kern_avg_us, "launches_timed": kern_n,
-                 "peak_source": peaks["source"], "algorithmic_bytes": alg_bytes, "algorithmic_flops": alg_flops,
-                 "step_roofline_us": max(t_hbm_us, t_tc_us),
-                 "step_frac_of_roofline": max(t_hbm_us, t_tc_us) / (ms_max * 1e3 / args.steps),
+    roof.update({"traffic": traffic, "traffic_note": traffic_note, "kernel": kname, "kernel_us": kern_avg_us,
+                 "launches_timed": kern_n, "peak_source": peaks["source"], "algorithmic_bytes": pt.alg_bytes,
+                 "algorithmic_flops": pt.alg_flops, "step_roofline_us": re["roofline_us"], "step_frac_of_roofline": re["frac"],
+                 "step_frac_of_roofline_sustained_tensor_peak": re["frac_sustained"],
                  "us_per_step_with_kernel_events": ms_prof * 1e3 / args.steps})
+    head = {"workload": headline_key, "B": inp.n_dec, "C": inp.chunk_len, "P": inp.prefix_len, "step_us": own_us,
+            "kernel_us": kern_avg_us, "host_enqueue_us": host_s * 1e6 / args.steps, "steps": args.steps, "l2": pt.l2,
+            "chunk_pairs": info["chunk_pairs"], "dec_ctas_first": info["dec_ctas_first"],
+            "kernels_per_step": info["kernels"] + (1 if inp.chunk_len else 0), "graph": info["graph"]}
+    head.update(re)
+    order = {point_key(ci, cc): i for i, (ci, cc) in enumerate(SWEEP)}
+    sweep = sorted(sweep + [head], key=lambda e: order.get(e["workload"], 99))
 
     cpu = None
     if not args.no_cpu_baseline:
-        n_rep = 3 if args.config <= 1 else 1
-        ts, cores = oracle_step_seconds(inp, n_rep)
+        ts, cores, label = oracle_step_seconds(inp, 1)
         cpu = {"value": float(np.median(ts)) * 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"full {inp.name} step (append + every decode and chunk row), median of {n_rep}"}
+               "sample": f"{inp.name}: {label}"}
 
     line = {
         "metric": METRIC, "value": us_per_step, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_max / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": workload_label(args.config, inp), "parallelism": f"replicas x{world} (no collective)",
-                   "l2": f"inputs rotate over {replicas} disjoint pool/query copies ({replicas * step_touch / 2**20:.0f} MiB > 2x L2)",
-                   "step": "kairos_append_latent(chunk) + kairos_mixed_step (planner H2D + persistent attention kernel(s) + combine)",
+                   "l2": pt.l2,
+                   "step": "kairos_append_latent(chunk) + kairos_mixed_step (cached plan replayed as a CUDA graph: attention grid(s) + combine)",
                    "plan": info, "library": K.version()},
         "clocks": clocks,
-        "e2e": {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "api": "kairos_mixed_step_host (pinned host buffers, synchronous)", "steps": e2e_steps},
+        "host_enqueue_us": host_s * 1e6 / args.steps,
+        "e2e": e2e,
         "gpu_launches": int(args.steps * ((1 if inp.chunk_len else 0) + info["kernels"])),
         "roofline": roof,
         "cpu_baseline": cpu,
-        "achieved": {"algorithmic_GBps": alg_bytes / (us_per_step * world * 1e-6) / 1e9,
-                     "algorithmic_TFLOPs": alg_flops / (us_per_step * world * 1e-6) / 1e12},
+        "achieved": {"algorithmic_GBps": pt.alg_bytes / (us_per_step * world * 1e-6) / 1e9,
+                     "algorithmic_TFLOPs": pt.alg_flops / (us_per_step * world * 1e-6) / 1e12},
+        "sweep": sweep,
     }
     print(json.dumps(line), flush=True)
     if world > 1:

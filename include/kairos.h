@@ -23,23 +23,34 @@
  *              512 latent values then 64 RoPE-key values.  Must be 128-byte aligned.
  *   page table int32, entry b = physical page of tokens 64b .. 64b+63 of that sequence.
  *   q          bf16 [n][16][576], row = [latent part 512 | rope part 64], 16-byte aligned.
- *   out        bf16 [n][16][512]; lse fp32 [n][16].
+ *   out        bf16 [n][16][512], 16-byte aligned; lse fp32 [n][16].
+ * Precondition on the pool: slots at positions >= the attended length never influence a result, whatever FINITE
+ * or NON-FINITE bit pattern they hold (the kernels zero the invisible rows of a boundary page in shared memory
+ * before the PV product, so a NaN/Inf left by an allocator cannot reach an output through 0 * NaN).  Visible
+ * slots must hold finite values.
  *
  * Ownership: the caller owns every buffer it passes (pool, workspace, q, out, page tables) and the CUDA
  * stream; the context owns only its descriptors, a small pinned staging area and its plan buffers.  No
  * pointer is retained past the call that received it, except `pool` / `workspace` given at create time.
  *
  * Asynchrony: kairos_append_latent and kairos_mixed_step enqueue on `cuda_stream` (a cudaStream_t cast to
- * void*; NULL = legacy default stream) and return without synchronising.  Host arrays (dec_ctx_lens) are
- * read before the call returns.  Calls on one context must be issued from one thread at a time and on
+ * void*; NULL = legacy default stream) and return without synchronising.  The stream must not be in capture
+ * mode (the library replays its own CUDA graphs, see below; kairos_run_schedule builds one for a whole chunk
+ * schedule).  Host arrays (dec_ctx_lens) are read before the call returns.  Calls on one context must be issued from one thread at a time and on
  * one stream at a time (the plan buffers are reused per call, ordered by that stream).  Stream order is
  * what the caller sees: a later operation on `cuda_stream` observes every output of an earlier call.  Inside
  * that order the library overlaps its own work: the step's work list is copied on a stream of the context,
  * and kernels are launched with programmatic stream serialisation (a grid may become resident while its
  * predecessor drains, and waits for it on the device before touching anything the predecessor may still use).
  *
- * Errors: every call returns 0 (KAIROS_OK) or a negative kairos_status.  Argument errors are detected on
- * the host before anything is enqueued.  Page ids are trusted (not range-checked on the device).
+ * Plan reuse: the context keeps the last few host plans (a0) with their device copies.  A step whose
+ * (n_dec, dec_ctx_lens, chunk_len, prefix_len) match a kept plan skips the planner and the host->device copy; when
+ * it also passes the same buffers as the previous use of that plan, its kernels are replayed as one CUDA graph
+ * (programmatic launch edges kept).  A step that only moved lengths inside the requests' last pages re-uses the
+ * plan's structure (lengths patched, one small copy).  Results never depend on which path was taken.
+ *
+ * Errors: every call returns 0 (KAIROS_OK) or a negative kairos_status.  Argument errors (NULL pointers, sizes,
+ * lengths, misaligned q / out / lse pointers) are detected on the host before anything is enqueued.  Page ids are trusted (not range-checked on the device).
  * kairos_last_error gives a human-readable message for the last failure on this thread.
  * There is no CPU fallback anywhere: without a CUDA device every compute entry returns KAIROS_ERR_CUDA.
  */
@@ -154,8 +165,12 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
  * deployment-time profiling of PAPER.md:302-304 for this one layer's attention, the input of Eq. 4-6
  * (PAPER.md:253-269).  For every (B, K, C): synthetic page tables over the context's pool (B*ceil(K/64) +
  * ceil((prefix_len+C)/64) distinct pages, strided through the pool), `warmup` untimed steps, then `reps`
- * timed steps (CUDA events around kairos_mixed_step on `cuda_stream`; when flush_l2 != 0 a buffer larger
- * than L2 is rewritten before every timed step, outside the timed interval).  Synchronising call.
+ * timed steps (one CUDA event pair per rep around kairos_mixed_step on `cuda_stream`; when flush_l2 != 0 a buffer
+ * larger than L2 is rewritten before every step, outside the timed interval).  The reps of a point are enqueued back
+ * to back and read after one synchronisation, so with warmup >= 2 an interval is the DEVICE time of the step (the
+ * cached plan's graph is already queued when the start event fires); warmup < 2 puts the planner and the plan copy
+ * of the first use inside the first interval.  The chunk's tokens are not appended (timing only: the pool's bytes
+ * are read as they are).  Scratch buffers belong to the context and are allocated on first use.  Synchronising call.
  *   Bs, Ks, Cs         HOST int32 arrays (B >= 0, K >= 1, C >= 0; B == 0 and C == 0 together give 0 us)
  *   out_median_us      HOST double [nB*nK*nC], index (iB*nK + iK)*nC + iC
  *   out_min_us         HOST double [nB*nK*nC] or NULL
@@ -192,7 +207,9 @@ int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_l
 /* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
  * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched
  * by that call, [5] = workspace bytes used, [6] = 2-CTA clusters the chunk ran on (0 = the chunk ran as tiles of the
- * decode grid's queue).  n = number of int64 slots available in info (at most 7 are written). */
+ * decode grid's queue), [7] = plan cache (0 planned, 1 structure re-used with patched lengths, 2 exact hit),
+ * [8] = 1 if the kernels were replayed as a CUDA graph, [9] = CTAs of the decode grid when it is launched before the
+ * clusters (0 otherwise).  n = number of int64 slots available in info (at most 10 are written). */
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
 
 /*
@@ -204,7 +221,20 @@ int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
 int kairos_profile_enable(kairos_ctx* ctx, int32_t on);
 int kairos_profile_read(kairos_ctx* ctx, double* main_kernel_us_total, int64_t* launches);
 
-/* Message for the last failing call on this thread ("" if none). Never NULL. */
+/*
+ * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
+ * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
+ *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;
+ *                 -(n + 1) n clusters first, the decode grid behind them (see kairos_plan_dump pair_mode)
+ *   "dec_only"    0 = never use the decode-only instantiation of the queue kernel; -1 default
+ *   "copy_stream" 0 = plan copies on the caller's stream; 1 default (the context's copy stream)
+ *   "graph"       0 = never replay a plan as a CUDA graph; 1 default
+ *   "plan_cache"  0 = plan every step; 1 default
+ * Errors: INVALID_ARG for an unknown key.
+ */
+int kairos_debug_set(kairos_ctx* ctx, const char* key, int32_t value);
+
+/* Message for the last failing call on this thread ("" if none; thread-local, so no context argument). Never NULL. */
 const char* kairos_last_error(void);
 
 /* Library build tag, e.g. "kairos-b200 sm_100a <kernel generation>". Never NULL. */

@@ -27,41 +27,152 @@ constexpr size_t kCounterBytes = 256;
 
 static size_t max_partial_slots(int32_t max_decodes) { return size_t(std::max(0, max_decodes)) + 12 * size_t(kMaxCtas); }
 
-int staging_acquire(kairos_ctx* ctx, size_t bytes, StagingSlot** out) {
-    StagingSlot& s = ctx->staging[ctx->staging_next];
-    ctx->staging_next = (ctx->staging_next + 1) % kairos_ctx::kStagingSlots;
-    if (s.used) KAIROS_CUDA_TRY(cudaEventSynchronize(s.done));  // its last H2D copy has left the pinned buffer
-    if (s.bytes < bytes) {
-        if (s.host) cudaFreeHost(s.host);
-        if (s.dev) cudaFree(s.dev);
-        s.host = s.dev = nullptr;
-        s.bytes = 0;
-        size_t cap = std::max<size_t>(bytes * 2, 64 * 1024);
-        KAIROS_CUDA_TRY(cudaMallocHost(&s.host, cap));
-        KAIROS_CUDA_TRY(cudaMalloc(&s.dev, cap));
-        s.bytes = cap;
-    }
-    if (!s.done) KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
-    s.used = true;
-    *out = &s;
-    return KAIROS_OK;
-}
-
 static int check_ctx(const kairos_ctx* ctx) {
     if (!ctx) return fail(KAIROS_ERR_INVALID_ARG, "ctx is NULL");
     return KAIROS_OK;
 }
 
-// Shared by kairos_mixed_step and the latency table: validate, plan, stage, launch.
-static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
-                           int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len,
-                           const void* q_chunk, const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec,
-                           void* out_chunk, float* lse_dec, float* lse_chunk, cudaStream_t stream) {
+static bool same_args(const StepArgs& a, const StepArgs& b) {
+    return a.n_dec == b.n_dec && a.q_dec == b.q_dec && a.dec_page_tables == b.dec_page_tables &&
+           a.dec_table_stride == b.dec_table_stride && a.chunk_len == b.chunk_len && a.prefix_len == b.prefix_len &&
+           a.q_chunk == b.q_chunk && a.chunk_page_table == b.chunk_page_table && a.out_dec == b.out_dec &&
+           a.out_chunk == b.out_chunk && a.lse_dec == b.lse_dec && a.lse_chunk == b.lse_chunk;
+}
+
+static void drop_graph(PlanBuffer& b) {
+    if (b.exec) cudaGraphExecDestroy(b.exec);
+    b.exec = nullptr;
+    b.same_args_uses = 0;
+}
+
+// Plan -> byte layout of its device copy: items | combines | pair items (256-byte aligned sections).
+static void layout_entry(PlanEntry& e) {
+    e.items_bytes = e.plan.items.size() * sizeof(WorkItem);
+    e.comb_bytes = e.plan.combines.size() * sizeof(CombineItem);
+    e.comb_off = (e.items_bytes + 255) / 256 * 256;
+    e.pair_bytes = e.plan.pair_items.size() * sizeof(WorkItem);
+    e.pair_off = (e.comb_off + e.comb_bytes + 255) / 256 * 256;
+    e.total_bytes = e.pair_off + e.pair_bytes;
+}
+
+// Copies the entry's plan into buffer `bi` and sends it to the device.  The copy runs on the context's copy stream so that it
+// overlaps whatever the caller's stream is still running (this step's append, the previous step's tail); the caller's stream
+// waits for it.  The buffer's previous contents may still be read by kernels of an earlier step (`last_use`) and its pinned
+// source by an earlier copy (`uploaded`): both are waited for, the first on the device, the second on the host (it completed
+// long ago unless the host runs several steps ahead of the GPU).
+static int upload_plan(kairos_ctx* ctx, PlanEntry& e, int bi, cudaStream_t stream) {
+    PlanBuffer& b = e.buf[bi];
+    const size_t need = e.total_bytes + 256;
+    if (b.ever_used && b.uploaded) KAIROS_CUDA_TRY(cudaEventSynchronize(b.uploaded));
+    if (b.cap < need) {
+        if (b.ever_used && b.last_use) KAIROS_CUDA_TRY(cudaEventSynchronize(b.last_use));  // rare: the buffer grows
+        drop_graph(b);  // it holds the old device pointer
+        if (b.host) cudaFreeHost(b.host);
+        if (b.dev) cudaFree(b.dev);
+        b.host = b.dev = nullptr;
+        b.cap = 0;
+        const size_t cap = std::max<size_t>(need * 2, 64 * 1024);
+        KAIROS_CUDA_TRY(cudaMallocHost(&b.host, cap));
+        KAIROS_CUDA_TRY(cudaMalloc(&b.dev, cap));
+        b.cap = cap;
+    }
+    if (!b.uploaded) KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&b.uploaded, cudaEventDisableTiming));
+    if (!b.last_use) KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&b.last_use, cudaEventDisableTiming));
+    uint8_t* h = static_cast<uint8_t*>(b.host);
+    std::memcpy(h, e.plan.items.data(), e.items_bytes);
+    if (e.comb_bytes) std::memcpy(h + e.comb_off, e.plan.combines.data(), e.comb_bytes);
+    if (e.pair_bytes) std::memcpy(h + e.pair_off, e.plan.pair_items.data(), e.pair_bytes);
+    cudaStream_t cs = (ctx->use_copy_stream && ctx->copy_stream) ? ctx->copy_stream : stream;
+    if (b.ever_used && cs != stream) KAIROS_CUDA_TRY(cudaStreamWaitEvent(cs, b.last_use, 0));
+    KAIROS_CUDA_TRY(cudaMemcpyAsync(b.dev, b.host, e.total_bytes, cudaMemcpyHostToDevice, cs));
+    KAIROS_CUDA_TRY(cudaEventRecord(b.uploaded, cs));
+    b.upload_pending = cs != stream;
+    b.ever_used = true;
+    return KAIROS_OK;
+}
+
+// The kernels of one step, in the order plan.cpp::choose_pairs decided, on `stream` (the caller's, or the capture stream).
+static int launch_step_kernels(kairos_ctx* ctx, const PlanEntry& e, const PlanBuffer& b, const StepArgs& a, cudaStream_t stream,
+                               cudaEvent_t e0, cudaEvent_t e1) {
+    const Plan& plan = e.plan;
+    const uint8_t* dev = static_cast<const uint8_t*>(b.dev);
+    const WorkItem* dev_items = reinterpret_cast<const WorkItem*>(dev);
+    const CombineItem* dev_comb = reinterpret_cast<const CombineItem*>(dev + e.comb_off);
+    const WorkItem* dev_pair = reinterpret_cast<const WorkItem*>(dev + e.pair_off);
+    const int n_items = int32_t(plan.items.size()), n_pair_items = int32_t(plan.pair_items.size());
+    const int n_pairs = plan.n_pairs;
+    const bool have_queue = n_items > 0;
+    // Roofline leg of bench.py: one pair of events around the attention kernels of the step (the decode grid and, when the
+    // planner uses it, the concurrent pair grid).
+    if (e0) KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
+    if (n_pairs > 0 && have_queue) {
+        // The two grids share the SMs in time (plan.cpp::choose_pairs).  dec_ctas > 0: the decode grid goes first, as 2-CTA
+        // clusters on dec_ctas SMs (whole TPCs), then one chunk cluster per SM pair -- those that do not fit yet start when
+        // the decode CTAs exit.  dec_ctas == 0: the clusters go first and the decode CTAs follow as SMs free up.  The second
+        // kernel is launched with programmatic stream serialisation and starts once every CTA of the first is resident (both
+        // trigger launch_dependents on entry), so the order in which the grids take SMs is the launch order.
+        if (plan.dec_ctas > 0) {
+            if (int rc = launch_attn_umma(ctx, plan, a, dev_items, n_items, stream, plan.dec_ctas, /*as_clusters=*/true, /*pdl=*/false)) return rc;
+            if (int rc = launch_attn_pair(ctx, a, dev_pair, n_pair_items, n_pairs, stream, /*pdl=*/true)) return rc;
+        } else {
+            if (int rc = launch_attn_pair(ctx, a, dev_pair, n_pair_items, n_pairs, stream, /*pdl=*/false)) return rc;
+            if (int rc = launch_attn_umma(ctx, plan, a, dev_items, n_items, stream, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/true)) return rc;
+        }
+    } else if (n_pairs > 0) {
+        if (int rc = launch_attn_pair(ctx, a, dev_pair, n_pair_items, n_pairs, stream, /*pdl=*/false)) return rc;
+    } else if (have_queue) {
+        if (int rc = launch_attn_umma(ctx, plan, a, dev_items, n_items, stream, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/false)) return rc;
+    }
+    if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
+    if (!plan.combines.empty())
+        if (int rc = launch_combine(ctx, a, dev_comb, int32_t(plan.combines.size()), stream)) return rc;
+    return KAIROS_OK;
+}
+
+static int kernels_of(const Plan& plan) {
+    return (plan.n_pairs > 0 ? 1 : 0) + (plan.items.empty() ? 0 : 1) + (plan.combines.empty() ? 0 : 1);
+}
+
+// Captures the step's launches (programmatic edges included) on the context's capture stream.  A failure is not an error of
+// the step: graphs are switched off for this context and the caller launches directly.
+static bool capture_graph(kairos_ctx* ctx, const PlanEntry& e, PlanBuffer& b, const StepArgs& a) {
+    drop_graph(b);
+    if (!ctx->capture_stream) return false;
+    if (cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->use_graph = 0;
+        return false;
+    }
+    const int rc = launch_step_kernels(ctx, e, b, a, ctx->capture_stream, nullptr, nullptr);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(ctx->capture_stream, &graph);
+    cudaGraphExec_t exec = nullptr;
+    bool ok = rc == KAIROS_OK && ce == cudaSuccess && graph != nullptr;
+    if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) {
+        cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        ctx->use_graph = 0;
+        return false;
+    }
+    b.exec = exec;
+    b.gargs = a;
+    return true;
+}
+
+int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                    int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len,
+                    const void* q_chunk, const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec,
+                    void* out_chunk, float* lse_dec, float* lse_chunk, cudaStream_t stream) {
     if (int rc = check_ctx(ctx)) return rc;
     if (n_dec < 0 || chunk_len < 0 || prefix_len < 0) return fail(KAIROS_ERR_INVALID_ARG, "negative size");
+    auto misaligned = [](const void* p, uintptr_t a) { return reinterpret_cast<uintptr_t>(p) % a != 0; };
     if (n_dec > 0) {
         if (!q_dec || !dec_page_tables || !dec_ctx_lens || !out_dec) return fail(KAIROS_ERR_INVALID_ARG, "NULL decode argument");
         if (dec_table_stride < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_table_stride < 1");
+        if (misaligned(q_dec, 16) || misaligned(out_dec, 16) || misaligned(lse_dec, 4) || misaligned(dec_page_tables, 4))
+            return fail(KAIROS_ERR_INVALID_ARG, "q_dec / out_dec must be 16-byte aligned (lse_dec, page tables: 4)");
         for (int32_t i = 0; i < n_dec; ++i) {
             if (dec_ctx_lens[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens[" + std::to_string(i) + "] < 1");
             if (int64_t(dec_ctx_lens[i]) > int64_t(dec_table_stride) * kPage)
@@ -72,138 +183,128 @@ static int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
         if (!q_chunk || !chunk_page_table || !out_chunk) return fail(KAIROS_ERR_INVALID_ARG, "NULL chunk argument");
         if (int64_t(prefix_len) + chunk_len > int64_t(chunk_table_len) * kPage)
             return fail(KAIROS_ERR_INVALID_ARG, "chunk page table shorter than prefix_len + chunk_len");
+        if (misaligned(q_chunk, 16) || misaligned(out_chunk, 16) || misaligned(lse_chunk, 4) || misaligned(chunk_page_table, 4))
+            return fail(KAIROS_ERR_INVALID_ARG, "q_chunk / out_chunk must be 16-byte aligned (lse_chunk, page table: 4)");
     }
     std::memset(ctx->last_info, 0, sizeof(ctx->last_info));
     if (n_dec == 0 && chunk_len == 0) return KAIROS_OK;
 
-    StepArgs a{n_dec, q_dec, dec_page_tables, dec_table_stride, chunk_len, prefix_len,
-               q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk};
+    const StepArgs a{n_dec, q_dec, dec_page_tables, dec_table_stride, chunk_len, prefix_len,
+                     q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk};
+    const int32_t target_ctas = umma_resident_ctas(ctx);
+    const int32_t pair_mode = ctx->force_pairs;
 
-    if (ctx->impl == 0) {
-        StagingSlot* st = nullptr;
-        if (int rc = staging_acquire(ctx, sizeof(int32_t) * size_t(std::max(n_dec, 1)), &st)) return rc;
-        if (n_dec > 0) {
-            std::memcpy(st->host, dec_ctx_lens, sizeof(int32_t) * size_t(n_dec));
-            KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, sizeof(int32_t) * size_t(n_dec), cudaMemcpyHostToDevice, stream));
-        }
-        KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
-        if (int rc = launch_attn_simple(ctx, a, reinterpret_cast<const int32_t*>(st->dev), stream)) return rc;
-        ctx->last_info[0] = n_dec + chunk_len;
-        ctx->last_info[3] = n_dec + chunk_len;
-        ctx->last_info[4] = 1;
-        return KAIROS_OK;
-    }
-
-    // ---- impl 1: plan -> staging -> persistent kernel (+ combine)
-    static const bool dbg = std::getenv("KAIROS_DEBUG_TIMING") != nullptr;
-    static double t_plan = 0, t_stage = 0, t_copy = 0, t_launch = 0; static long n_calls = 0;
-    auto now = [] { return std::chrono::steady_clock::now(); };
-    auto us = [](auto a, auto b) { return std::chrono::duration<double, std::micro>(b - a).count(); };
-    auto T0 = now();
-    Plan& plan = ctx->plan;
-    build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, umma_resident_ctas(ctx), umma_chunk_tile_tokens(), &plan,
-               ctx->force_pairs, pair_tile_tokens());
-    const size_t ws_needed = kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes;
-    if (ws_needed > ctx->cfg.workspace_bytes)
-        return fail(KAIROS_ERR_WORKSPACE, "workspace too small: need " + std::to_string(ws_needed) + " bytes");
-    const size_t items_bytes = plan.items.size() * sizeof(WorkItem);
-    const size_t comb_bytes = plan.combines.size() * sizeof(CombineItem);
-    const size_t comb_off = (items_bytes + 255) / 256 * 256;
-    const size_t pair_bytes = plan.pair_items.size() * sizeof(WorkItem);
-    const size_t pair_off = (comb_off + comb_bytes + 255) / 256 * 256;
-    StagingSlot* st = nullptr;
-    auto T1 = now();
-    if (int rc = staging_acquire(ctx, pair_off + pair_bytes + 256, &st)) return rc;
-    auto T2 = now();
-    std::memcpy(st->host, plan.items.data(), items_bytes);
-    if (comb_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + comb_off, plan.combines.data(), comb_bytes);
-    if (pair_bytes) std::memcpy(static_cast<uint8_t*>(st->host) + pair_off, plan.pair_items.data(), pair_bytes);
-    // The work list goes to the device on the library's copy stream, so that it overlaps whatever the caller's stream is
-    // still running (the append of this step, the previous step's tail); the caller's stream then waits for it.  The
-    // slot's device buffer is not overwritten before the kernels of its previous use have read it (`consumed`).
-    if (ctx->copy_stream) {
-        if (st->consumed) KAIROS_CUDA_TRY(cudaStreamWaitEvent(ctx->copy_stream, st->consumed, 0));
-        KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
-        KAIROS_CUDA_TRY(cudaEventRecord(st->done, ctx->copy_stream));
-        KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, st->done, 0));
-    } else {
-        KAIROS_CUDA_TRY(cudaMemcpyAsync(st->dev, st->host, pair_off + pair_bytes, cudaMemcpyHostToDevice, stream));
-        KAIROS_CUDA_TRY(cudaEventRecord(st->done, stream));
-    }
-    auto T3 = now();
-    int kernels = 0;
-    // Roofline leg of bench.py: one pair of events around the attention kernels of the step (the decode grid and, when
-    // the planner uses it, the concurrent pair grid; fork and join are inside the bracket).
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (ctx->profile) {
-        if (ctx->prof_used + 2 > ctx->prof_events.size()) {
-            for (int i = 0; i < 2; ++i) {
-                cudaEvent_t e;
-                KAIROS_CUDA_TRY(cudaEventCreate(&e));
-                ctx->prof_events.push_back(e);
+    // ---- a0: find the plan (exact hit: same lengths; structural hit: same page count per request), else build it
+    PlanEntry* hit = nullptr;
+    PlanEntry* structural = nullptr;
+    PlanEntry* victim = &ctx->plans[0];
+    if (ctx->use_plan_cache) {
+        for (PlanEntry& e : ctx->plans) {
+            if (!e.valid) { if (victim->valid) victim = &e; continue; }
+            if (victim->valid && e.stamp < victim->stamp) victim = &e;
+            if (e.n_dec != n_dec || e.chunk_len != chunk_len || e.prefix_len != prefix_len || e.target_ctas != target_ctas ||
+                e.pair_mode != pair_mode)
+                continue;
+            if (n_dec == 0 || std::memcmp(e.lens.data(), dec_ctx_lens, sizeof(int32_t) * size_t(n_dec)) == 0) { hit = &e; break; }
+            if (!structural) {
+                bool same = true;
+                for (int32_t i = 0; i < n_dec && same; ++i) same = (e.lens[i] + kPage - 1) / kPage == (dec_ctx_lens[i] + kPage - 1) / kPage;
+                if (same) structural = &e;
             }
         }
-        e0 = ctx->prof_events[ctx->prof_used];
-        e1 = ctx->prof_events[ctx->prof_used + 1];
-        ctx->prof_used += 2;
-        KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
     }
-    const WorkItem* dev_pair = reinterpret_cast<const WorkItem*>(static_cast<uint8_t*>(st->dev) + pair_off);
-    const int n_pairs = plan.n_pairs;
-    const bool have_queue = !plan.items.empty();
-    const WorkItem* dev_items = reinterpret_cast<const WorkItem*>(st->dev);
-    const CombineItem* dev_comb = reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off);
-    if (n_pairs > 0 && have_queue) {
-        // The two grids share the SMs in time (plan.cpp::choose_pairs).  dec_ctas > 0: the decode grid goes first, as 2-CTA
-        // clusters on dec_ctas SMs (whole TPCs), then one chunk cluster per SM pair -- those that do not fit yet start when
-        // the decode CTAs exit.  dec_ctas == 0: the clusters take every SM pair and the decode CTAs follow as SMs free up.
-        // Both kernels go to the caller's stream; the second one is launched with programmatic stream serialisation and
-        // starts once every CTA of the first is resident (both trigger launch_dependents on entry), so the order in
-        // which the grids take SMs is the launch order.
-        if (plan.dec_ctas > 0) {
-            if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
-                                          &kernels, plan.dec_ctas, /*as_clusters=*/true, /*pdl=*/false))
-                return rc;
-            if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/true)) return rc;
+    int cache_state = 0;  // 0 miss, 1 structural hit, 2 exact hit
+    PlanEntry* e = hit;
+    if (hit) {
+        cache_state = 2;
+    } else if (structural) {
+        // only n_keys of the decode items moves with the lengths (plan.cpp never looks below page granularity)
+        e = structural;
+        cache_state = 1;
+        e->lens.assign(dec_ctx_lens, dec_ctx_lens + n_dec);
+        for (WorkItem& w : e->plan.items)
+            if (w.kind == 0) w.n_keys = dec_ctx_lens[w.q_index];
+        e->cur ^= 1;
+        if (int rc = upload_plan(ctx, *e, e->cur, stream)) return rc;
+    } else {
+        e = victim;
+        for (PlanBuffer& b : e->buf) drop_graph(b);
+        e->valid = false;
+        build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, target_ctas, umma_chunk_tile_tokens(), &e->plan, pair_mode, pair_tile_tokens());
+        const size_t ws_needed = kCounterBytes + size_t(e->plan.n_partial_slots) * kPartialSlotBytes;
+        if (ws_needed > ctx->cfg.workspace_bytes)
+            return fail(KAIROS_ERR_WORKSPACE, "workspace too small: need " + std::to_string(ws_needed) + " bytes");
+        e->n_dec = n_dec; e->chunk_len = chunk_len; e->prefix_len = prefix_len; e->target_ctas = target_ctas; e->pair_mode = pair_mode;
+        e->lens.assign(dec_ctx_lens, dec_ctx_lens + n_dec);
+        layout_entry(*e);
+        e->cur = 0;
+        if (int rc = upload_plan(ctx, *e, 0, stream)) return rc;
+        e->valid = true;
+    }
+    e->stamp = ++ctx->plan_clock;
+    PlanBuffer& b = e->buf[e->cur];
+    const Plan& plan = e->plan;
+
+    // ---- q tensor maps (kept while the caller passes the same buffers); everything that can fail on the host happens
+    // before the first enqueue on the caller's stream
+    if (n_dec > 0 && !plan.items.empty())
+        if (int rc = encode_q_map(&ctx->qd_map, q_dec, uint64_t(n_dec) * kHeads, 16)) return rc;
+    if (chunk_len > 0 && plan.n_chunk_items > 0)
+        if (int rc = encode_q_map(&ctx->qc_map, q_chunk, uint64_t(chunk_len) * kHeads, 64)) return rc;
+    if (chunk_len > 0 && plan.n_pairs > 0)
+        if (int rc = encode_q_map(&ctx->qp_map, q_chunk, uint64_t(chunk_len) * kHeads, 128)) return rc;
+
+    if (b.upload_pending) {
+        KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, b.uploaded, 0));
+        if (cache_state == 2 && cudaEventQuery(b.uploaded) == cudaSuccess) b.upload_pending = false;
+    }
+
+    // ---- launch: a plan used again with the same buffers is replayed as a CUDA graph (one cudaGraphLaunch instead of 2-3
+    // launches with their attributes); kairos_profile_enable forces direct launches because it brackets them with events
+    bool graphed = false;
+    if (ctx->use_graph && !ctx->profile) {
+        if (b.exec && same_args(b.gargs, a)) {
+            graphed = true;
         } else {
-            if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/false)) return rc;
-            if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
-                                          &kernels, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/true))
-                return rc;
+            if (b.same_args_uses > 0 && same_args(b.gargs, a)) {
+                if (++b.same_args_uses >= 2) graphed = capture_graph(ctx, *e, b, a);
+            } else {
+                drop_graph(b);
+                b.gargs = a;
+                b.same_args_uses = 1;
+            }
         }
-    } else if (n_pairs > 0) {
-        if (int rc = launch_attn_pair(ctx, a, dev_pair, int32_t(plan.pair_items.size()), n_pairs, stream, /*pdl=*/false)) return rc;
-    } else if (have_queue) {
-        if (int rc = launch_attn_umma(ctx, a, dev_items, int32_t(plan.items.size()), dev_comb, int32_t(plan.combines.size()), stream,
-                                      &kernels, umma_resident_ctas(ctx), /*as_clusters=*/false, /*pdl=*/false))
-            return rc;
     }
-    if (n_pairs > 0) ++kernels;
-    if (e1) KAIROS_CUDA_TRY(cudaEventRecord(e1, stream));
-    if (!plan.combines.empty()) {
-        if (int rc = launch_combine(ctx, a, reinterpret_cast<const CombineItem*>(static_cast<uint8_t*>(st->dev) + comb_off),
-                                    int32_t(plan.combines.size()), stream))
-            return rc;
-        ++kernels;
+    if (graphed) {
+        KAIROS_CUDA_TRY(cudaGraphLaunch(b.exec, stream));
+    } else {
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (ctx->profile) {
+            if (ctx->prof_used + 2 > ctx->prof_events.size()) {
+                for (int i = 0; i < 2; ++i) {
+                    cudaEvent_t ev;
+                    KAIROS_CUDA_TRY(cudaEventCreate(&ev));
+                    ctx->prof_events.push_back(ev);
+                }
+            }
+            e0 = ctx->prof_events[ctx->prof_used];
+            e1 = ctx->prof_events[ctx->prof_used + 1];
+            ctx->prof_used += 2;
+        }
+        if (int rc = launch_step_kernels(ctx, *e, b, a, stream, e0, e1)) return rc;
     }
-    if (ctx->copy_stream) {
-        if (!st->consumed) KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&st->consumed, cudaEventDisableTiming));
-        KAIROS_CUDA_TRY(cudaEventRecord(st->consumed, stream));
-    }
-    if (dbg) {
-        auto T4 = now();
-        t_plan += us(T0, T1); t_stage += us(T1, T2); t_copy += us(T2, T3); t_launch += us(T3, T4);
-        if (++n_calls % 500 == 0)
-            std::fprintf(stderr, "[kairos host us/call] plan %.1f staging_wait %.1f copy+record %.1f encode+launch %.1f\n",
-                         t_plan / n_calls, t_stage / n_calls, t_copy / n_calls, t_launch / n_calls);
-    }
+    KAIROS_CUDA_TRY(cudaEventRecord(b.last_use, stream));
+
     ctx->last_info[0] = int64_t(plan.items.size());
     ctx->last_info[1] = plan.n_decode_items;
     ctx->last_info[2] = plan.n_chunk_items + int64_t(plan.pair_items.size());
     ctx->last_info[3] = std::min<int64_t>(plan.n_pairs > 0 && plan.dec_ctas > 0 ? plan.dec_ctas : umma_resident_ctas(ctx), int64_t(plan.items.size()));
-    ctx->last_info[4] = kernels;
-    ctx->last_info[5] = int64_t(ws_needed);
+    ctx->last_info[4] = kernels_of(plan);
+    ctx->last_info[5] = int64_t(kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes);
     ctx->last_info[6] = plan.n_pairs;
+    ctx->last_info[7] = cache_state;
+    ctx->last_info[8] = graphed ? 1 : 0;
+    ctx->last_info[9] = plan.dec_ctas;
     return KAIROS_OK;
 }
 
@@ -235,28 +336,23 @@ int kairos_create(const kairos_config* cfg, kairos_ctx** out) {
     cudaDeviceProp prop;
     KAIROS_CUDA_TRY(cudaGetDeviceProperties(&prop, cfg->device));
     if (prop.major != 10) return fail(KAIROS_ERR_UNSUPPORTED, "libkairos is built for sm_100a (B200) only");
+    if (cfg->workspace_bytes < kCounterBytes)
+        return fail(KAIROS_ERR_WORKSPACE, "workspace must hold at least 256 bytes (work-queue counters)");
     kairos_ctx* ctx = new (std::nothrow) kairos_ctx();
     if (!ctx) return fail(KAIROS_ERR_INVALID_ARG, "out of host memory");
     ctx->cfg = *cfg;
     ctx->sm_count = prop.multiProcessorCount;
-    const char* impl = std::getenv("KAIROS_IMPL");
-    ctx->impl = (impl && std::string(impl) == "simple") ? 0 : 1;
-    if (ctx->impl == 1) {
-        if (cfg->workspace_bytes < kCounterBytes) {
-            delete ctx;
-            return fail(KAIROS_ERR_WORKSPACE, "workspace must hold at least 256 bytes (work-queue counters)");
-        }
-        if (int rc = umma_init(ctx)) {
-            delete ctx;
-            return rc;
-        }
-        if (int rc = pair_init(ctx)) {
-            delete ctx;
-            return rc;
-        }
-        if (!std::getenv("KAIROS_NO_COPY_STREAM")) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
-        if (const char* fp = std::getenv("KAIROS_PAIRS")) ctx->force_pairs = std::atoi(fp);  // debug / sweeps: 0 = gen-1 chunk tiles only
-        if (const char* fd = std::getenv("KAIROS_DEC_ONLY")) ctx->force_dec_only = std::atoi(fd);
+    int rc = umma_init(ctx);
+    if (rc == KAIROS_OK) rc = pair_init(ctx);
+    if (rc == KAIROS_OK && cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess)
+        rc = fail(KAIROS_ERR_CUDA, "cudaStreamCreateWithFlags(copy stream) failed");
+    if (rc == KAIROS_OK && cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking) != cudaSuccess)
+        rc = fail(KAIROS_ERR_CUDA, "cudaStreamCreateWithFlags(capture stream) failed");
+    if (rc != KAIROS_OK) {
+        const std::string msg = g_last_error;
+        kairos_destroy(ctx);
+        g_last_error = msg;
+        return rc;
     }
     *out = ctx;
     return KAIROS_OK;
@@ -265,17 +361,36 @@ int kairos_create(const kairos_config* cfg, kairos_ctx** out) {
 int kairos_destroy(kairos_ctx* ctx) {
     if (!ctx) return KAIROS_OK;
     cudaSetDevice(ctx->cfg.device);
-    for (auto& s : ctx->staging) {
-        if (s.used && s.done) cudaEventSynchronize(s.done);
-        if (s.host) cudaFreeHost(s.host);
-        if (s.dev) cudaFree(s.dev);
-        if (s.done) cudaEventDestroy(s.done);
-        if (s.consumed) cudaEventDestroy(s.consumed);
-    }
+    for (PlanEntry& e : ctx->plans)
+        for (PlanBuffer& b : e.buf) {
+            if (b.ever_used && b.uploaded) cudaEventSynchronize(b.uploaded);
+            if (b.ever_used && b.last_use) cudaEventSynchronize(b.last_use);
+            if (b.exec) cudaGraphExecDestroy(b.exec);
+            if (b.host) cudaFreeHost(b.host);
+            if (b.dev) cudaFree(b.dev);
+            if (b.uploaded) cudaEventDestroy(b.uploaded);
+            if (b.last_use) cudaEventDestroy(b.last_use);
+        }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
+    if (ctx->table_buf) cudaFree(ctx->table_buf);
+    if (ctx->flush_buf) cudaFree(ctx->flush_buf);
     for (auto e : ctx->prof_events) cudaEventDestroy(e);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
     delete ctx;
+    return KAIROS_OK;
+}
+
+int kairos_debug_set(kairos_ctx* ctx, const char* key, int32_t value) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!key) return fail(KAIROS_ERR_INVALID_ARG, "key is NULL");
+    const std::string k(key);
+    if (k == "pairs") ctx->force_pairs = value;
+    else if (k == "dec_only") ctx->force_dec_only = value;
+    else if (k == "copy_stream") ctx->use_copy_stream = value != 0;
+    else if (k == "graph") ctx->use_graph = value != 0;
+    else if (k == "plan_cache") ctx->use_plan_cache = value != 0;
+    else return fail(KAIROS_ERR_INVALID_ARG, "unknown debug key '" + k + "'");
     return KAIROS_OK;
 }
 
@@ -426,7 +541,7 @@ int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_l
 
 int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n) {
     if (!ctx || !info || n < 0) return fail(KAIROS_ERR_INVALID_ARG, "NULL argument");
-    for (int32_t i = 0; i < n && i < 7; ++i) info[i] = ctx->last_info[i];
+    for (int32_t i = 0; i < n && i < 10; ++i) info[i] = ctx->last_info[i];
     return KAIROS_OK;
 }
 
@@ -453,7 +568,9 @@ int kairos_profile_read(kairos_ctx* ctx, double* main_kernel_us_total, int64_t* 
 
 const char* kairos_last_error(void) { return g_last_error.c_str(); }
 
-const char* kairos_version(void) { return "kairos-b200 sm_100a gen1 (tcgen05 swapped-operand split-KV + persistent work queue)"; }
+const char* kairos_version(void) {
+    return "kairos-b200 sm_100a r2 (tcgen05 split-KV decode grid + 2-CTA chunk clusters, time-shared persistent grids, cached plans replayed as CUDA graphs)";
+}
 
 }  // extern "C"
 
@@ -478,11 +595,6 @@ __global__ void flush_kernel(uint4* buf, size_t n, uint32_t v) {
         buf[i] = make_uint4(v, v, v, v);
 }
 
-struct DevBuf {
-    void* p = nullptr;
-    ~DevBuf() { if (p) cudaFree(p); }
-};
-
 }  // namespace
 }  // namespace kairos
 
@@ -496,79 +608,105 @@ extern "C" int kairos_step_latency_table(kairos_ctx* ctx, const int32_t* Bs, int
     for (int i = 0; i < nB; ++i) { if (Bs[i] < 0) return fail(KAIROS_ERR_INVALID_ARG, "B < 0"); maxB = std::max(maxB, Bs[i]); }
     for (int i = 0; i < nK; ++i) { if (Ks[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "K < 1"); maxK = std::max(maxK, Ks[i]); }
     for (int i = 0; i < nC; ++i) { if (Cs[i] < 0) return fail(KAIROS_ERR_INVALID_ARG, "C < 0"); maxC = std::max(maxC, Cs[i]); }
-    const int64_t max_dec_pages = int64_t(maxB) * ((maxK + kPage - 1) / kPage);
-    const int64_t max_chunk_pages = (int64_t(prefix_len) + maxC + kPage - 1) / kPage;
-    if (max_dec_pages + max_chunk_pages > ctx->cfg.num_pages)
+    // every point must fit the pool (the largest B and the largest K need not occur together)
+    int64_t need_pages = 0;
+    for (int iB = 0; iB < nB; ++iB)
+        for (int iK = 0; iK < nK; ++iK)
+            need_pages = std::max(need_pages, int64_t(Bs[iB]) * ((Ks[iK] + kPage - 1) / kPage));
+    const int64_t max_chunk_pages = maxC > 0 ? (int64_t(prefix_len) + maxC + kPage - 1) / kPage : 0;
+    if (need_pages + max_chunk_pages > ctx->cfg.num_pages)
         return fail(KAIROS_ERR_WORKSPACE, "pool has too few pages for the largest grid point: need " +
-                                              std::to_string(max_dec_pages + max_chunk_pages));
+                                              std::to_string(need_pages + max_chunk_pages));
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     KAIROS_CUDA_TRY(cudaSetDevice(ctx->cfg.device));
     const int32_t stride = std::max(1, (maxK + kPage - 1) / kPage);
-    DevBuf q_dec, q_chunk, o_dec, o_chunk, dpt, cpt, flush;
+    // one scratch allocation kept by the context (grown on demand): q_dec | q_chunk | out_dec | out_chunk | page tables
+    auto al = [](size_t x) { return (x + 255) / 256 * 256; };
     const size_t nqd = size_t(std::max(maxB, 1)) * kHeads * kDim, nqc = size_t(std::max(maxC, 1)) * kHeads * kDim;
-    KAIROS_CUDA_TRY(cudaMalloc(&q_dec.p, nqd * 2));
-    KAIROS_CUDA_TRY(cudaMalloc(&q_chunk.p, nqc * 2));
-    KAIROS_CUDA_TRY(cudaMalloc(&o_dec.p, size_t(std::max(maxB, 1)) * kHeads * kLatent * 2));
-    KAIROS_CUDA_TRY(cudaMalloc(&o_chunk.p, size_t(std::max(maxC, 1)) * kHeads * kLatent * 2));
-    KAIROS_CUDA_TRY(cudaMalloc(&dpt.p, size_t(std::max(maxB, 1)) * stride * 4));
-    KAIROS_CUDA_TRY(cudaMalloc(&cpt.p, size_t(std::max<int64_t>(max_chunk_pages, 1)) * 4));
+    const size_t b_qd = al(nqd * 2), b_qc = al(nqc * 2);
+    const size_t b_od = al(size_t(std::max(maxB, 1)) * kHeads * kLatent * 2), b_oc = al(size_t(std::max(maxC, 1)) * kHeads * kLatent * 2);
+    const size_t b_dpt = al(size_t(std::max(maxB, 1)) * stride * 4), b_cpt = al(size_t(std::max<int64_t>(max_chunk_pages, 1)) * 4);
+    const size_t total = b_qd + b_qc + b_od + b_oc + b_dpt + b_cpt;
+    if (ctx->table_bytes < total) {
+        KAIROS_CUDA_TRY(cudaStreamSynchronize(stream));
+        if (ctx->table_buf) cudaFree(ctx->table_buf);
+        ctx->table_buf = nullptr;
+        ctx->table_bytes = 0;
+        KAIROS_CUDA_TRY(cudaMalloc(&ctx->table_buf, total));
+        ctx->table_bytes = total;
+    }
     const size_t flush_bytes = size_t(256) << 20;  // > 126 MB L2
-    if (flush_l2) KAIROS_CUDA_TRY(cudaMalloc(&flush.p, flush_bytes));
-    fill_q_kernel<<<256, 256, 0, stream>>>(static_cast<uint16_t*>(q_dec.p), nqd, 0x1234u);
-    fill_q_kernel<<<256, 256, 0, stream>>>(static_cast<uint16_t*>(q_chunk.p), nqc, 0x9876u);
+    if (flush_l2 && !ctx->flush_buf) KAIROS_CUDA_TRY(cudaMalloc(&ctx->flush_buf, flush_bytes));
+    uint8_t* p = static_cast<uint8_t*>(ctx->table_buf);
+    uint16_t* q_dec = reinterpret_cast<uint16_t*>(p);    p += b_qd;
+    uint16_t* q_chunk = reinterpret_cast<uint16_t*>(p);  p += b_qc;
+    void* o_dec = p;                                     p += b_od;
+    void* o_chunk = p;                                   p += b_oc;
+    int32_t* dpt = reinterpret_cast<int32_t*>(p);        p += b_dpt;
+    int32_t* cpt = reinterpret_cast<int32_t*>(p);
+    fill_q_kernel<<<256, 256, 0, stream>>>(q_dec, nqd, 0x1234u);
+    fill_q_kernel<<<256, 256, 0, stream>>>(q_chunk, nqc, 0x9876u);
     KAIROS_CUDA_TRY(cudaGetLastError());
-    cudaEvent_t e0, e1;
-    KAIROS_CUDA_TRY(cudaEventCreate(&e0));
-    KAIROS_CUDA_TRY(cudaEventCreate(&e1));
+    // one event pair per timed rep: the reps of a point are enqueued back to back (the host runs ahead while the flush
+    // kernel or the previous step executes), so an interval is the device time of the step, not the host's enqueue time
+    struct Events {
+        std::vector<cudaEvent_t> ev;
+        ~Events() { for (auto e : ev) cudaEventDestroy(e); }
+    } events;
+    for (int i = 0; i < 2 * reps; ++i) {
+        cudaEvent_t e;
+        KAIROS_CUDA_TRY(cudaEventCreate(&e));
+        events.ev.push_back(e);
+    }
     std::vector<int32_t> h_dpt, h_cpt, lens;
     std::vector<double> times;
-    int rc = KAIROS_OK;
-    for (int iB = 0; iB < nB && rc == KAIROS_OK; ++iB)
-        for (int iK = 0; iK < nK && rc == KAIROS_OK; ++iK)
-            for (int iC = 0; iC < nC && rc == KAIROS_OK; ++iC) {
+    for (int iB = 0; iB < nB; ++iB)
+        for (int iK = 0; iK < nK; ++iK)
+            for (int iC = 0; iC < nC; ++iC) {
                 const int32_t B = Bs[iB], K = Ks[iK], C = Cs[iC];
                 const size_t o = (size_t(iB) * nK + iK) * nC + iC;
                 if (B == 0 && C == 0) { out_median_us[o] = 0.0; if (out_min_us) out_min_us[o] = 0.0; continue; }
-                // distinct pages, strided through the pool (an odd multiplicative step visits each page once)
+                // distinct pages, strided through the pool (a step coprime with num_pages visits each page once)
                 const int64_t kp = (K + kPage - 1) / kPage, cp = C > 0 ? (int64_t(prefix_len) + C + kPage - 1) / kPage : 0;
-                const int64_t need = int64_t(B) * kp + cp, np = ctx->cfg.num_pages;
+                const int64_t np = ctx->cfg.num_pages;
                 int64_t step = (np / 2) | 1;
                 while (std::gcd(step, np) != 1) step += 2;
                 auto page_of = [&](int64_t i) { return int32_t((i * step) % np); };
-                (void)need;
                 h_dpt.assign(size_t(std::max(B, 1)) * stride, 0);
                 for (int64_t b = 0; b < B; ++b)
-                    for (int64_t p = 0; p < kp; ++p) h_dpt[size_t(b) * stride + p] = page_of(b * kp + p);
+                    for (int64_t pg = 0; pg < kp; ++pg) h_dpt[size_t(b) * stride + pg] = page_of(b * kp + pg);
                 h_cpt.assign(size_t(std::max<int64_t>(cp, 1)), 0);
-                for (int64_t p = 0; p < cp; ++p) h_cpt[size_t(p)] = page_of(int64_t(B) * kp + p);
+                for (int64_t pg = 0; pg < cp; ++pg) h_cpt[size_t(pg)] = page_of(int64_t(B) * kp + pg);
                 lens.assign(size_t(std::max(B, 1)), K);
-                cudaMemcpyAsync(dpt.p, h_dpt.data(), h_dpt.size() * 4, cudaMemcpyHostToDevice, stream);
-                cudaMemcpyAsync(cpt.p, h_cpt.data(), h_cpt.size() * 4, cudaMemcpyHostToDevice, stream);
-                cudaStreamSynchronize(stream);
-                times.clear();
-                for (int it = 0; it < warmup + reps && rc == KAIROS_OK; ++it) {
-                    if (flush_l2) flush_kernel<<<1184, 256, 0, stream>>>(static_cast<uint4*>(flush.p), flush_bytes / 16, uint32_t(it));
-                    cudaEventRecord(e0, stream);
-                    rc = mixed_step_impl(ctx, B, q_dec.p, static_cast<int32_t*>(dpt.p), stride, lens.data(), C, prefix_len,
-                                         q_chunk.p, static_cast<int32_t*>(cpt.p), int32_t(std::max<int64_t>(cp, 1)), o_dec.p,
-                                         o_chunk.p, nullptr, nullptr, stream);
-                    cudaEventRecord(e1, stream);
-                    if (cudaEventSynchronize(e1) != cudaSuccess) rc = fail(KAIROS_ERR_CUDA, "latency table: step failed on the device");
-                    float ms = 0.f;
-                    cudaEventElapsedTime(&ms, e0, e1);
-                    if (it >= warmup) times.push_back(double(ms) * 1e3);
+                KAIROS_CUDA_TRY(cudaMemcpyAsync(dpt, h_dpt.data(), h_dpt.size() * 4, cudaMemcpyHostToDevice, stream));
+                KAIROS_CUDA_TRY(cudaMemcpyAsync(cpt, h_cpt.data(), h_cpt.size() * 4, cudaMemcpyHostToDevice, stream));
+                KAIROS_CUDA_TRY(cudaStreamSynchronize(stream));  // the pageable sources above are reused by the next point
+                for (int it = 0; it < warmup + reps; ++it) {
+                    if (flush_l2) {
+                        flush_kernel<<<1184, 256, 0, stream>>>(static_cast<uint4*>(ctx->flush_buf), flush_bytes / 16, uint32_t(it));
+                        KAIROS_CUDA_TRY(cudaGetLastError());
+                    }
+                    const int r = it - warmup;
+                    if (r >= 0) KAIROS_CUDA_TRY(cudaEventRecord(events.ev[2 * r], stream));
+                    if (int rc = mixed_step_impl(ctx, B, q_dec, dpt, stride, lens.data(), C, prefix_len, q_chunk, cpt,
+                                                 int32_t(std::max<int64_t>(cp, 1)), o_dec, o_chunk, nullptr, nullptr, stream))
+                        return rc;
+                    if (r >= 0) KAIROS_CUDA_TRY(cudaEventRecord(events.ev[2 * r + 1], stream));
                 }
-                if (rc != KAIROS_OK) break;
+                if (cudaStreamSynchronize(stream) != cudaSuccess) {
+                    const cudaError_t ce = cudaGetLastError();
+                    return fail(KAIROS_ERR_CUDA, std::string("latency table: step failed on the device: ") + cudaGetErrorString(ce));
+                }
+                times.clear();
+                for (int r = 0; r < reps; ++r) {
+                    float ms = 0.f;
+                    KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, events.ev[2 * r], events.ev[2 * r + 1]));
+                    times.push_back(double(ms) * 1e3);
+                }
                 std::sort(times.begin(), times.end());
                 const size_t n = times.size();
                 out_median_us[o] = n % 2 ? times[n / 2] : 0.5 * (times[n / 2 - 1] + times[n / 2]);
                 if (out_min_us) out_min_us[o] = times[0];
             }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (rc == KAIROS_OK) {
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return fail(KAIROS_ERR_CUDA, std::string("latency table: ") + cudaGetErrorString(e));
-    }
-    return rc;
+    return KAIROS_OK;
 }

@@ -79,14 +79,8 @@ struct PairSmall {
 };
 static_assert(sizeof(PairSmall) <= kPairSmallBytes, "PairSmall does not fit");
 
-#ifdef KAIROS_TRACE
-#define PTRACE(ev, g) do { if (blockIdx.x < 2 && (g) < 64) p.trace[(ev) * 64 + (g)] = clock64(); } while (0)
-#else
-#define PTRACE(ev, g) do { } while (0)
-#endif
 
 struct PairParams {
-    unsigned long long* trace;
     const WorkItem* items;
     int32_t n_items;
     int32_t* counter;      // queue head of the pair kernel
@@ -149,10 +143,8 @@ __device__ __forceinline__ void sc_load_q(PairSmall* sm, const WorkItem& w, cons
             tma_load_2d(qst + c * 16384, qmap, &sm->qst_full[c], c * 64, row0, kEvictFirst);
         }
     }
-    if (row == 0) PTRACE(10, it * 4 + 0);
     mbar_wait(&sm->q_free, (it & 1) ^ 1);  // previous item's S-MMAs have retired
     tc_fence_after();
-    if (row == 0) PTRACE(10, it * 4 + 1);
     {
         // Q tile [128 rows x 576] -> TMEM through two 16 KB staging buffers: one TMA box (64 dims x 128 rows, SWIZZLE_128B,
         // rows past the chunk's end zero-filled) per 64-dim chunk; each thread then reads its own row's 128 B (conflict
@@ -183,7 +175,6 @@ __device__ __forceinline__ void sc_load_q(PairSmall* sm, const WorkItem& w, cons
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->q_ready);
-    if (row == 0) PTRACE(10, it * 4 + 2);
 
 }
 
@@ -211,7 +202,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
         mbar_wait(&sm->s_full[b], ph);
-        if (row == 0) PTRACE(2, g);
         tc_fence_after();
         float x[64];
         tmem_ld32(tmem + lane_base + kColS2 + b * 64, reinterpret_cast<uint32_t*>(x));
@@ -220,7 +210,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->s_empty[b]);
-        if (row == 0) PTRACE(3, g);
 
         const int key0 = (w.page_begin + pg) * kPage;
         const bool boundary = key0 + kPage > w.n_keys;  // some row of the tile does not see every key of this page
@@ -254,9 +243,7 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
         }
         l += sum;
         // ---- P row (bf16, 128 B) -> O-CTA shared memory, K-major SWIZZLE_128B: row r at r*128, 16-B chunk c at c ^ (r & 7)
-        if (row == 0) PTRACE(4, g);
         mbar_wait_cluster(&sm->p_empty[b], ph ^ 1);
-        if (row == 0) PTRACE(5, g);
         // local staging (K-major SWIZZLE_128B: row r at r*128, 16-B chunk c at c ^ (r & 7)), then one 4 KB bulk copy per
         // warp into the O-CTA's P buffer, completing on its p_full mbarrier (DSMEM moves ~20 B/clk: asynchronous, so the
         // softmax threads do not wait for it)
@@ -286,7 +273,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
                            "r"(smem_u32(pstage + 2 * kPBytes + (b * 128 + q4 * 32) * 4)), "r"(128u), "r"(bar)
                          : "memory");
         }
-        if (row == 0) PTRACE(6, g);
     }
     // ---- end of item: 1 / l to the O-CTA's epilogue; lse from here
     mbar_wait_cluster(&sm->fin_empty, (it & 1) ^ 1);
@@ -304,7 +290,6 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
         }
     }
     if (tok < w.n_q && p.lse_chunk) p.lse_chunk[size_t(w.q_index + tok) * kHeads + head] = (m_ref + log2f(l)) * kLn2b;
-    if (row == 0) PTRACE(10, it * 4 + 3);
     // Every S-MMA of this item has retired (its last s_full was consumed above): Q may be replaced.  The next item's Q is
     // loaded only now, after the last P and 1/l have left, so that the ~7k-cycle load overlaps the O-CTA's last PV and its
     // epilogue (which otherwise stall the next item's first pages) instead of delaying them.
@@ -322,7 +307,6 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t st = g % kStagesK, sph = (g / kStagesK) & 1, b = g & 1, bph = (g >> 1) & 1;
         mbar_wait(&sm->s_empty[b], bph ^ 1);
-        PTRACE(0, g);
         const uint32_t kb_lo = smem_desc_lo(kv_base + st * kKStage, 16);
         mbar_wait(&ring->kv_full[st * kGroups], sph);
         tc_fence_after();
@@ -339,7 +323,6 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_
             umma_commit_elect(&ring->kv_empty[st * kGroups + gr]);
         }
         umma_commit_elect(&sm->s_full[b]);
-        PTRACE(1, g);
     }
     umma_commit_elect(&sm->q_free);
 }
@@ -347,12 +330,33 @@ __device__ __forceinline__ void sc_mma_item(PairSmall* sm, ScRing* ring, uint32_
 // ------------------------------------------------------------------------------------------------------------
 // O-CTA, correction + epilogue warps (128 threads, thread = query row = TMEM lane)
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint32_t peer_small, const WorkItem& w, const PairParams& p,
+__device__ __forceinline__ void oc_epilogue_item(PairSmall* sm, uint8_t* v_stages, uint32_t peer_small, const WorkItem& w, const PairParams& p,
                                                  uint32_t tmem, int row, int q4, int lane, uint32_t& g, uint32_t it) {
     const uint32_t lane_base = uint32_t(q4 * 32) << 16;
     const int npages = w.page_end - w.page_begin;
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t b = g & 1, ph = (g >> 1) & 1;
+        {
+            // Keys that no row of the tile sees (stale slots of the sequence's last page) have P = 0, but the PV MMA still
+            // multiplies their V rows, and 0 * NaN = NaN: zero those rows of the landed V stage (128 B per 64-dim chunk; the
+            // 128-byte swizzle permutes inside a row).  Thread = (token row & 63, half of the 8 chunks).
+            const int key0 = (w.page_begin + pg) * kPage, vis_max = w.n_keys + w.n_q - 1;
+            if (key0 + kPage > vis_max) {
+                const uint32_t st = g % kStages;
+                mbar_wait(&sm->v_full[st], (g / kStages) & 1);
+                const int t = row & 63;
+                if (key0 + t >= vis_max) {
+                    uint8_t* vst = v_stages + st * kVStage + t * 128;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        uint4* dst = reinterpret_cast<uint4*>(vst + ((row >> 6) * 4 + c) * 8192);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) dst[j] = make_uint4(0u, 0u, 0u, 0u);
+                    }
+                }
+                fence_proxy_async_smem();
+            }
+        }
         mbar_wait_cluster(&sm->p_full[b], ph);
         const float a = *reinterpret_cast<volatile float*>(&sm->alpha[b][row]);
         if (__any_sync(0xffffffffu, a != 1.f)) {  // warp-uniform: tcgen05.ld / st are warp-collective
@@ -447,10 +451,8 @@ __device__ __forceinline__ void oc_mma_item(PairSmall* sm, uint32_t peer_small, 
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const uint32_t st = g % kStages, sph = (g / kStages) & 1, b = g & 1, bph = (g >> 1) & 1;
         mbar_wait(&sm->corr_done[b], bph);
-        PTRACE(7, g);
         mbar_wait(&sm->v_full[st], sph);
         if (pg == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O
-        PTRACE(8, g);
         fence_proxy_async_smem();  // P arrived through the generic proxy of the peer's threads
         tc_fence_after();
         const uint32_t pa_lo = smem_desc_lo(p_base + b * kPBytes, 16);
@@ -465,7 +467,6 @@ __device__ __forceinline__ void oc_mma_item(PairSmall* sm, uint32_t peer_small, 
         umma_commit_elect(&sm->pv_done[b]);
         umma_commit_elect_addr(peer_small + uint32_t(offsetof(PairSmall, p_empty)) + b * 8);
         if (pg == npages - 1) umma_commit_elect(&sm->o_full);
-        PTRACE(9, g);
     }
 }
 
@@ -618,7 +619,7 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
                     if (rank == 0) sc_mma_item(sm, ring, tmem, smem_u32(base), npages, g, it, p);
                     else oc_mma_item(sm, peer_small, tmem, smem_u32(base), smem_u32(base + kOffP), npages, g, it, p);
                 } else {
-                    oc_epilogue_item(sm, peer_small, w, p, tmem, row, q4, lane, g, it);
+                    oc_epilogue_item(sm, base, peer_small, w, p, tmem, row, q4, lane, g, it);
                 }
             }
         }
@@ -647,11 +648,6 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
 
 int pair_tile_tokens() { return kPairTileTokens; }
 
-typedef CUresult (*EncodeTiledFn2)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static EncodeTiledFn2 g_encode2 = nullptr;
-
 int pair_init(kairos_ctx* ctx) {
     typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -660,7 +656,6 @@ int pair_init(kairos_ctx* ctx) {
     cudaDriverEntryPointQueryResult q;
     KAIROS_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
     if (!fn || q != cudaDriverEntryPointSuccess) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled not available");
-    g_encode2 = reinterpret_cast<EncodeTiledFn2>(fn);
     // latent part of a page: pool viewed as [chunk 9][row num_pages*64][64 elems], box = 8 chunks x 64 rows x 64 elems
     cuuint64_t dims[3] = {64, cuuint64_t(ctx->cfg.num_pages) * kPage, 9};
     cuuint64_t strides[2] = {cuuint64_t(kTokenBytes), 128};
@@ -683,7 +678,6 @@ int pair_init(kairos_ctx* ctx) {
 int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,
                      cudaStream_t stream, bool pdl) {
     PairParams p;
-    p.trace = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + ctx->cfg.workspace_bytes - 8192);  // KAIROS_TRACE builds only
     p.items = dev_items;
     p.n_items = n_items;
     p.counter = reinterpret_cast<int32_t*>(ctx->cfg.workspace) + 2;
@@ -694,17 +688,7 @@ int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     p.lse_chunk = a.lse_chunk;
     p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
     n_pairs = std::max(1, std::min(n_pairs, n_items));
-    CUtensorMap q_map;  // q_chunk as [C*16 rows][576], box = 64 dims x 128 rows (one tile, one 64-dim chunk)
-    {
-        cuuint64_t dims[2] = {cuuint64_t(kDim), cuuint64_t(a.chunk_len) * kHeads};
-        cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
-        cuuint32_t box[2] = {64, 128};
-        cuuint32_t es[2] = {1, 1};
-        CUresult r = g_encode2(&q_map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(a.q_chunk), dims, strides, box, es,
-                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q tile) failed: " + std::to_string(int(r)));
-    }
+    const CUtensorMap& q_map = ctx->qp_map.map;  // q_chunk as [C*16 rows][576], box = 64 dims x 128 rows (encoded by the caller)
     // pdl: launched right behind the decode grid on the same stream with programmatic stream serialisation, so that the
     // clusters start as soon as every decode CTA is resident (that kernel triggers launch_dependents at its start) and
     // run beside it; neither kernel reads what the other writes, so this kernel only executes griddepcontrol.wait before it exits.
@@ -719,7 +703,6 @@ int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
     KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_chunk_pair_kernel, ctx->pool_map_c, ctx->pool_map_v, q_map, p));
-    KAIROS_CUDA_TRY(cudaGetLastError());
     return KAIROS_OK;
 }
 

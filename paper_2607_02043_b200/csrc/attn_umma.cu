@@ -103,18 +103,8 @@ struct Small {
 };
 static_assert(sizeof(Small) <= kSmallBytes, "Small does not fit");
 
-#ifdef KAIROS_TRACE
-#define KTRACE(ev, g) do { if (blockIdx.x == 0 && (g) < 64) p.trace[(ev) * 64 + (g)] = clock64(); } while (0)
-// per-CTA statistics (globaltimer ns) 16 KB below the CTA-0 timeline: [cta][0 start, 1 end, 2 pages, 3 items]
-#define KSTAT(k, v) do { (p.trace - 2048)[blockIdx.x * 4 + (k)] = (v); } while (0)
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#else
-#define KSTAT(k, v) do { } while (0)
-#define KTRACE(ev, g) do { } while (0)
-#endif
 
 struct KParams {
-    unsigned long long* trace;
     const WorkItem* items;
     int32_t n_items;
     int32_t* counters;  // [0] queue head, [1] finished CTAs
@@ -208,7 +198,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const int b = g & 1;
         mbar_wait(&sm->s_full[b], (g >> 1) & 1);
-        if (tid_s == 0) KTRACE(5, g);
         tc_fence_after();
         float x[NC];
 #pragma unroll
@@ -218,7 +207,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->s_empty[b]);
-        if (tid_s == 0) KTRACE(6, g);
 
         const int page = w.page_begin + pg;
         const int key_pos = page * kPage + tok_in_page;
@@ -236,7 +224,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
 #pragma unroll
         for (int c = 0; c < NC; ++c) dmax = fmaxf(dmax, x[c] - sm->m_ref[cbase + c]);
         const bool need = named_or(2, dmax > kRescaleThreshold);
-        if (tid_s == 0) KTRACE(7, g);
         if (need) {
             // exact column (query-row) max over the 64 keys of the page: warp redux, then 4 quadrants through smem
 #pragma unroll
@@ -273,12 +260,25 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
                 for (int c = 0; c < NC; ++c) l[c] *= sm->alpha[cbase + c];
             }
         }
-        if (tid_s == 0) KTRACE(8, g);
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             const float pv = ex2(x[c] - sm->m_ref[cbase + c]);
             l[c] += pv;
             x[c] = pv;
+        }
+        if (boundary && lane_ok && key_pos >= w.n_keys + w.n_q - 1) {
+            // This key is invisible to every row of the item (a stale slot of the sequence's last page): its P^T row is 0, but
+            // the PV MMA still multiplies the page's V rows, and 0 * NaN = NaN.  Zero the token's latent row in the page's
+            // slots (128 B per 64-dim chunk; the 128-byte swizzle permutes inside the row) -- the S MMAs that read it as K
+            // have completed (s_full), the fence below orders the stores before the PV MMAs.  Each column half takes 4 chunks.
+            const PageSlots zs = page_slots<R>(g);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int ch = (sw >> 2) * 4 + c;
+                uint4* dst = reinterpret_cast<uint4*>(kv + (zs.pair[ch >> 1] + (ch & 1)) * kSlotBytes + tok_in_page * 128);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) dst[j] = make_uint4(0u, 0u, 0u, 0u);
+            }
         }
         if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
             uint8_t* ps = kv + page_slots<R>(g).rope * kSlotBytes;
@@ -296,13 +296,11 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->p_full[b]);
-        if (tid_s == 0) KTRACE(9, g);
     }
 
     // ---- epilogue: all PV MMAs of the item are complete
     mbar_wait(&sm->o_full, it & 1);
     tc_fence_after();
-    if (tid_s == 0 && it == 0) KTRACE(10, 5);
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         float v = l[c];
@@ -313,7 +311,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         if (lane == (c & 15)) sm->red[w4][cbase + c] = v;
     }
     named_sync(1);
-    if (tid_s == 0 && it == 0) KTRACE(11, 0);
     const bool is_final = w.partial_slot < 0;
     if (tid_s < N) {
         const float L = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
@@ -333,7 +330,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
         }
     }
     named_sync(2);
-    if (tid_s == 0 && it == 0) KTRACE(11, 1);
     // TMEM reads run at 64 B/clk per SM and each tcgen05.ld round trip costs several hundred cycles: the loads of block
     // b4 + 1 are in flight while block b4 is converted and stored
     uint32_t rr[2][NC];
@@ -344,7 +340,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
     load_block(0, rr[0]);
 #pragma unroll
     for (int b4 = 0; b4 < 4; ++b4) {
-        if (tid_s == 0 && it == 0) KTRACE(11, 2 + b4);
         tmem_wait_ld();
         if (b4 < 3) load_block(b4 + 1, rr[(b4 + 1) & 1]);
         const uint32_t* r = rr[b4 & 1];
@@ -368,7 +363,6 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->o_empty);
-    if (tid_s == 0 && it == 0) KTRACE(10, 6);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -394,7 +388,6 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
             if (ready || s_next == npages) {
                 if (!ready) mbar_wait(&sm->p_full[pst], pph);
                 if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
-                KTRACE(3, gg);
                 tc_fence_after();
                 const PageSlots ps = page_slots<R>(gg);
                 const uint32_t st = gg & (kPageRing - 1);
@@ -410,7 +403,6 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                 umma_commit_elect(&sm->kv_empty[st]);
                 umma_commit_elect(&sm->pv_done[pst]);
                 if (pv_next == npages - 1) umma_commit_elect(&sm->o_full);
-                KTRACE(4, gg);
                 ++pv_next;
                 spins = 0;
                 continue;
@@ -420,7 +412,6 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
             const uint32_t gg = g0 + s_next;
             const uint32_t st = gg & 1;
             if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[gg & (kPageRing - 1)], (gg / kPageRing) & 1))) {
-                KTRACE(1, gg);
                 // No wait on s_empty: S(g) reuses the S^T buffer of page g - 2, whose PV has been issued (s_next <= pv_next + 1,
                 // and an item returns only after its last PV), i.e. p_full(g - 2) was observed, and every softmax warp arrives
                 // on s_empty (after its tcgen05.ld of S^T) before it arrives on p_full.  A completed mbarrier wait still costs
@@ -442,7 +433,6 @@ __device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_ba
                     umma_commit_elect(&sm->q_empty[qbuf]);
                     if (N == 64) umma_commit_elect(&sm->q_empty[1]);
                 }
-                KTRACE(2, gg);
                 spins = 0;
                 continue;
             }
@@ -463,10 +453,6 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     Small* sm = reinterpret_cast<Small*>(base + G::kOffSmall);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) KTRACE(10, 0);
-#ifdef KAIROS_TRACE
-    if (threadIdx.x == 0) KSTAT(0, gtime());
-#endif
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
@@ -501,7 +487,6 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm->tmem_base;
-    if (threadIdx.x == 0) KTRACE(10, 1);
 
     if (warp == 0) {
         // ================= producer: pop work items, TMA-load Q tiles and KV pages =================
@@ -517,19 +502,14 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                 idx = __shfl_sync(0xffffffffu, idx, 0);
             }
             if (idx >= p.n_items) idx = -1;
-            if (lane == 0 && it == 0) KTRACE(10, 2);
             if (lane == 0) {
                 mbar_wait(&sm->item_empty[it & 1], ((it >> 1) & 1) ^ 1);
                 sm->item_ring[it & 1] = idx;
                 mbar_arrive(&sm->item_full[it & 1]);
             }
-#ifdef KAIROS_TRACE
-            if (idx < 0 && lane == 0) { KSTAT(2, (unsigned long long)g); KSTAT(3, (unsigned long long)it); }
-#endif
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
             const int N = (!DEC && w.kind) ? 64 : 16;
-            if (lane == 0 && it == 0) KTRACE(10, 3);
             const bool is_chunk = !DEC && w.kind;
             const int qb = is_chunk ? 0 : int(it & 1);
             if (lane == 0) {
@@ -548,7 +528,6 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
             for (int i = 0; i < npages; i += 32) {
                 const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
                 const int cnt = min(32, npages - i);
-                if (lane == 0 && it == 0 && i == 0) KTRACE(10, 4);
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
@@ -565,7 +544,6 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                             free_slots -= n;
                         };
                         reserve(ps.odd ? 1 : 2);
-                        KTRACE(0, g);
                         mbar_arrive_expect_tx(full, 9 * kSlotBytes);
                         if (ps.odd) tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, full, row, 8, policy);
 #pragma unroll
@@ -629,10 +607,6 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
     // does so before it exits, so that "this grid has completed" implies "the pair grid has completed" for everything that
     // follows in the stream (the combine, the caller's consumers of out_chunk).  No-op for an ordinary launch.
     if (threadIdx.x == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (threadIdx.x == 0) KTRACE(10, 7);
-#ifdef KAIROS_TRACE
-    if (threadIdx.x == 0) KSTAT(1, gtime());
-#endif
     if (warp == 1) tmem_dealloc(tmem, kTmemCols);
     if (threadIdx.x == 0) {
         __threadfence();
@@ -744,22 +718,30 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
 
-int encode_rows_map(CUtensorMap* map, const void* ptr, uint64_t rows, uint32_t box_rows) {
-    cuuint64_t dims[2] = {cuuint64_t(kDim), rows};
-    cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
-    cuuint32_t box[2] = {64, box_rows};
-    cuuint32_t es[2] = {1, 1};
-    CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es,
-                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: " + std::to_string(int(r)));
-    return KAIROS_OK;
-}
-
 }  // namespace
 
 int umma_chunk_tile_tokens() { return kChunkTileTokens; }
 int umma_resident_ctas(const kairos_ctx* ctx) { return ctx->sm_count; }
+
+// q viewed as [rows][576] bf16 with boxes of 64 dims x box_rows rows.  cuTensorMapEncodeTiled costs a few microseconds of
+// host time, so the encoded map is kept while the caller passes the same buffer.
+int encode_q_map(QMapCache* cache, const void* ptr, uint64_t rows, uint32_t box_rows) {
+    if (cache->ptr == ptr && cache->rows == rows) return KAIROS_OK;
+    cuuint64_t dims[2] = {cuuint64_t(kDim), rows};
+    cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
+    cuuint32_t box[2] = {64, box_rows};
+    cuuint32_t es[2] = {1, 1};
+    CUresult r = g_encode(&cache->map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        cache->ptr = nullptr;
+        return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: " + std::to_string(int(r)));
+    }
+    cache->ptr = ptr;
+    cache->rows = rows;
+    return KAIROS_OK;
+}
 
 int umma_init(kairos_ctx* ctx) {
     if (!g_encode) {
@@ -778,7 +760,6 @@ int umma_init(kairos_ctx* ctx) {
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed: " + std::to_string(int(r)));
-    ctx->has_pool_map = true;
     // the ring is filled by boxes of 2 latent chunks (16 KB) and 1 RoPE chunk (8 KB)
     for (int n = 1; n <= 2; ++n) {
         cuuint32_t boxn[3] = {64, 64, cuuint32_t(n)};
@@ -793,17 +774,12 @@ int umma_init(kairos_ctx* ctx) {
     return KAIROS_OK;
 }
 
-int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
-                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched, int max_ctas,
-                     bool as_clusters, bool pdl) {
-    CUtensorMap qd_map = ctx->pool_map, qc_map = ctx->pool_map;  // placeholders when a side is empty (never dereferenced)
-    if (a.n_dec > 0)
-        if (int rc = encode_rows_map(&qd_map, a.q_dec, uint64_t(a.n_dec) * kHeads, 16)) return rc;
-    if (a.chunk_len > 0)
-        if (int rc = encode_rows_map(&qc_map, a.q_chunk, uint64_t(a.chunk_len) * kHeads, 64)) return rc;
+int launch_attn_umma(kairos_ctx* ctx, const Plan& plan, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
+                     cudaStream_t stream, int max_ctas, bool as_clusters, bool pdl) {
+    // placeholders when a side is empty (never dereferenced); the caller has encoded the maps the step needs
+    const CUtensorMap& qd_map = a.n_dec > 0 ? ctx->qd_map.map : ctx->pool_map;
+    const CUtensorMap& qc_map = (a.chunk_len > 0 && plan.n_chunk_items > 0) ? ctx->qc_map.map : ctx->pool_map;
     KParams p;
-    p.trace = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctx->cfg.workspace) +
-                                                    ctx->cfg.workspace_bytes - 8192);  // KAIROS_TRACE builds only
     p.items = dev_items;
     p.n_items = n_items;
     p.counters = reinterpret_cast<int32_t*>(ctx->cfg.workspace);
@@ -820,11 +796,11 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
     // beside the pair kernel the grid is launched as 2-CTA clusters (nothing in the kernel uses the cluster): it then
     // occupies whole TPCs, which the chunk clusters need, and the first item comes from the queue (a CTA that becomes
     // resident late must not be holding a statically assigned item)
-    const bool with_pairs = ctx->plan.n_pairs > 0;
+    const bool with_pairs = plan.n_pairs > 0;
     if (as_clusters) grid = std::max(2, std::min(max_ctas, umma_resident_ctas(ctx)) & ~1);
     p.static_first = with_pairs ? 0 : 1;
     // decode-only queues (no chunk, or the chunk is on the pair grid) take the instantiation with the deeper page ring
-    bool dec_only = a.chunk_len == 0 || ctx->plan.n_chunk_items == 0;
+    bool dec_only = a.chunk_len == 0 || plan.n_chunk_items == 0;
     if (ctx->force_dec_only >= 0) dec_only = dec_only && ctx->force_dec_only != 0;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(unsigned(grid), 1, 1);
@@ -851,10 +827,6 @@ int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_ite
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_mixed_kernel<true>, ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p));
     else
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_mixed_kernel<false>, ctx->pool_map2, ctx->pool_map1, qd_map, qc_map, p));
-    KAIROS_CUDA_TRY(cudaGetLastError());
-    *kernels_launched = 1;
-    (void)dev_combines;
-    (void)n_combines;
     return KAIROS_OK;
 }
 
@@ -878,7 +850,6 @@ int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_co
         // with two attention kernels in flight the second one waits for the first before it exits, so following it is enough
         cfg.numAttrs = 1;
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, partials, out_dec, out_chunk, lse_dec, lse_chunk));
-        KAIROS_CUDA_TRY(cudaGetLastError());
     }
     return KAIROS_OK;
 }

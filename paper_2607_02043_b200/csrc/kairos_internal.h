@@ -73,57 +73,10 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
 constexpr size_t kPartialSlotBytes = size_t(kHeads) * kLatent * 4 + size_t(kHeads) * 2 * 4;  // o[16][512] f32 + (m,l)[16]
 
 // ---- context ---------------------------------------------------------------------------------------
-struct StagingSlot {
-    void* host = nullptr;    // pinned
-    void* dev = nullptr;
-    size_t bytes = 0;
-    cudaEvent_t done = nullptr;  // recorded after the H2D copy out of `host`
-    cudaEvent_t consumed = nullptr;  // recorded on the caller's stream after the kernels that read `dev` (plan copies only)
-    bool used = false;
-};
-
 struct HostStage {  // device staging for kairos_mixed_step_host
     void* dev = nullptr;
     size_t bytes = 0;
 };
-
-}  // namespace kairos
-
-struct kairos_ctx {
-    kairos_config cfg;
-    int sm_count = 0;
-    int impl = 1;                 // 0 = simple CUDA-core kernel (debug cross-check), 1 = tcgen05 path
-    CUtensorMap pool_map;         // TMA descriptor of the pool (filled when impl needs it)
-    bool has_pool_map = false;
-    CUtensorMap pool_map2, pool_map1;  // boxes of 2 latent chunks / 1 chunk of a page: the slot ring of kairos_mixed_kernel
-    int force_dec_only = -1;      // KAIROS_DEC_ONLY env (sweeps): 0 = never use the decode-only instantiation
-    CUtensorMap pool_map_c;       // one 64-dim chunk of a page (8 KB box): K ring of the pair kernel's S-CTA
-    CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
-    cudaStream_t copy_stream = nullptr; // the plan's H2D copy runs here, beside whatever precedes the step on the caller's stream
-    int force_pairs = -1;         // KAIROS_PAIRS env (sweeps): -1 auto, 0 never use the pair kernel, n > 0 decode grid first beside n
-                                  // clusters, -(n + 1) n clusters first (plan.cpp::choose_pairs)
-    static constexpr int kStagingSlots = 4;
-    kairos::StagingSlot staging[kStagingSlots];
-    int staging_next = 0;
-    kairos::HostStage host_stage;
-    kairos::Plan plan;            // reused per call
-    int64_t last_info[7] = {0, 0, 0, 0, 0, 0, 0};
-    bool profile = false;         // bracket the main kernel with events (kairos_profile_enable)
-    std::vector<cudaEvent_t> prof_events;  // pairs: [2i] start, [2i+1] stop
-    size_t prof_used = 0;         // events in use since the last kairos_profile_read
-};
-
-namespace kairos {
-
-// Acquire a pinned+device staging pair of at least `bytes` (waits for the slot's previous copy).
-int staging_acquire(kairos_ctx* ctx, size_t bytes, StagingSlot** out);
-
-// ---- kernel launchers (each returns a kairos_status) -----------------------------------------------
-int launch_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
-                  int32_t start_pos, cudaStream_t stream);
-int launch_append_decode(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
-                         int32_t table_stride, const int32_t* positions, cudaStream_t stream);
-int launch_gather(kairos_ctx* ctx, const int32_t* page_table, int32_t n_tokens, void* out, cudaStream_t stream);
 
 struct StepArgs {
     int32_t n_dec;
@@ -139,19 +92,95 @@ struct StepArgs {
     float* lse_chunk;
 };
 
-// impl 0: one CTA per query token on CUDA cores (attn_simple.cu). dev_lens = device copy of dec_ctx_lens.
-int launch_attn_simple(kairos_ctx* ctx, const StepArgs& a, const int32_t* dev_lens, cudaStream_t stream);
+// Device-resident copy of one plan's work lists (items | combines | pair items) with its pinned source.
+struct PlanBuffer {
+    void* host = nullptr;              // pinned
+    void* dev = nullptr;
+    size_t cap = 0;
+    cudaEvent_t uploaded = nullptr;    // recorded behind the H2D copy out of `host`
+    cudaEvent_t last_use = nullptr;    // recorded on the caller's stream behind the kernels that read `dev`
+    bool upload_pending = false;       // the H2D may still be in flight: the caller's stream waits on `uploaded`
+    bool ever_used = false;
+    cudaGraphExec_t exec = nullptr;    // the step's kernels captured for `gargs` (replayed by cudaGraphLaunch)
+    StepArgs gargs{};
+    int same_args_uses = 0;            // consecutive uses with the pointer set of `gargs`
+};
 
-// impl 1: persistent tcgen05/TMA kernel over the plan's work items + LSE combine (attn_umma.cu).
+// One cached plan (a0): reused by every later step with the same (lengths, C, P) without planning, copying or encoding
+// anything (exact hit), or -- when only lengths inside the last pages moved, so that every request keeps its page count --
+// patched in place and re-uploaded to the other buffer (structural hit).
+struct PlanEntry {
+    bool valid = false;
+    uint64_t stamp = 0;                // LRU clock
+    int32_t n_dec = 0, chunk_len = 0, prefix_len = 0, target_ctas = 0, pair_mode = 0;
+    std::vector<int32_t> lens;
+    Plan plan;
+    size_t items_bytes = 0, comb_off = 0, comb_bytes = 0, pair_off = 0, pair_bytes = 0, total_bytes = 0;
+    PlanBuffer buf[2];
+    int cur = 0;
+};
+
+struct QMapCache {  // a q tensor map stays valid while (pointer, rows) do not change
+    const void* ptr = nullptr;
+    uint64_t rows = 0;
+    CUtensorMap map;
+};
+
+}  // namespace kairos
+
+struct kairos_ctx {
+    kairos_config cfg;
+    int sm_count = 0;
+    CUtensorMap pool_map;         // TMA descriptor of the pool (placeholder q map when a side of the step is empty)
+    CUtensorMap pool_map2, pool_map1;  // boxes of 2 latent chunks / 1 chunk of a page: the slot ring of kairos_mixed_kernel
+    CUtensorMap pool_map_c;       // a group of 64-dim chunks of a page: K ring of the pair kernel's S-CTA
+    CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
+    kairos::QMapCache qd_map, qc_map, qp_map;  // decode q (box 16 rows), chunk q for gen-1 tiles (64 rows), for the pair kernel (128 rows)
+    cudaStream_t copy_stream = nullptr;   // plan H2D copies run here, beside whatever precedes the step on the caller's stream
+    cudaStream_t capture_stream = nullptr;  // the step's launches are captured here when a plan is replayed as a CUDA graph
+    // kairos_debug_set knobs (tests and sweeps only)
+    int force_pairs = -1;         // -1 auto, 0 never use the pair kernel, n > 0 decode grid first beside n clusters, -(n + 1) n clusters first
+    int force_dec_only = -1;      // 0 = never use the decode-only instantiation
+    int use_copy_stream = 1, use_graph = 1, use_plan_cache = 1;
+    static constexpr int kPlanEntries = 8;
+    kairos::PlanEntry plans[kPlanEntries];
+    uint64_t plan_clock = 0;
+    kairos::HostStage host_stage;
+    int64_t last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    bool profile = false;         // bracket the attention kernels with events (kairos_profile_enable)
+    std::vector<cudaEvent_t> prof_events;  // pairs: [2i] start, [2i+1] stop
+    size_t prof_used = 0;         // events in use since the last kairos_profile_read
+    // latency-table scratch (allocated once, grown on demand; freed by kairos_destroy)
+    void* table_buf = nullptr;
+    size_t table_bytes = 0;
+    void* flush_buf = nullptr;
+};
+
+namespace kairos {
+
+// Shared by kairos_mixed_step, the latency table and the schedule runner: validate, plan (or reuse), stage, launch.
+int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                    const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len, const void* q_chunk,
+                    const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk, float* lse_dec,
+                    float* lse_chunk, cudaStream_t stream);
+
+// ---- kernel launchers (each returns a kairos_status) -----------------------------------------------
+int launch_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
+                  int32_t start_pos, cudaStream_t stream);
+int launch_append_decode(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                         int32_t table_stride, const int32_t* positions, cudaStream_t stream);
+int launch_gather(kairos_ctx* ctx, const int32_t* page_table, int32_t n_tokens, void* out, cudaStream_t stream);
+
+// persistent tcgen05/TMA kernel over the plan's work items + LSE combine (attn_umma.cu)
 int umma_chunk_tile_tokens();
 int umma_resident_ctas(const kairos_ctx* ctx);
-int launch_attn_umma(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
-                     const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream, int* kernels_launched,
-                     int max_ctas, bool as_clusters, bool pdl);
+int encode_q_map(QMapCache* cache, const void* ptr, uint64_t rows, uint32_t box_rows);  // no-op when (ptr, rows) are unchanged
+int launch_attn_umma(kairos_ctx* ctx, const Plan& plan, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
+                     cudaStream_t stream, int max_ctas, bool as_clusters, bool pdl);
 int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream);
 int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
 
-// impl 1, chunk tiles on 2-CTA clusters (attn_pair.cu)
+// chunk tiles on 2-CTA clusters (attn_pair.cu)
 int pair_tile_tokens();
 int pair_init(kairos_ctx* ctx);
 int launch_attn_pair(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, int32_t n_pairs,

@@ -60,6 +60,8 @@ _lib.kairos_profile_enable.argtypes = [_vp, _i32]
 _lib.kairos_profile_enable.restype = _c.c_int
 _lib.kairos_profile_read.argtypes = [_vp, _vp, _vp]
 _lib.kairos_profile_read.restype = _c.c_int
+_lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
+_lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
 _lib.kairos_last_error.restype = _c.c_char_p
 _lib.kairos_version.argtypes = []
@@ -67,7 +69,8 @@ _lib.kairos_version.restype = _c.c_char_p
 
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
-           "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_last_error", "kairos_version"]
+           "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
+           "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
           -4: "KAIROS_ERR_CUDA"}
@@ -212,10 +215,15 @@ class Kairos:
         return float(us.value), int(n.value)
 
     def last_plan_info(self) -> dict:
-        info = (_c.c_int64 * 7)()
-        _check(_lib.kairos_last_plan_info(self._h, info, 7))
-        keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes", "chunk_pairs"]
+        info = (_c.c_int64 * 10)()
+        _check(_lib.kairos_last_plan_info(self._h, info, 10))
+        keys = ["work_items", "decode_splits", "chunk_tiles", "ctas", "kernels", "workspace_bytes", "chunk_pairs",
+                "plan_cache", "graph", "dec_ctas_first"]
         return dict(zip(keys, (int(x) for x in info)))
+
+    def debug_set(self, key: str, value: int) -> None:
+        """Test-only knobs (kairos_debug_set)."""
+        _check(_lib.kairos_debug_set(self._h, key.encode(), int(value)))
 
 
 def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ctas: int = 148, pair_mode: int = 0,

@@ -6,8 +6,6 @@ outputs concatenated.  Cache append / gather are compared bit for bit.
 """
 from __future__ import annotations
 
-import os
-
 import numpy as np
 
 from oracle import oracle
@@ -26,32 +24,24 @@ def oracle_pool_after_append(inp: W.MixedStepInputs) -> np.ndarray:
 
 
 class GpuRun:
-    """Uploads the inputs, appends the chunk, runs kairos_mixed_step.  Keeps device tensors for reuse."""
+    """Uploads the inputs, appends the chunk, runs kairos_mixed_step.  Keeps device tensors for reuse.
 
-    def __init__(self, inp: W.MixedStepInputs, impl: str = "umma", workspace_bytes=None, pairs=None):
+    `pairs` forces the launch order of the two grids through the test-only kairos_debug_set (None = the planner decides);
+    `knobs` = further kairos_debug_set pairs, e.g. dict(graph=0, plan_cache=0).
+    """
+
+    def __init__(self, inp: W.MixedStepInputs, workspace_bytes=None, pairs=None, knobs=None):
         import torch
         from paper_2607_02043_b200 import kairos as K
         self.K, self.torch, self.inp = K, torch, inp
-        old = os.environ.get("KAIROS_IMPL")
-        old_pairs = os.environ.get("KAIROS_PAIRS")
-        os.environ["KAIROS_IMPL"] = impl
-        if pairs is not None:  # force the chunk onto `pairs` 2-CTA clusters (0 = never), read at kairos_create
-            os.environ["KAIROS_PAIRS"] = str(pairs)
-        try:
-            self.pool = K.bf16_tensor(inp.pool)
-            ws = K.workspace_bytes(max(inp.n_dec, 1), max(inp.chunk_len, 1)) if workspace_bytes is None else workspace_bytes
-            self.ws = torch.empty(ws, dtype=torch.uint8, device="cuda")
-            self.ctx = K.Kairos(self.pool, self.ws, inp.softmax_scale)
-        finally:
-            if old is None:
-                os.environ.pop("KAIROS_IMPL", None)
-            else:
-                os.environ["KAIROS_IMPL"] = old
-            if pairs is not None:
-                if old_pairs is None:
-                    os.environ.pop("KAIROS_PAIRS", None)
-                else:
-                    os.environ["KAIROS_PAIRS"] = old_pairs
+        self.pool = K.bf16_tensor(inp.pool)
+        ws = K.workspace_bytes(max(inp.n_dec, 1), max(inp.chunk_len, 1)) if workspace_bytes is None else workspace_bytes
+        self.ws = torch.empty(ws, dtype=torch.uint8, device="cuda")
+        self.ctx = K.Kairos(self.pool, self.ws, inp.softmax_scale)
+        if pairs is not None:
+            self.ctx.debug_set("pairs", pairs)
+        for k, v in (knobs or {}).items():
+            self.ctx.debug_set(k, v)
         dev = "cuda"
         self.q_dec = K.bf16_tensor(inp.q_dec)
         self.q_chunk = K.bf16_tensor(inp.q_chunk)
@@ -59,15 +49,24 @@ class GpuRun:
         self.chunk_pt = torch.from_numpy(inp.chunk_page_table).to(dev)
         self.latent = K.bf16_tensor(inp.chunk_latent)
         self.k_rope = K.bf16_tensor(inp.chunk_k_rope)
+        self.out = None
 
     def append(self):
         if self.inp.chunk_len:
             self.ctx.append_latent(self.latent, self.k_rope, self.chunk_pt, self.inp.prefix_len)
 
-    def step(self):
+    def step(self, reuse_outputs=False):
+        """One kairos_mixed_step.  reuse_outputs: pass the previous call's output tensors again (same pointers: the
+        plan's kernels are then replayed as a CUDA graph from the second such call on), poisoned first."""
         i = self.inp
-        od, oc, ld, lc = self.ctx.mixed_step(self.q_dec, self.dec_pt, i.dec_ctx_lens, self.q_chunk, self.chunk_pt,
-                                             i.chunk_len, i.prefix_len)
+        kw = {}
+        if reuse_outputs and self.out is not None:
+            for t in self.out:
+                t.fill_(float("nan"))
+            kw = dict(out_dec=self.out[0], out_chunk=self.out[1], lse_dec=self.out[2], lse_chunk=self.out[3])
+        self.out = self.ctx.mixed_step(self.q_dec, self.dec_pt, i.dec_ctx_lens, self.q_chunk, self.chunk_pt,
+                                       i.chunk_len, i.prefix_len, **kw)
+        od, oc, ld, lc = self.out
         self.torch.cuda.synchronize()
         f = lambda t: W.bf16_bits_to_f32(self.K.bf16_bits(t))
         return f(od), f(oc), ld.cpu().numpy(), lc.cpu().numpy()
