@@ -354,7 +354,8 @@ def main():
                 continue
             pt = Point(ci, cc, 0, dev, K, torch)
             pt.warm(args.warmup)
-            n = max(args.steps, 30)
+            ms, _, _, _ = pt.timed(10, barrier)  # sizes the timed region: at least K steps and about 30 ms
+            n = int(min(max(args.steps, 30e3 / max(ms * 1e3 / 10, 1.0)), 400))
             ms, host_s, _, _ = pt.timed(n, barrier)
             _, _, k_us, k_n = pt.timed(n, barrier, profile=True)
             us, kern = ms * 1e3 / n, k_us / max(k_n, 1)

@@ -221,6 +221,89 @@ int kairos_last_plan_info(const kairos_ctx* ctx, int64_t* info, int32_t n);
 int kairos_profile_enable(kairos_ctx* ctx, int32_t on);
 int kairos_profile_read(kairos_ctx* ctx, double* main_kernel_us_total, int64_t* launches);
 
+/* ------------------------------------------------------------------------------------------------------------
+ * the consumer of the latency table: KAIROS' step-latency model, TBT-safe chunk schedule and
+ * deflection decision (section 4.2-4.4, Eq. 1-7; Algorithm 1).  Pure HOST code: no CUDA
+ * call, no context; every pointer below is a HOST pointer; all latencies are in the unit of the samples the model was
+ * fitted on (microseconds when they come from kairos_step_latency_table).
+ *
+ * Eq. 4: T_step = T0 + dT_pf, both "simple linear regressors" fitted once per model/hardware
+ * (PAPER.md:302-313).  The paper lumps all cached tokens into K_n; one attention layer treats a decode's cached token
+ * (read once per step) and a cached token of the deflected request (met by every query token of the chunk) differently,
+ * so the model keeps them apart (reading G20):
+ *     T0(B, Kd)       = a[0] + a[1]*B + a[2]*Kd                              Kd = tokens cached by the B in-flight decodes
+ *     dT_pf(C, P, Kd) = b[0] + b[1]*C + b[2]*C*(P + (C+1)/2) + b[3]*Kd       C > 0 prefill tokens over a P-token prefix
+ *     dT_pf = 0 for C = 0.
+ * Prefill-node step latency: T_pf_step(tokens, cached) = p[0] + p[1]*tokens + p[2]*cached + p[3]*tokens*cached.
+ */
+typedef struct {
+    double a[3];
+    double b[4];
+} kairos_step_model;
+
+typedef struct {
+    double p[4];
+} kairos_prefill_model;
+
+/*
+ * Closed-form weighted least squares for the two regressors of Eq. 4, as PAPER.md:312 describes: T0 from the samples
+ * with C == 0, then dT_pf from the residual T - T0 of the samples with C > 0.  Rows are weighted by 1/T so that the
+ * fit minimises relative error, the criterion the paper states (MAPE < 10 %; reading G21).
+ *   B, Kd, C, P   int64 [n]    sample points (Kd = B * K for a table entry with per-decode context K)
+ *   T             double [n]   measured step latency, each > 0
+ *   model         out
+ *   mape_out      out or NULL: mean |pred - T| / T over the n samples
+ * Errors: INVALID_ARG (NULL, n < 1, T <= 0, fewer than 3 decode-only or 4 mixed samples, or a singular system, e.g.
+ * every sample with the same B).
+ */
+int kairos_fit_latency_model(const int64_t* B, const int64_t* Kd, const int64_t* C, const int64_t* P, const double* T,
+                             int32_t n, kairos_step_model* model, double* mape_out);
+
+/* Eq. 4 evaluated: predicted latency of a step with B decodes caching Kd tokens and C prefill tokens over a P-token prefix. */
+double kairos_predict_step(const kairos_step_model* model, int64_t B, int64_t Kd, int64_t C, int64_t P);
+
+typedef struct {
+    int32_t prompt_len;          /* l_r >= 1 */
+    const int32_t* queue_lens;   /* prompt lengths queued ahead of r on its prefill node (FIFO), [n_queue] */
+    int32_t n_queue;
+    int32_t chi_p;               /* prefill-node chunk size >= 1 */
+    const int32_t* node_B;       /* decode-node states: B_n in-flight decodes ...            [n_nodes] */
+    const int64_t* node_K;       /* ... caching K_n tokens in total                          [n_nodes] */
+    int32_t n_nodes;
+    const int32_t* candidates;   /* chunk-size candidates chi_1 > ... > chi_C > 0: TOTAL tokens of a step (the paper's
+                                    chi), of which chi - B_n are prefill tokens     [n_candidates] */
+    int32_t n_candidates;
+    double tbt_slo;              /* tau */
+    double beta;                 /* safety factor of Eq. 5, > 0 */
+    double alpha;                /* deflection margin of Eq. 7, >= 1 */
+    double ttft_slo;
+} kairos_decide_input;
+
+typedef struct {
+    int32_t decision;            /* 0 = KEEP on the prefill node, 1 = DEFLECT */
+    int32_t node;                /* n* (index into node_B / node_K), -1 when kept */
+    int32_t n_steps;             /* |X*|, 0 when kept */
+    double ttft_pf;              /* Eq. 1 */
+    double ttft_dec;             /* Eq. 6 of the fastest feasible node (+inf if none is feasible) */
+} kairos_decide_output;
+
+/*
+ * Algorithm 1: (1) prefill-node TTFT estimate, Eq. 1-3; (2) for every decode node the greedy TBT-safe
+ * schedule X = [chi(1) .. chi(m)] -- at each step the largest candidate with T_step <= beta * tau (Eq. 5) -- and its
+ * TTFT estimate (Eq. 6); (3) the fastest feasible node; (4) DEFLECT iff Eq. 7 holds.  Readings of the garbled spots
+ * (G19): Eq. 3 sums i = 0 .. ceil(l_r/chi_p) - 1; a step serves chi - B_n prefill tokens, candidates <= B_n
+ * are skipped; the feasible set starts empty; the threshold is beta * tau.  State projected for step i of a schedule on
+ * node n: Kd = K_n + (i-1)*B_n, P = prefill tokens served so far, C = chi(i) - B_n.  Ties between nodes go to the lowest index.
+ *   schedule_out   int32 [max_schedule] or NULL: X* (the chi values, in order).  kairos_run_schedule takes the prefill
+ *                  tokens per step, chi(i) - B_n (the last one trimmed to what is left of the prompt).
+ * Never returns DEFLECT for a schedule the model predicts unsafe.  Cost: O(n_nodes * ceil(l_r /
+ * (chi_min - B)) * n_candidates) evaluations of Eq. 4.
+ * Errors: INVALID_ARG (NULL, sizes < 1, candidates not strictly decreasing, beta <= 0, alpha < 1), WORKSPACE if X* is
+ * longer than max_schedule (out->n_steps holds the length needed).
+ */
+int kairos_decide(const kairos_step_model* model, const kairos_prefill_model* prefill, const kairos_decide_input* in,
+                  int32_t* schedule_out, int32_t max_schedule, kairos_decide_output* out);
+
 /*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.

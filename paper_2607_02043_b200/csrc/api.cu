@@ -197,8 +197,10 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     // ---- a0: find the plan (exact hit: same lengths; structural hit: same page count per request), else build it
     PlanEntry* hit = nullptr;
     PlanEntry* structural = nullptr;
-    PlanEntry* victim = &ctx->plans[0];
+    PlanEntry* victim = &ctx->plans[ctx->plan_clock % kairos_ctx::kPlanEntries];  // cache off: rotate, so that a step's plan
+                                                                                   // copy never waits for the previous step
     if (ctx->use_plan_cache) {
+        victim = &ctx->plans[0];
         for (PlanEntry& e : ctx->plans) {
             if (!e.valid) { if (victim->valid) victim = &e; continue; }
             if (victim->valid && e.stamp < victim->stamp) victim = &e;

@@ -60,6 +60,35 @@ _lib.kairos_profile_enable.argtypes = [_vp, _i32]
 _lib.kairos_profile_enable.restype = _c.c_int
 _lib.kairos_profile_read.argtypes = [_vp, _vp, _vp]
 _lib.kairos_profile_read.restype = _c.c_int
+
+
+class StepModel(_c.Structure):
+    """kairos_step_model (Eq. 4): T0 = a0 + a1*B + a2*Kd; dT_pf = b0 + b1*C + b2*C*(P + (C+1)/2) + b3*Kd for C > 0."""
+    _fields_ = [("a", _c.c_double * 3), ("b", _c.c_double * 4)]
+
+
+class PrefillModel(_c.Structure):
+    """kairos_prefill_model: T = p0 + p1*tokens + p2*cached + p3*tokens*cached."""
+    _fields_ = [("p", _c.c_double * 4)]
+
+
+class DecideInput(_c.Structure):
+    _fields_ = [("prompt_len", _i32), ("queue_lens", _vp), ("n_queue", _i32), ("chi_p", _i32), ("node_B", _vp),
+                ("node_K", _vp), ("n_nodes", _i32), ("candidates", _vp), ("n_candidates", _i32), ("tbt_slo", _c.c_double),
+                ("beta", _c.c_double), ("alpha", _c.c_double), ("ttft_slo", _c.c_double)]
+
+
+class DecideOutput(_c.Structure):
+    _fields_ = [("decision", _i32), ("node", _i32), ("n_steps", _i32), ("ttft_pf", _c.c_double), ("ttft_dec", _c.c_double)]
+
+
+_lib.kairos_fit_latency_model.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, _c.POINTER(StepModel), _vp]
+_lib.kairos_fit_latency_model.restype = _c.c_int
+_lib.kairos_predict_step.argtypes = [_c.POINTER(StepModel), _c.c_int64, _c.c_int64, _c.c_int64, _c.c_int64]
+_lib.kairos_predict_step.restype = _c.c_double
+_lib.kairos_decide.argtypes = [_c.POINTER(StepModel), _c.POINTER(PrefillModel), _c.POINTER(DecideInput), _vp, _i32,
+                               _c.POINTER(DecideOutput)]
+_lib.kairos_decide.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
 _lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
@@ -70,6 +99,7 @@ _lib.kairos_version.restype = _c.c_char_p
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
+           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -240,6 +270,51 @@ def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ct
     if with_pairs:
         return items, int(slots.value), int(pairs.value)
     return items, int(slots.value)
+
+
+# -- latency model, chunk schedule, deflection decision (host only)
+def fit_latency_model(B, Kd, C, P, T):
+    """kairos_fit_latency_model: (StepModel, in-sample MAPE)."""
+    arr = [np.ascontiguousarray(np.asarray(x, dtype=np.int64)) for x in (B, Kd, C, P)]
+    Tn = np.ascontiguousarray(np.asarray(T, dtype=np.float64))
+    m, mape = StepModel(), _c.c_double(0.0)
+    _check(_lib.kairos_fit_latency_model(*(a.ctypes.data_as(_vp) for a in arr), Tn.ctypes.data_as(_vp), int(Tn.size),
+                                         _c.byref(m), _c.byref(mape)))
+    return m, float(mape.value)
+
+
+def step_model(a, b) -> StepModel:
+    m = StepModel()
+    m.a[:] = [float(x) for x in a]
+    m.b[:] = [float(x) for x in b]
+    return m
+
+
+def prefill_model(p) -> PrefillModel:
+    m = PrefillModel()
+    m.p[:] = [float(x) for x in p]
+    return m
+
+
+def predict_step(model: StepModel, B: int, Kd: int, C: int, P: int) -> float:
+    return float(_lib.kairos_predict_step(_c.byref(model), int(B), int(Kd), int(C), int(P)))
+
+
+def decide(model: StepModel, prefill: PrefillModel, prompt_len: int, queue_lens, chi_p: int, nodes, candidates,
+           tbt_slo: float, beta: float, alpha: float, ttft_slo: float, max_schedule: int = 4096):
+    """kairos_decide (Algorithm 1): (decision 'KEEP'|'DEFLECT', n_star, X_star, ttft_pf, ttft_dec)."""
+    q = np.ascontiguousarray(np.asarray(queue_lens, dtype=np.int32))
+    nb = np.ascontiguousarray(np.asarray([n[0] for n in nodes], dtype=np.int32))
+    nk = np.ascontiguousarray(np.asarray([n[1] for n in nodes], dtype=np.int64))
+    cand = np.ascontiguousarray(np.asarray(candidates, dtype=np.int32))
+    ptr = lambda a: a.ctypes.data_as(_vp) if a.size else None
+    inp = DecideInput(int(prompt_len), ptr(q), int(q.size), int(chi_p), ptr(nb), ptr(nk), int(nb.size), ptr(cand),
+                      int(cand.size), float(tbt_slo), float(beta), float(alpha), float(ttft_slo))
+    sched = np.zeros(max_schedule, dtype=np.int32)
+    out = DecideOutput()
+    _check(_lib.kairos_decide(_c.byref(model), _c.byref(prefill), _c.byref(inp), sched.ctypes.data_as(_vp), max_schedule,
+                              _c.byref(out)))
+    return ("DEFLECT" if out.decision else "KEEP"), int(out.node), sched[:out.n_steps].tolist(), float(out.ttft_pf), float(out.ttft_dec)
 
 
 def bf16_tensor(bits: np.ndarray, device="cuda") -> torch.Tensor:

@@ -278,7 +278,7 @@ def test_structural_plan_hit_lengths_move_inside_last_pages():
     from oracle import oracle
     import torch
     lens0 = np.array([70, 135, 700, 2500, 68], np.int32)
-    inp = W.make_inputs("structural", 41, lens0, 24, 40, q_scale=0.5, extra_pages=2)
+    inp = W.make_inputs("structural", 41, lens0.tolist(), 24, 40, q_scale=0.5, extra_pages=2)
     run = Hp.GpuRun(inp)
     run.append()
     pool_np = Hp.oracle_pool_after_append(inp)
@@ -310,7 +310,7 @@ def test_soak_many_steps_rotating_pages(pairs):
     from paper_2607_02043_b200 import kairos as K
     rng = np.random.default_rng(17)
     lens = np.array([64, 200, 700, 1500], np.int32)
-    inp = W.make_inputs("soak", 53, lens, 48, 30, q_scale=0.5, extra_pages=4)
+    inp = W.make_inputs("soak", 53, lens.tolist(), 48, 30, q_scale=0.5, extra_pages=4)
     run = Hp.GpuRun(inp, pairs=pairs)
     n_steps = 60
     lat = rng.integers(0, 2 ** 16, (n_steps, inp.chunk_len, 512), dtype=np.uint16) & np.uint16(0xBF7F)  # finite bf16, |x| < 2
