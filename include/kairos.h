@@ -305,6 +305,46 @@ int kairos_decide(const kairos_step_model* model, const kairos_prefill_model* pr
                   int32_t* schedule_out, int32_t max_schedule, kairos_decide_output* out);
 
 /*
+ * what the decode node does with a deflected request (section 4.3.2;
+ * PAPER.md:363-367 section 5.4; Fig. 1's "successive chunks"): the chunk schedule X = [chi(1) ..
+ * chi(m)] executed as m successive steps behind one call.  Step i (0-based):
+ *   1. if dec_latent != NULL, every in-flight decode j caches its newest token (dec_latent[i][j] | dec_k_rope[i][j]) at
+ *      position dec_ctx_lens[j] + i of its sequence and then attends to dec_ctx_lens[j] + i + 1 tokens; with dec_latent ==
+ *      NULL the decodes' contexts do not move (each attends to dec_ctx_lens[j] tokens in every step);
+ *   2. chunk i of the prompt -- chunk_sizes[i] PREFILL tokens (the paper's chi(i) - B_n) -- is appended at positions
+ *      prefix_len + sum_{k<i} chunk_sizes[k] .. of the request's sequence;
+ *   3. one mixed step: the n_dec decode queries q_dec[i] plus the chunk's queries, causal over the request's prefix.
+ * The whole schedule is planned up front (a0 for every step), its work lists are copied to the device once, and its
+ * launches -- appends, attention grids, combines, programmatic edges included -- are captured into ONE CUDA graph that is
+ * launched on `cuda_stream`; a call that repeats the previous call's arguments replays the graph.  Results are those of
+ * m calls of kairos_append_* / kairos_mixed_step (chunk invariance: the prompt's outputs equal a one-shot
+ * causal prefill row for row).
+ *   q_dec        DEVICE bf16 [n_steps][n_dec][16][576]      out_dec DEVICE bf16 [n_steps][n_dec][16][512]
+ *   dec_page_tables DEVICE int32 [n_dec][dec_table_stride], covering dec_ctx_lens[j] + n_steps tokens when contexts grow
+ *   dec_ctx_lens HOST int32 [n_dec]: tokens cached BEFORE the schedule starts (>= 1, or >= 0 when contexts grow)
+ *   dec_latent   DEVICE bf16 [n_steps][n_dec][512] or NULL  dec_k_rope DEVICE bf16 [n_steps][n_dec][64] or NULL
+ *   chunk_sizes  HOST int32 [n_steps], each >= 1, summing to prompt_len
+ *   q_prompt     DEVICE bf16 [prompt_len][16][576]          prompt_latent [prompt_len][512], prompt_k_rope [prompt_len][64]
+ *   prompt_page_table DEVICE int32 [prompt_table_len], covering prefix_len + prompt_len tokens
+ *   out_prompt   DEVICE bf16 [prompt_len][16][512]          lse_dec [n_steps][n_dec][16] / lse_prompt [prompt_len][16] or NULL
+ *   ttft_us      HOST or NULL: measured TTFT_dec of the schedule (the left-hand side of Eq. 6): device time
+ *                from the first append to the end of the last step, CUDA events on `cuda_stream`
+ *   step_us      HOST double [n_steps] or NULL: device time of every step (this mode launches the steps one by one
+ *                with an event pair around each instead of replaying the graph)
+ * Asynchronous unless ttft_us or step_us is given (then it synchronises the stream).  A call whose arguments differ from
+ * the previous call's synchronises `cuda_stream` once before it overwrites the schedule's device arena.
+ * Errors: INVALID_ARG (sizes, NULL, chunk sizes not summing to prompt_len, a page table too short, misaligned buffers),
+ * WORKSPACE (a step's split-KV partials exceed the workspace), CUDA.
+ */
+int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                        int32_t dec_table_stride, const int32_t* dec_ctx_lens, const void* dec_latent,
+                        const void* dec_k_rope, int32_t prompt_len, const int32_t* chunk_sizes, int32_t n_steps,
+                        const void* q_prompt, const void* prompt_latent, const void* prompt_k_rope,
+                        const int32_t* prompt_page_table, int32_t prompt_table_len, int32_t prefix_len, void* out_dec,
+                        void* out_prompt, float* lse_dec, float* lse_prompt, double* step_us, double* ttft_us,
+                        void* cuda_stream);
+
+/*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
  *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;

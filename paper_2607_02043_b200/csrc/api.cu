@@ -310,6 +310,241 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     return KAIROS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// a whole chunk schedule X = [chi(1) .. chi(m)] as m successive (append -> mixed step) steps
+// ---------------------------------------------------------------------------------------------------------------
+struct ScheduleArgs {
+    int32_t n_dec;
+    const void* q_dec;
+    const int32_t* dec_page_tables;
+    int32_t dec_table_stride;
+    const void* dec_latent;
+    const void* dec_k_rope;
+    const void* q_prompt;
+    const void* prompt_latent;
+    const void* prompt_k_rope;
+    const int32_t* prompt_page_table;
+    int32_t prompt_table_len, prefix_len;
+    void* out_dec;
+    void* out_prompt;
+    float* lse_dec;
+    float* lse_prompt;
+};
+
+// Enqueues steps [0, m) on `stream` (the caller's, or the capture stream).  ev: 2 events per step (start, stop) or NULL.
+static int enqueue_schedule(kairos_ctx* ctx, const ScheduleArgs& s, const std::vector<PlanEntry>& steps, const std::vector<int32_t>& lens0,
+                            const int32_t* chunk_sizes, int32_t m, const uint8_t* arena, const std::vector<size_t>& plan_off,
+                            size_t pos_off, cudaStream_t stream, cudaEvent_t* ev) {
+    const bool grow = s.dec_latent != nullptr;
+    int64_t done = 0;
+    for (int32_t i = 0; i < m; ++i) {
+        const int32_t C = chunk_sizes[i];
+        const int32_t P = s.prefix_len + int32_t(done);
+        if (ev) KAIROS_CUDA_TRY(cudaEventRecord(ev[2 * i], stream));
+        if (grow && s.n_dec > 0)  // every in-flight decode caches its newest token first
+            if (int rc = launch_append_decode(ctx, static_cast<const uint8_t*>(s.dec_latent) + size_t(i) * s.n_dec * kLatent * 2,
+                                              static_cast<const uint8_t*>(s.dec_k_rope) + size_t(i) * s.n_dec * kRope * 2, s.n_dec,
+                                              s.dec_page_tables, s.dec_table_stride,
+                                              reinterpret_cast<const int32_t*>(arena + pos_off) + size_t(i) * s.n_dec, stream))
+                return rc;
+        if (C > 0)
+            if (int rc = launch_append(ctx, static_cast<const uint8_t*>(s.prompt_latent) + size_t(done) * kLatent * 2,
+                                       static_cast<const uint8_t*>(s.prompt_k_rope) + size_t(done) * kRope * 2, C, s.prompt_page_table, P, stream))
+                return rc;
+        StepArgs a{};
+        a.n_dec = s.n_dec;
+        a.q_dec = static_cast<const uint8_t*>(s.q_dec) + size_t(i) * s.n_dec * kHeads * kDim * 2;
+        a.dec_page_tables = s.dec_page_tables;
+        a.dec_table_stride = s.dec_table_stride;
+        a.chunk_len = C;
+        a.prefix_len = P;
+        a.q_chunk = static_cast<const uint8_t*>(s.q_prompt) + size_t(done) * kHeads * kDim * 2;
+        a.chunk_page_table = s.prompt_page_table;
+        a.out_dec = static_cast<uint8_t*>(s.out_dec) + size_t(i) * s.n_dec * kHeads * kLatent * 2;
+        a.out_chunk = static_cast<uint8_t*>(s.out_prompt) + size_t(done) * kHeads * kLatent * 2;
+        a.lse_dec = s.lse_dec ? s.lse_dec + size_t(i) * s.n_dec * kHeads : nullptr;
+        a.lse_chunk = s.lse_prompt ? s.lse_prompt + size_t(done) * kHeads : nullptr;
+        const PlanEntry& e = steps[i];
+        if (s.n_dec > 0 && !e.plan.items.empty())
+            if (int rc = encode_q_map(&ctx->qd_map, a.q_dec, uint64_t(s.n_dec) * kHeads, 16)) return rc;
+        if (C > 0 && e.plan.n_chunk_items > 0)
+            if (int rc = encode_q_map(&ctx->qc_map, a.q_chunk, uint64_t(C) * kHeads, 64)) return rc;
+        if (C > 0 && e.plan.n_pairs > 0)
+            if (int rc = encode_q_map(&ctx->qp_map, a.q_chunk, uint64_t(C) * kHeads, 128)) return rc;
+        PlanBuffer b;
+        b.dev = const_cast<uint8_t*>(arena) + plan_off[i];
+        if (int rc = launch_step_kernels(ctx, e, b, a, stream, nullptr, nullptr)) return rc;
+        if (ev) KAIROS_CUDA_TRY(cudaEventRecord(ev[2 * i + 1], stream));
+        done += C;
+    }
+    (void)lens0;
+    return KAIROS_OK;
+}
+
+}  // namespace kairos
+
+using namespace kairos;
+
+extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                                   int32_t dec_table_stride, const int32_t* dec_ctx_lens, const void* dec_latent,
+                                   const void* dec_k_rope, int32_t prompt_len, const int32_t* chunk_sizes, int32_t n_steps,
+                                   const void* q_prompt, const void* prompt_latent, const void* prompt_k_rope,
+                                   const int32_t* prompt_page_table, int32_t prompt_table_len, int32_t prefix_len,
+                                   void* out_dec, void* out_prompt, float* lse_dec, float* lse_prompt, double* step_us,
+                                   double* ttft_us, void* cuda_stream) {
+    if (!ctx) return fail(KAIROS_ERR_INVALID_ARG, "ctx is NULL");
+    if (n_dec < 0 || prompt_len < 1 || n_steps < 1 || prefix_len < 0 || !chunk_sizes)
+        return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: bad size or NULL chunk_sizes");
+    if (!q_prompt || !prompt_latent || !prompt_k_rope || !prompt_page_table || !out_prompt)
+        return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: NULL prompt argument");
+    if (n_dec > 0 && (!q_dec || !dec_page_tables || !dec_ctx_lens || !out_dec || dec_table_stride < 1))
+        return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: NULL decode argument");
+    if ((dec_latent == nullptr) != (dec_k_rope == nullptr)) return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: dec_latent and dec_k_rope go together");
+    int64_t total = 0;
+    for (int32_t i = 0; i < n_steps; ++i) {
+        if (chunk_sizes[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: chunk_sizes[" + std::to_string(i) + "] < 1");
+        total += chunk_sizes[i];
+    }
+    if (total != prompt_len) return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: chunk_sizes must sum to prompt_len");
+    if (int64_t(prefix_len) + prompt_len > int64_t(prompt_table_len) * kPage)
+        return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: prompt page table shorter than prefix_len + prompt_len");
+    const bool grow = dec_latent != nullptr;
+    for (int32_t j = 0; j < n_dec; ++j) {
+        if (dec_ctx_lens[j] < (grow ? 0 : 1)) return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: dec_ctx_lens[" + std::to_string(j) + "] too small");
+        if (int64_t(dec_ctx_lens[j]) + (grow ? n_steps : 0) > int64_t(dec_table_stride) * kPage)
+            return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: decode " + std::to_string(j) + " outgrows its page table");
+    }
+    for (const void* ptr : {q_dec, q_prompt, prompt_latent, prompt_k_rope, dec_latent, dec_k_rope, static_cast<const void*>(out_dec),
+                            static_cast<const void*>(out_prompt)})
+        if (reinterpret_cast<uintptr_t>(ptr) % 16) return fail(KAIROS_ERR_INVALID_ARG, "run_schedule: device buffers must be 16-byte aligned");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    KAIROS_CUDA_TRY(cudaSetDevice(ctx->cfg.device));
+
+    const ScheduleArgs s{n_dec, q_dec, dec_page_tables, dec_table_stride, dec_latent, dec_k_rope, q_prompt, prompt_latent, prompt_k_rope,
+                         prompt_page_table, prompt_table_len, prefix_len, out_dec, out_prompt, lse_dec, lse_prompt};
+    // ---- the cached schedule is replayed when every argument, length and chunk size is the same
+    std::vector<uint8_t> key(sizeof(ScheduleArgs) + sizeof(int32_t) * (size_t(n_dec) + n_steps + 2));
+    {
+        uint8_t* k = key.data();
+        std::memset(k, 0, key.size());
+        ScheduleArgs z;
+        std::memset(&z, 0, sizeof(z));  // padding bytes of the struct must compare equal
+        z = s;
+        std::memcpy(k, &z, sizeof(z)); k += sizeof(z);
+        std::memcpy(k, &prompt_len, 4); k += 4;
+        std::memcpy(k, &n_steps, 4); k += 4;
+        if (n_dec) std::memcpy(k, dec_ctx_lens, sizeof(int32_t) * size_t(n_dec));
+        k += sizeof(int32_t) * size_t(n_dec);
+        std::memcpy(k, chunk_sizes, sizeof(int32_t) * size_t(n_steps));
+    }
+    ScheduleCache& sc = ctx->schedule;
+    const bool want_steps = step_us != nullptr;
+    const bool hit = sc.exec && sc.key == key && ctx->use_graph && !want_steps;
+    if (!hit) {
+        // ---- plan every step (a0) and pack the work lists and the decodes' append positions into one arena
+        if (sc.exec) { cudaGraphExecDestroy(sc.exec); sc.exec = nullptr; }
+        sc.key.clear();
+        sc.steps.assign(size_t(n_steps), PlanEntry());
+        sc.plan_off.assign(size_t(n_steps), 0);
+        std::vector<int32_t> lens(dec_ctx_lens, dec_ctx_lens + n_dec);
+        size_t off = 0, ws_needed = 0;
+        int64_t done = 0;
+        sc.kernels = 0;
+        for (int32_t i = 0; i < n_steps; ++i) {
+            if (grow) for (int32_t j = 0; j < n_dec; ++j) lens[j] = dec_ctx_lens[j] + i + 1;
+            PlanEntry& e = sc.steps[i];
+            build_plan(lens.data(), n_dec, chunk_sizes[i], prefix_len + int32_t(done), umma_resident_ctas(ctx), umma_chunk_tile_tokens(),
+                       &e.plan, ctx->force_pairs, pair_tile_tokens());
+            layout_entry(e);
+            sc.plan_off[i] = off;
+            off += (e.total_bytes + 255) / 256 * 256;
+            ws_needed = std::max(ws_needed, kCounterBytes + size_t(e.plan.n_partial_slots) * kPartialSlotBytes);
+            sc.kernels += kernels_of(e.plan) + 1 + (grow && n_dec > 0 ? 1 : 0);
+            done += chunk_sizes[i];
+        }
+        if (ws_needed > ctx->cfg.workspace_bytes)
+            return fail(KAIROS_ERR_WORKSPACE, "run_schedule: workspace too small: need " + std::to_string(ws_needed) + " bytes");
+        sc.pos_off = off;
+        off += (size_t(n_steps) * std::max(n_dec, 1) * 4 + 255) / 256 * 256;
+        KAIROS_CUDA_TRY(cudaStreamSynchronize(stream));  // a previous schedule may still be reading the arena
+        if (sc.cap < off) {
+            if (sc.host) cudaFreeHost(sc.host);
+            if (sc.dev) cudaFree(sc.dev);
+            sc.host = sc.dev = nullptr;
+            sc.cap = 0;
+            KAIROS_CUDA_TRY(cudaMallocHost(&sc.host, off));
+            KAIROS_CUDA_TRY(cudaMalloc(&sc.dev, off));
+            sc.cap = off;
+        }
+        uint8_t* h = static_cast<uint8_t*>(sc.host);
+        for (int32_t i = 0; i < n_steps; ++i) {
+            const PlanEntry& e = sc.steps[i];
+            uint8_t* hp = h + sc.plan_off[i];
+            std::memcpy(hp, e.plan.items.data(), e.items_bytes);
+            if (e.comb_bytes) std::memcpy(hp + e.comb_off, e.plan.combines.data(), e.comb_bytes);
+            if (e.pair_bytes) std::memcpy(hp + e.pair_off, e.plan.pair_items.data(), e.pair_bytes);
+        }
+        int32_t* pos = reinterpret_cast<int32_t*>(h + sc.pos_off);
+        for (int32_t i = 0; i < n_steps; ++i)
+            for (int32_t j = 0; j < n_dec; ++j) pos[size_t(i) * n_dec + j] = dec_ctx_lens[j] + i;  // the slot of step i's new token
+        KAIROS_CUDA_TRY(cudaMemcpyAsync(sc.dev, sc.host, off, cudaMemcpyHostToDevice, stream));
+        // ---- one CUDA graph for the whole schedule (programmatic launch edges kept)
+        if (ctx->use_graph && !want_steps && ctx->capture_stream &&
+            cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const int rc = enqueue_schedule(ctx, s, sc.steps, lens, chunk_sizes, n_steps, static_cast<const uint8_t*>(sc.dev), sc.plan_off,
+                                            sc.pos_off, ctx->capture_stream, nullptr);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(ctx->capture_stream, &graph);
+            bool ok = rc == KAIROS_OK && ce == cudaSuccess && graph != nullptr;
+            if (ok) ok = cudaGraphInstantiate(&sc.exec, graph, 0) == cudaSuccess;
+            if (graph) cudaGraphDestroy(graph);
+            if (!ok) {
+                cudaGetLastError();
+                sc.exec = nullptr;
+            } else {
+                sc.key = key;
+            }
+        }
+    }
+    // ---- run it: TTFT_dec (Eq. 6's left-hand side, measured) is the device time from the first append to the last kernel
+    const bool timed = ttft_us || step_us;
+    std::vector<cudaEvent_t> ev;
+    struct EvGuard {
+        std::vector<cudaEvent_t>& v;
+        ~EvGuard() { for (auto e : v) cudaEventDestroy(e); }
+    } guard{ev};
+    const int n_ev = timed ? 2 + (want_steps ? 2 * n_steps : 0) : 0;
+    for (int i = 0; i < n_ev; ++i) {
+        cudaEvent_t e;
+        KAIROS_CUDA_TRY(cudaEventCreate(&e));
+        ev.push_back(e);
+    }
+    if (timed) KAIROS_CUDA_TRY(cudaEventRecord(ev[0], stream));
+    if (sc.exec && !want_steps) {
+        KAIROS_CUDA_TRY(cudaGraphLaunch(sc.exec, stream));
+    } else {
+        std::vector<int32_t> lens(dec_ctx_lens, dec_ctx_lens + n_dec);
+        if (int rc = enqueue_schedule(ctx, s, sc.steps, lens, chunk_sizes, n_steps, static_cast<const uint8_t*>(sc.dev), sc.plan_off,
+                                      sc.pos_off, stream, want_steps ? ev.data() + 2 : nullptr))
+            return rc;
+    }
+    ctx->last_info[4] = sc.kernels;
+    ctx->last_info[8] = (sc.exec && !want_steps) ? 1 : 0;
+    if (timed) {
+        KAIROS_CUDA_TRY(cudaEventRecord(ev[1], stream));
+        KAIROS_CUDA_TRY(cudaEventSynchronize(ev[1]));
+        float ms = 0.f;
+        KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+        if (ttft_us) *ttft_us = double(ms) * 1e3;
+        for (int32_t i = 0; want_steps && i < n_steps; ++i) {
+            KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, ev[2 + 2 * i], ev[3 + 2 * i]));
+            step_us[i] = double(ms) * 1e3;
+        }
+    }
+    return KAIROS_OK;
+}
+
+namespace kairos {
 }  // namespace kairos
 
 using namespace kairos;
@@ -374,6 +609,9 @@ int kairos_destroy(kairos_ctx* ctx) {
             if (b.last_use) cudaEventDestroy(b.last_use);
         }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
+    if (ctx->schedule.exec) cudaGraphExecDestroy(ctx->schedule.exec);
+    if (ctx->schedule.host) cudaFreeHost(ctx->schedule.host);
+    if (ctx->schedule.dev) cudaFree(ctx->schedule.dev);
     if (ctx->table_buf) cudaFree(ctx->table_buf);
     if (ctx->flush_buf) cudaFree(ctx->flush_buf);
     for (auto e : ctx->prof_events) cudaEventDestroy(e);

@@ -120,6 +120,19 @@ struct PlanEntry {
     int cur = 0;
 };
 
+// kairos_run_schedule: the plans of every step of the last schedule, their device copies and the captured graph
+struct ScheduleCache {
+    std::vector<uint8_t> key;          // every argument, length and chunk size of the schedule the graph was captured for
+    std::vector<PlanEntry> steps;
+    std::vector<size_t> plan_off;
+    size_t pos_off = 0;
+    void* host = nullptr;              // pinned arena: work lists of every step | append positions of the decodes
+    void* dev = nullptr;
+    size_t cap = 0;
+    cudaGraphExec_t exec = nullptr;
+    int kernels = 0;
+};
+
 struct QMapCache {  // a q tensor map stays valid while (pointer, rows) do not change
     const void* ptr = nullptr;
     uint64_t rows = 0;
@@ -146,6 +159,7 @@ struct kairos_ctx {
     kairos::PlanEntry plans[kPlanEntries];
     uint64_t plan_clock = 0;
     kairos::HostStage host_stage;
+    kairos::ScheduleCache schedule;
     int64_t last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     bool profile = false;         // bracket the attention kernels with events (kairos_profile_enable)
     std::vector<cudaEvent_t> prof_events;  // pairs: [2i] start, [2i+1] stop

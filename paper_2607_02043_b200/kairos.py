@@ -89,6 +89,9 @@ _lib.kairos_predict_step.restype = _c.c_double
 _lib.kairos_decide.argtypes = [_c.POINTER(StepModel), _c.POINTER(PrefillModel), _c.POINTER(DecideInput), _vp, _i32,
                                _c.POINTER(DecideOutput)]
 _lib.kairos_decide.restype = _c.c_int
+_lib.kairos_run_schedule.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _vp, _i32, _i32,
+                                     _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.kairos_run_schedule.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
 _lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
@@ -99,7 +102,7 @@ _lib.kairos_version.restype = _c.c_char_p
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
-           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide",
+           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -222,6 +225,34 @@ class Kairos:
                                            hp(out_chunk), None, None, _c.byref(h2d), _c.byref(d2h),
                                            _stream_ptr(stream)))
         return int(h2d.value), int(d2h.value)
+
+    # -- SURVEY.md 8(f) row 3
+    def run_schedule(self, q_dec, dec_page_tables, dec_ctx_lens, dec_latent, dec_k_rope, chunk_sizes, q_prompt,
+                     prompt_latent, prompt_k_rope, prompt_page_table, prefix_len: int = 0, out_dec=None, out_prompt=None,
+                     lse_dec=None, lse_prompt=None, time_steps: bool = False, timed: bool = True, stream=None):
+        """kairos_run_schedule.  Returns (out_dec [m,B,16,512], out_prompt [l,16,512], lse_dec, lse_prompt, ttft_us, step_us)."""
+        dev = self.pool.device
+        lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        cs = np.ascontiguousarray(np.asarray(chunk_sizes, dtype=np.int32))
+        B, m, L = int(lens.shape[0]), int(cs.shape[0]), int(cs.sum())
+        if out_dec is None:
+            out_dec = torch.empty((m, B, 16, 512), dtype=torch.bfloat16, device=dev)
+        if out_prompt is None:
+            out_prompt = torch.empty((L, 16, 512), dtype=torch.bfloat16, device=dev)
+        if lse_dec is None:
+            lse_dec = torch.empty((m, B, 16), dtype=torch.float32, device=dev)
+        if lse_prompt is None:
+            lse_prompt = torch.empty((L, 16), dtype=torch.float32, device=dev)
+        ttft = _c.c_double(0.0)
+        steps = np.zeros(m, dtype=np.float64)
+        stride = int(dec_page_tables.shape[1]) if B else 1
+        _check(_lib.kairos_run_schedule(self._h, B, _dp(q_dec), _dp(dec_page_tables), stride, lens.ctypes.data_as(_vp),
+                                        _dp(dec_latent), _dp(dec_k_rope), L, cs.ctypes.data_as(_vp), m, _dp(q_prompt),
+                                        _dp(prompt_latent), _dp(prompt_k_rope), _dp(prompt_page_table),
+                                        int(prompt_page_table.numel()), int(prefix_len), _dp(out_dec), _dp(out_prompt),
+                                        _dp(lse_dec), _dp(lse_prompt), steps.ctypes.data_as(_vp) if time_steps else None,
+                                        _c.byref(ttft) if (timed or time_steps) else None, _stream_ptr(stream)))
+        return out_dec, out_prompt, lse_dec, lse_prompt, float(ttft.value), (steps if time_steps else None)
 
     # -- a11
     def step_latency_table(self, Bs: Sequence[int], Ks: Sequence[int], Cs: Sequence[int], prefix_len: int = 0,
