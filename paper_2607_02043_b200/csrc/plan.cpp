@@ -31,7 +31,8 @@ constexpr int64_t kPairPageCycles = 1800;
 constexpr int64_t kPairItemCycles = 27000;
 constexpr int64_t kDecPageCycles = 2600;
 constexpr int64_t kDecPageHbmSmCycles = 4260;
-constexpr int64_t kGen1PairPageSmCycles = 7570;
+constexpr int32_t kGen1MaxTiles = 16;
+constexpr int64_t kGen1MaxDecPages = 512;  // ... and only beside little decode work (long decodes want every SM streaming early)
 constexpr int64_t kKernelFloorCycles = 25000;  // launch, first loads, first chain, epilogue of a persistent kernel (~12.7 us)
 
 // When the chunk runs on the pair kernel, clusters are launched for EVERY SM pair (up to one per tile) and the two grids
@@ -50,6 +51,10 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
     for (int32_t i = 0; i < n_dec; ++i) dec_pages += ceil_div(dec_ctx_lens[i], kPage);
     const int32_t max_pairs = std::min(n_tiles, ctas / 2);
     if (max_pairs < 1) return;
+    // A chunk of at most kGen1MaxTiles 8-token tiles keeps too few SM pairs busy: it rides in the decode queue as 4-token
+    // gen-1 tiles (KV-split across CTAs).  Anything larger runs on clusters: measured over a (B, K, C, P) grid off the five
+    // BASELINE configs (profiles/r02_planner_offpoints.md), gen-1 tiles lose up to 1.9x there and win only below ~128 tokens.
+    if (pair_mode == -1 && n_tiles <= kGen1MaxTiles && dec_pages <= kGen1MaxDecPages) return;
     const int64_t work_c = pair_pages * kPairPageCycles + int64_t(n_tiles) * kPairItemCycles;
     int32_t dec_ctas = 0;
     int32_t n_p = max_pairs;
@@ -76,13 +81,16 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
         if (pair_mode > 0) {
             best_c = std::min({pair_mode, max_pairs, (ctas - 2) / 2});
             if (pair_mode >= max_pairs) { best_c = 0; best_n = max_pairs; }
-        } else if (ceil_div(work_c, (td_all + kKernelFloorCycles) * 8 / 10) <= std::min(max_pairs, 48)) {
-            // a chunk that is small beside the decode work (measured, profiles/r01_bench_gen3.md: configs[3] C <= 1024): just
-            // enough clusters to finish it a little before the decodes would, launched first; the decode grid (the
+        } else if (ceil_div(work_c, (td_all + kKernelFloorCycles) * 4 / 10) <= std::min(max_pairs, 48)) {
+            // a chunk that is small beside the decode work (measured: configs[3] C <= 1024): just enough clusters to finish
+            // it within ~40 % of the decodes' time, launched first (fewer clusters gain 1-3 % when the estimate is right and
+            // lose > 10 % when it is not, profiles/r02_planner_offpoints.md); the decode grid (the
             // decode-only instantiation with the deeper ring) streams on the other SMs and inherits theirs
-            best_n = std::max(std::min(8, max_pairs), ceil_div(work_c, (td_all + kKernelFloorCycles) * 8 / 10));
+            best_n = std::max(std::min(8, max_pairs), ceil_div(work_c, (td_all + kKernelFloorCycles) * 4 / 10));
         } else {
-            for (int32_t c = 1; c <= std::min(max_pairs, (ctas - 2) / 2); ++c) {
+            // decode first only pays when the tiles outnumber the SM pairs at least twice (measured: with fewer tiles the
+            // clusters that start late run alone at the end)
+            for (int32_t c = 1; n_tiles >= ctas && c <= std::min(max_pairs, (ctas - 2) / 2); ++c) {
                 const int64_t t = t_dec_first(c);
                 if (best < 0 || t < best) { best = t; best_c = c; best_n = 0; }
             }
@@ -90,9 +98,6 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
                 const int64_t t = t_pairs_first(n);
                 if (best < 0 || t < best) { best = t; best_c = 0; best_n = n; }
             }
-            // one queue for everything (gen-1 tiles ride in the decode grid) unless sharing is clearly faster
-            const int64_t t_gen1 = (dec_pages * kDecPageHbmSmCycles + pair_pages * kGen1PairPageSmCycles) / ctas;
-            if (best * 10 > t_gen1 * 9) return;
             // a chunk that dwarfs the decode work: a static share idles (tile quantisation, contention) more than the overlap
             // gains; measured on configs[2] and [4] (profiles/r01_bench_gen3.md): the decode CTAs fill the clusters' tail instead
             if (work_c / max_pairs >= 4 * td_all) { best_c = 0; best_n = max_pairs; }
@@ -100,7 +105,7 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
         if (best_c > 0) dec_ctas = ctas - 2 * best_c;
         else n_p = best_n;
     } else if (pair_mode < 0) {
-        if (work_c / max_pairs > pair_pages * kGen1PairPageSmCycles / ctas) return;  // few short tiles: gen-1 tiles use every SM
+        // chunk only: one cluster per tile, up to one per SM pair
     } else {
         n_p = std::min(pair_mode, max_pairs);
     }

@@ -19,6 +19,7 @@ from . import kairos as K
 
 CONFIG3 = dict(Bs=[256], Ks=[2048], Cs=[0, 256, 512, 1024, 2048, 4096, 8192])
 GRID = dict(Bs=[16, 64, 256], Ks=[512, 2048, 8192], Cs=[0, 256, 512, 1024, 2048, 4096])
+GRID_PREFIX = dict(Bs=[16, 64, 256], Ks=[2048], Cs=[256, 1024, 2048], prefix=4096)  # later chunks of a request
 # the paper's own microbenchmark grid (Fig. 1 caption PAPER.md:159): its chi counts B + C tokens
 PAPER_GRID = dict(Bs=[4, 8, 16, 32], Ks=[842, 998, 3569, 13968, 14013], chis=[128, 256, 512, 1024, 2048])
 
@@ -43,6 +44,23 @@ def run_table(ctx, Bs, Ks, Cs, prefix=0, warmup=5, reps=20, flush=True) -> dict:
             "wall_s": round(time.time() - t0, 2)}
 
 
+def table_samples(table: dict, keys=("grid", "grid_prefix", "configs3")):
+    """Rows (B, Kd, C, P, T_us) of a table written by this module: the samples kairos_fit_latency_model takes."""
+    rows = []
+    for key in keys:
+        g = table.get(key)
+        if g is None:
+            continue
+        m = np.array(g["median_us"])
+        for i, B in enumerate(g["Bs"]):
+            for j, Kc in enumerate(g["Ks"]):
+                for k, C in enumerate(g["Cs"]):
+                    if B == 0 and C == 0:
+                        continue
+                    rows.append((B, B * Kc, C, g["prefix_len"] if C > 0 else 0, float(m[i, j, k])))
+    return np.array(rows, dtype=np.float64)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", required=True)
@@ -55,10 +73,11 @@ def main():
     out = {"library": K.version(), "device": torch.cuda.get_device_name(0),
            "units": "one layer's attention, microseconds; K = per-decode context; C = prefill tokens only (include/kairos.h)"}
     if args.grid == "default":
-        n = max(pages_needed(**CONFIG3), pages_needed(**GRID))
+        n = max(pages_needed(**CONFIG3), pages_needed(**GRID), pages_needed(**GRID_PREFIX))
         ctx = make_context(n, 256, 8192)
         out["configs3"] = run_table(ctx, **CONFIG3, warmup=args.warmup, reps=args.reps, flush=not args.no_flush)
         out["grid"] = run_table(ctx, **GRID, warmup=args.warmup, reps=args.reps, flush=not args.no_flush)
+        out["grid_prefix"] = run_table(ctx, **GRID_PREFIX, warmup=args.warmup, reps=args.reps, flush=not args.no_flush)
     else:
         # Fig. 1's setting, attention only: B decodes with K cached tokens each, a batch of chi tokens of which chi - B are
         # prefill, five successive chunks of the same request (the prefix grows by one chunk each time)

@@ -106,7 +106,8 @@ def test_plan_with_pair_kernel(lens, C, P, pair_mode):
 def test_planner_policy_for_the_pair_kernel():
     n = lambda lens, C, P: K.plan_dump(lens, C, P, 148, pair_mode=-1, with_pairs=True)[2]
     assert n([64, 128, 200, 256], 64, 128) == 0          # configs[0]
-    assert 8 <= n([2048] * 256, 512, 0) <= 16            # small chunk beside many decodes: a few clusters first, decode grid behind
+    assert 8 <= n([2048] * 256, 512, 0) <= 32            # small chunk beside many decodes: a few clusters first, decode grid behind
+    assert n([3569] * 32, 96, 0) >= 8 and n([842] * 4, 124, 0) == 0   # gen-1 tiles only for a tiny chunk beside little decode work
     assert n([2048] * 256, 8192, 0) > 40                 # tensor-bound: most SM pairs go to the chunk
     assert n([32768] * 32, 4096, 28672) > 40             # configs[4]
     assert n([], 8192, 0) == 74
