@@ -245,15 +245,14 @@ class Point:
             R.out_chunk = torch.empty((inp.chunk_len, 16, 512), dtype=torch.bfloat16, device=dev)
             R.lse_dec = torch.empty((inp.n_dec, 16), dtype=torch.float32, device=dev)
             R.lse_chunk = torch.empty((inp.chunk_len, 16), dtype=torch.float32, device=dev)
+            # the step as a serving loop issues it: the same buffers every time, marshalled once (Kairos.bind_step)
+            R.bound = R.ctx.bind_step(R.q_dec, R.dec_pt, inp.dec_ctx_lens, R.q_chunk, R.chunk_pt, inp.chunk_len, inp.prefix_len,
+                                      R.out_dec, R.out_chunk, R.lse_dec, R.lse_chunk, R.latent, R.k_rope)
             self.reps.append(R)
         self.lens = inp.dec_ctx_lens
 
     def step(self, R):
-        inp = self.inp
-        if inp.chunk_len:
-            R.ctx.append_latent(R.latent, R.k_rope, R.chunk_pt, inp.prefix_len)
-        R.ctx.mixed_step(R.q_dec, R.dec_pt, self.lens, R.q_chunk, R.chunk_pt, inp.chunk_len, inp.prefix_len,
-                         out_dec=R.out_dec, out_chunk=R.out_chunk, lse_dec=R.lse_dec, lse_chunk=R.lse_chunk)
+        R.bound.run()  # kairos_append_latent(chunk) + kairos_mixed_step
 
     def warm(self, n):
         for i in range(max(n, 3) * self.replicas):  # every copy plans, hits its cache and captures its graph before timing

@@ -67,7 +67,7 @@ struct PairSmall {
     uint64_t p_empty[2];   // arrived by the O-CTA's tcgen05.commit when PV(g) has consumed P buffer g & 1
     uint64_t fin_empty;    // arrived by the O-CTA's epilogue warps: linv[] may be overwritten
     uint64_t item_empty[2];
-    uint64_t qst_full[2];  // Q chunk landed in staging buffer (TMA)
+    uint64_t qst_full[4];  // Q chunk landed in a landing buffer (TMA)
     // O-CTA
     uint64_t v_full[kStages], v_empty[kStages], p_full[2], corr_done[2], pv_done[2], o_full, o_empty, fin_full;
     // both
@@ -132,50 +132,59 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi) {
 // the O-CTA.  g counts pages over the whole kernel (S buffer / P buffer = g & 1), `it` counts items.
 // ------------------------------------------------------------------------------------------------------------
 // S-CTA: Q tile of item `it` -> TMEM (the 128 row-owning threads).  Waits for the S-MMAs of item it - 1 (q_free).
-__device__ __forceinline__ void sc_load_q(PairSmall* sm, const WorkItem& w, const PairParams& p, const CUtensorMap* qmap, uint32_t tmem,
-                                          int row, int q4, int lane, uint32_t& qcount, uint32_t it) {
+// The tile [128 rows x 576] moves through FOUR 16 KB landing buffers, one TMA box (64 dims x 128 rows, SWIZZLE_128B, rows past
+// the chunk's end zero-filled) per 64-dim chunk: the two dedicated Q buffers and the two P staging buffers, which are idle
+// between the last P of one item and the first P of the next.  `g` = global page counter of the item's first page: P
+// buffer g & 1 last carried page g - 2 and buffer (g + 1) & 1 page g - 1; each may be overwritten once the O-CTA's PV of
+// that page has retired (p_empty: by then the bulk copy that read the buffer has completed as well).  With 3-4 boxes in
+// flight the load is ~3k cycles instead of ~7k with two (it is the serial part of every tile boundary).
+__device__ __forceinline__ void sc_load_q(PairSmall* sm, uint8_t* pstage, const WorkItem& w, const PairParams& p, const CUtensorMap* qmap,
+                                          uint32_t tmem, int row, int q4, int lane, uint32_t& qcount, uint32_t it, uint32_t g) {
     const uint32_t lane_base = uint32_t(q4 * 32) << 16;
     uint8_t* qst = reinterpret_cast<uint8_t*>(sm) - kOffSmallO + kOffQStage;
+    uint8_t* buf[4] = {qst, qst + 16384, pstage + (g & 1u) * kPBytes, pstage + ((g + 1u) & 1u) * kPBytes};
     const int row0 = w.q_index * kHeads;
-    if (row == 0) {  // the first two Q chunks start moving before the previous item's S-MMAs have retired
-        for (int c = 0; c < 2; ++c) {
-            mbar_arrive_expect_tx(&sm->qst_full[c], 16384);
-            tma_load_2d(qst + c * 16384, qmap, &sm->qst_full[c], c * 64, row0, kEvictFirst);
-        }
+    auto issue = [&](int c) {  // row 0 only
+        const int bi = c & 3;
+        if (c == 2) mbar_wait_cluster(&sm->p_empty[g & 1u], ((g >> 1) & 1u) ^ 1u);
+        if (c == 3) mbar_wait_cluster(&sm->p_empty[(g + 1u) & 1u], (((g + 1u) >> 1) & 1u) ^ 1u);
+        if (c == 2 || c == 3) fence_proxy_async_smem();  // the buffer's last writes came from this CTA's threads (generic proxy)
+        mbar_arrive_expect_tx(&sm->qst_full[bi], 16384);
+        tma_load_2d(buf[bi], qmap, &sm->qst_full[bi], c * 64, row0, kEvictFirst);
+    };
+    if (row == 0) {  // the first boxes start moving before the previous item's S-MMAs have retired
+        issue(0);
+        issue(1);
+        issue(2);
     }
     mbar_wait(&sm->q_free, (it & 1) ^ 1);  // previous item's S-MMAs have retired
     tc_fence_after();
-    {
-        // Q tile [128 rows x 576] -> TMEM through two 16 KB staging buffers: one TMA box (64 dims x 128 rows, SWIZZLE_128B,
-        // rows past the chunk's end zero-filled) per 64-dim chunk; each thread then reads its own row's 128 B (conflict
-        // free) and stores 32 TMEM columns.  (Per-thread global loads of a row cost ~10k cycles: 32 lines per LDG.)
 #pragma unroll 1
-        for (int c = 0; c < 9; ++c) {
-            const uint32_t qb = c & 1;
-            mbar_wait(&sm->qst_full[qb], (qcount >> qb) & 1);  // qcount: one phase-parity bit per staging buffer
-            qcount ^= 1u << qb;
-            const uint8_t* src = qst + qb * 16384 + row * 128;
-            uint32_t r[32];
+    for (int c = 0; c < 9; ++c) {
+        const uint32_t bi = c & 3;
+        mbar_wait(&sm->qst_full[bi], (qcount >> bi) & 1);  // qcount: one phase-parity bit per landing buffer
+        qcount ^= 1u << bi;
+        // each thread reads its own row's 128 B (conflict free) and stores 32 TMEM columns
+        const uint8_t* src = buf[bi] + row * 128;
+        uint32_t r[32];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const uint4 v = *reinterpret_cast<const uint4*>(src + ((j ^ (row & 7)) << 4));
-                r[4 * j + 0] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
-            }
-            tmem_st32(tmem + lane_base + kColQ + 32 * c, r);
-            if (c + 2 < 9) {
-                asm volatile("bar.sync 3, 128;" ::: "memory");  // every row has read this buffer
-                if (row == 0) {
-                    mbar_arrive_expect_tx(&sm->qst_full[qb], 16384);
-                    tma_load_2d(qst + qb * 16384, qmap, &sm->qst_full[qb], (c + 2) * 64, row0, kEvictFirst);
-                }
+        for (int j = 0; j < 8; ++j) {
+            const uint4 v = *reinterpret_cast<const uint4*>(src + ((j ^ (row & 7)) << 4));
+            r[4 * j + 0] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
+        }
+        tmem_st32(tmem + lane_base + kColQ + 32 * c, r);
+        if (c == 0 || c + 4 < 9) {
+            asm volatile("bar.sync 3, 128;" ::: "memory");  // every row has read this buffer
+            if (row == 0) {
+                if (c == 0) issue(3);  // the fourth buffer frees last (PV of the previous item's last page)
+                if (c + 4 < 9) issue(c + 4);
             }
         }
-        tmem_wait_st();
     }
+    tmem_wait_st();
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm->q_ready);
-
 }
 
 __device__ __forceinline__ WorkItem sc_fetch_item(PairSmall* sm, const PairParams& p, int lane, uint32_t it, int* idx_out) {
@@ -294,7 +303,7 @@ __device__ __forceinline__ void sc_softmax_item(PairSmall* sm, uint8_t* pstage, 
     // loaded only now, after the last P and 1/l have left, so that the ~7k-cycle load overlaps the O-CTA's last PV and its
     // epilogue (which otherwise stall the next item's first pages) instead of delaying them.
     *next = sc_fetch_item(sm, p, lane, it + 1, next_idx);
-    if (*next_idx >= 0) sc_load_q(sm, *next, p, qmap, tmem, row, q4, lane, qcount, it + 1);
+    if (*next_idx >= 0) sc_load_q(sm, pstage, *next, p, qmap, tmem, row, q4, lane, qcount, it + 1, g);
 }
 
 // S-CTA, MMA warp (converged; one elected lane issues)
@@ -502,8 +511,7 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             mbar_init(&sm->item_full[i], 1);
             mbar_init(&sm->item_empty[i], 11);  // S-CTA: MMA warp + 4 softmax warps; O-CTA: producer + MMA + 4 epilogue warps
         }
-        mbar_init(&sm->qst_full[0], 1);
-        mbar_init(&sm->qst_full[1], 1);
+        for (int i = 0; i < 4; ++i) mbar_init(&sm->qst_full[i], 1);
         mbar_init(&sm->q_ready, 4);
         mbar_init(&sm->q_free, 1);
         mbar_init(&sm->fin_empty, 4);
@@ -589,7 +597,7 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             // S-CTA row-owning warps: item fetch and Q load run one item ahead of the softmax
             int idx;
             WorkItem w = sc_fetch_item(sm, p, lane, 0, &idx);
-            if (idx >= 0) sc_load_q(sm, w, p, &q_map, tmem, row, q4, lane, qcount, 0);
+            if (idx >= 0) sc_load_q(sm, base + kOffPStage, w, p, &q_map, tmem, row, q4, lane, qcount, 0, 0);
             for (uint32_t it = 0; idx >= 0; ++it) {
                 WorkItem nxt{};
                 int nidx = -1;

@@ -207,6 +207,14 @@ class Kairos:
                                       _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk), _stream_ptr(stream)))
         return out_dec, out_chunk, lse_dec, lse_chunk
 
+    def bind_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
+                  prefix_len: int, out_dec, out_chunk, lse_dec=None, lse_chunk=None, chunk_latent=None, chunk_k_rope=None):
+        """Marshals the arguments of a step ONCE (a serving loop passes the same buffers step after step) and returns a
+        BoundStep whose run() makes the two C calls -- kairos_append_latent for the chunk (when chunk_latent / chunk_k_rope are
+        given) and kairos_mixed_step -- with no per-call tensor inspection.  The tensors are kept alive by the object."""
+        return BoundStep(self, q_dec, dec_page_tables, dec_ctx_lens, q_chunk, chunk_page_table, chunk_len, prefix_len,
+                         out_dec, out_chunk, lse_dec, lse_chunk, chunk_latent, chunk_k_rope)
+
     def mixed_step_host(self, q_dec: np.ndarray, dec_page_tables: np.ndarray, dec_ctx_lens: np.ndarray,
                         q_chunk: np.ndarray, chunk_latent: np.ndarray, chunk_k_rope: np.ndarray,
                         chunk_page_table: np.ndarray, chunk_len: int, prefix_len: int, out_dec: np.ndarray,
@@ -285,6 +293,36 @@ class Kairos:
     def debug_set(self, key: str, value: int) -> None:
         """Test-only knobs (kairos_debug_set)."""
         _check(_lib.kairos_debug_set(self._h, key.encode(), int(value)))
+
+
+class BoundStep:
+    """Pre-marshalled (append, mixed step) pair: see Kairos.bind_step.  Argument marshalling only."""
+
+    def __init__(self, ctx, q_dec, dec_page_tables, dec_ctx_lens, q_chunk, chunk_page_table, chunk_len, prefix_len, out_dec,
+                 out_chunk, lse_dec, lse_chunk, chunk_latent, chunk_k_rope):
+        self._keep = (ctx, q_dec, dec_page_tables, q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk,
+                      chunk_latent, chunk_k_rope)
+        self._lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        B, C = int(self._lens.shape[0]), int(chunk_len)
+        stride = int(dec_page_tables.shape[1]) if B else 1
+        self._h = ctx._h
+        self._step_args = (B, _dp(q_dec), _dp(dec_page_tables), stride, self._lens.ctypes.data_as(_vp), C, int(prefix_len),
+                           _dp(q_chunk), _dp(chunk_page_table), int(chunk_page_table.numel()) if C else 0, _dp(out_dec),
+                           _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk))
+        self._append_args = None
+        if C and chunk_latent is not None:
+            self._append_args = (_dp(chunk_latent), _dp(chunk_k_rope), C, _dp(chunk_page_table), int(chunk_page_table.numel()),
+                                 int(prefix_len))
+
+    def run(self, stream: Optional[torch.cuda.Stream] = None) -> None:
+        sp = _stream_ptr(stream)
+        if self._append_args is not None:
+            rc = _lib.kairos_append_latent(self._h, *self._append_args, sp)
+            if rc:
+                raise KairosError(rc)
+        rc = _lib.kairos_mixed_step(self._h, *self._step_args, sp)
+        if rc:
+            raise KairosError(rc)
 
 
 def plan_dump(dec_ctx_lens: Sequence[int], chunk_len: int, prefix_len: int, n_ctas: int = 148, pair_mode: int = 0,

@@ -264,6 +264,17 @@ def test_plan_cache_and_graph_replay_match_direct_launch():
             for x, y in zip(first, got):
                 assert np.array_equal(x, y), (cfg, pairs, rep)
         assert states[0] == (0, 0) and states[1][0] == 2 and states[-1] == (2, 1), states
+        # the pre-marshalled form of the same calls (Kairos.bind_step) gives the same bits
+        import torch
+        od, oc, ld, lc = (torch.full_like(t, float("nan")) for t in run.out)
+        bound = run.ctx.bind_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, inp.chunk_len, inp.prefix_len,
+                                  od, oc, ld, lc, run.latent, run.k_rope)
+        for _ in range(3):
+            bound.run()
+        torch.cuda.synchronize()
+        f = lambda t: W.bf16_bits_to_f32(run.K.bf16_bits(t))
+        for x, y in zip(first, (f(od), f(oc), ld.cpu().numpy(), lc.cpu().numpy())):
+            assert np.array_equal(x, y)
         plain = Hp.GpuRun(inp, pairs=pairs, knobs=dict(graph=0, plan_cache=0, copy_stream=0))
         plain.append()
         got = plain.step()
