@@ -345,6 +345,24 @@ int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const
                         void* cuda_stream);
 
 /*
+ * the projections either side of the attention (absorbed MLA of DeepSeek-V2-Lite; the
+ * math is SURVEY.md 8(c)'s definition): per head h,
+ *   kairos_absorb_q     q_out[j][h][0:512]   = sum_k q_nope[j][h][k] * w_uk_t[h][d][k]   (128 -> 512, the key up-projection
+ *                       q_out[j][h][512:576] = q_rope[j][h][0:64]                         folded into the query), producing the
+ *                       q rows kairos_mixed_step takes;
+ *   kairos_project_out  v_out[j][h][e]       = sum_d o_lat[j][h][d] * w_uv_t[h][e][d]    (512 -> 128, the value up-projection)
+ *                       applied to kairos_mixed_step's outputs.
+ * bf16 operands, fp32 accumulation on tcgen05 (TMEM accumulator), bf16 round-to-nearest-even results.
+ *   q_nope  DEVICE bf16 [n][16][128]   q_rope DEVICE bf16 [n][16][64]   w_uk_t DEVICE bf16 [16][512][128]
+ *   q_out   DEVICE bf16 [n][16][576]   o_lat  DEVICE bf16 [n][16][512]  w_uv_t DEVICE bf16 [16][128][512]
+ *   v_out   DEVICE bf16 [n][16][128]   (all 16-byte aligned; weights are stored [head][output dim][input dim])
+ * Asynchronous on `cuda_stream`.  n == 0 is a no-op.  Errors: INVALID_ARG, CUDA.
+ */
+int kairos_absorb_q(kairos_ctx* ctx, const void* q_nope, const void* q_rope, const void* w_uk_t, int32_t n, void* q_out,
+                    void* cuda_stream);
+int kairos_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, int32_t n, void* v_out, void* cuda_stream);
+
+/*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
  *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;

@@ -660,6 +660,27 @@ int kairos_append_decode_tokens(kairos_ctx* ctx, const void* latent, const void*
                                 static_cast<cudaStream_t>(cuda_stream));
 }
 
+int kairos_absorb_q(kairos_ctx* ctx, const void* q_nope, const void* q_rope, const void* w_uk_t, int32_t n, void* q_out,
+                    void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (n < 0) return fail(KAIROS_ERR_INVALID_ARG, "n < 0");
+    if (n == 0) return KAIROS_OK;
+    if (!q_nope || !q_rope || !w_uk_t || !q_out) return fail(KAIROS_ERR_INVALID_ARG, "NULL pointer");
+    for (const void* p : {q_nope, q_rope, w_uk_t, static_cast<const void*>(q_out)})
+        if (reinterpret_cast<uintptr_t>(p) % 16) return fail(KAIROS_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
+    return launch_absorb_q(ctx, q_nope, q_rope, w_uk_t, n, q_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int kairos_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, int32_t n, void* v_out, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (n < 0) return fail(KAIROS_ERR_INVALID_ARG, "n < 0");
+    if (n == 0) return KAIROS_OK;
+    if (!o_lat || !w_uv_t || !v_out) return fail(KAIROS_ERR_INVALID_ARG, "NULL pointer");
+    for (const void* p : {o_lat, w_uv_t, static_cast<const void*>(v_out)})
+        if (reinterpret_cast<uintptr_t>(p) % 16) return fail(KAIROS_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
+    return launch_project_out(ctx, o_lat, w_uv_t, n, v_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int kairos_gather_latent(kairos_ctx* ctx, const int32_t* page_table, int32_t table_len, int32_t n_tokens, void* out,
                          void* cuda_stream) {
     if (int rc = check_ctx(ctx)) return rc;

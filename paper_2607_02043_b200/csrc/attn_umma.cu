@@ -726,17 +726,22 @@ int umma_resident_ctas(const kairos_ctx* ctx) { return ctx->sm_count; }
 // q viewed as [rows][576] bf16 with boxes of 64 dims x box_rows rows.  cuTensorMapEncodeTiled costs a few microseconds of
 // host time, so the encoded map is kept while the caller passes the same buffer.
 int encode_q_map(QMapCache* cache, const void* ptr, uint64_t rows, uint32_t box_rows) {
+    return encode_2d_map(cache, ptr, kDim, rows, kTokenBytes, 64, box_rows);
+}
+
+int encode_2d_map(QMapCache* cache, const void* ptr, uint64_t inner, uint64_t rows, uint64_t row_stride_bytes, uint32_t box_inner,
+                  uint32_t box_rows) {
     if (cache->ptr == ptr && cache->rows == rows) return KAIROS_OK;
-    cuuint64_t dims[2] = {cuuint64_t(kDim), rows};
-    cuuint64_t strides[1] = {cuuint64_t(kTokenBytes)};
-    cuuint32_t box[2] = {64, box_rows};
+    cuuint64_t dims[2] = {cuuint64_t(inner), rows};
+    cuuint64_t strides[1] = {cuuint64_t(row_stride_bytes)};
+    cuuint32_t box[2] = {box_inner, box_rows};
     cuuint32_t es[2] = {1, 1};
     CUresult r = g_encode(&cache->map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         cache->ptr = nullptr;
-        return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: " + std::to_string(int(r)));
+        return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)));
     }
     cache->ptr = ptr;
     cache->rows = rows;

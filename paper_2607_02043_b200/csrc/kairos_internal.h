@@ -133,7 +133,7 @@ struct ScheduleCache {
     int kernels = 0;
 };
 
-struct QMapCache {  // a q tensor map stays valid while (pointer, rows) do not change
+struct QMapCache {  // a tensor map stays valid while (pointer, rows) do not change
     const void* ptr = nullptr;
     uint64_t rows = 0;
     CUtensorMap map;
@@ -148,6 +148,7 @@ struct kairos_ctx {
     CUtensorMap pool_map2, pool_map1;  // boxes of 2 latent chunks / 1 chunk of a page: the slot ring of kairos_mixed_kernel
     CUtensorMap pool_map_c;       // a group of 64-dim chunks of a page: K ring of the pair kernel's S-CTA
     CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
+    kairos::QMapCache proj_a[2], proj_b[2];    // operand maps of kairos_absorb_q [0] and kairos_project_out [1]
     kairos::QMapCache qd_map, qc_map, qp_map;  // decode q (box 16 rows), chunk q for gen-1 tiles (64 rows), for the pair kernel (128 rows)
     cudaStream_t copy_stream = nullptr;   // plan H2D copies run here, beside whatever precedes the step on the caller's stream
     cudaStream_t capture_stream = nullptr;  // the step's launches are captured here when a plan is replayed as a CUDA graph
@@ -189,10 +190,17 @@ int launch_gather(kairos_ctx* ctx, const int32_t* page_table, int32_t n_tokens, 
 int umma_chunk_tile_tokens();
 int umma_resident_ctas(const kairos_ctx* ctx);
 int encode_q_map(QMapCache* cache, const void* ptr, uint64_t rows, uint32_t box_rows);  // no-op when (ptr, rows) are unchanged
+// bf16 matrix [rows][inner] with `row_stride_bytes` between rows, boxes of box_inner x box_rows, SWIZZLE_128B (cached like encode_q_map)
+int encode_2d_map(QMapCache* cache, const void* ptr, uint64_t inner, uint64_t rows, uint64_t row_stride_bytes, uint32_t box_inner,
+                  uint32_t box_rows);
 int launch_attn_umma(kairos_ctx* ctx, const Plan& plan, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
                      cudaStream_t stream, int max_ctas, bool as_clusters, bool pdl);
 int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream);
 int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
+
+// projections either side of the attention (proj.cu)
+int launch_absorb_q(kairos_ctx* ctx, const void* q_nope, const void* q_rope, const void* w_uk_t, int32_t n, void* q_out, cudaStream_t stream);
+int launch_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, int32_t n, void* v_out, cudaStream_t stream);
 
 // chunk tiles on 2-CTA clusters (attn_pair.cu)
 int pair_tile_tokens();

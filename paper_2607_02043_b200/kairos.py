@@ -92,6 +92,10 @@ _lib.kairos_decide.restype = _c.c_int
 _lib.kairos_run_schedule.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp, _vp, _vp, _i32, _i32,
                                      _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.kairos_run_schedule.restype = _c.c_int
+_lib.kairos_absorb_q.argtypes = [_vp, _vp, _vp, _vp, _i32, _vp, _vp]
+_lib.kairos_absorb_q.restype = _c.c_int
+_lib.kairos_project_out.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp]
+_lib.kairos_project_out.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
 _lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
@@ -102,7 +106,7 @@ _lib.kairos_version.restype = _c.c_char_p
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
-           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule",
+           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -233,6 +237,21 @@ class Kairos:
                                            hp(out_chunk), None, None, _c.byref(h2d), _c.byref(d2h),
                                            _stream_ptr(stream)))
         return int(h2d.value), int(d2h.value)
+
+    # -- SURVEY.md 8(f) row 2
+    def absorb_q(self, q_nope, q_rope, w_uk_t, q_out=None, stream=None):
+        n = int(q_nope.shape[0])
+        if q_out is None:
+            q_out = torch.empty((n, 16, 576), dtype=torch.bfloat16, device=self.pool.device)
+        _check(_lib.kairos_absorb_q(self._h, _dp(q_nope), _dp(q_rope), _dp(w_uk_t), n, _dp(q_out), _stream_ptr(stream)))
+        return q_out
+
+    def project_out(self, o_lat, w_uv_t, v_out=None, stream=None):
+        n = int(o_lat.shape[0])
+        if v_out is None:
+            v_out = torch.empty((n, 16, 128), dtype=torch.bfloat16, device=self.pool.device)
+        _check(_lib.kairos_project_out(self._h, _dp(o_lat), _dp(w_uv_t), n, _dp(v_out), _stream_ptr(stream)))
+        return v_out
 
     # -- SURVEY.md 8(f) row 3
     def run_schedule(self, q_dec, dec_page_tables, dec_ctx_lens, dec_latent, dec_k_rope, chunk_sizes, q_prompt,
