@@ -82,6 +82,10 @@ def main():
         # Fig. 1's setting, attention only: B decodes with K cached tokens each, a batch of chi tokens of which chi - B are
         # prefill, five successive chunks of the same request (the prefix grows by one chunk each time)
         g = PAPER_GRID
+        import os
+        pk = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+        peaks = json.load(open(pk)) if os.path.exists(pk) else {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}
+        peaks = {"hbm_gbs": peaks["hbm_gbs"], "bf16_tflops": peaks["bf16_tflops"]}
         n = max(b * -(-k // 64) for b in g["Bs"] for k in g["Ks"]) + -(-(5 * max(g["chis"])) // 64) + 1
         ctx = make_context(n, max(g["Bs"]), max(g["chis"]))
         rows = []
@@ -91,9 +95,17 @@ def main():
                 for j in range(5):
                     t = run_table(ctx, [B], g["Ks"], [0, C], prefix=j * C, warmup=args.warmup, reps=args.reps, flush=not args.no_flush)
                     for iK, Kc in enumerate(g["Ks"]):
-                        rows.append({"chi": chi, "B": B, "K": Kc, "C": C, "chunk_index": j, "prefix": j * C,
-                                     "decode_only_us": t["median_us"][0][iK][0], "mixed_us": t["median_us"][0][iK][1]})
-        out["paper_grid"] = {"note": "PAPER.md:143 grid, attention only, one layer", "rows": rows}
+                        mixed = t["median_us"][0][iK][1]
+                        P = j * C
+                        nbytes = B * Kc * 1152 + B * 34816 + (P + C) * 1152 + C * 34816      # SURVEY.md 8(d) algorithmic work
+                        flops = 34816 * (B * Kc + C * P + C * (C + 1) // 2)
+                        roof = max(nbytes / (peaks["hbm_gbs"] * 1e3), flops / (peaks["bf16_tflops"] * 1e6))
+                        rows.append({"chi": chi, "B": B, "K": Kc, "C": C, "chunk_index": j, "prefix": P,
+                                     "decode_only_us": t["median_us"][0][iK][0], "mixed_us": mixed,
+                                     "delta_us": round(mixed - t["median_us"][0][iK][0], 2), "roofline_us": round(roof, 2),
+                                     "frac_of_roofline": round(roof / mixed, 3)})
+        out["paper_grid"] = {"note": "PAPER.md:143 grid (B x K x chi, five successive chunks), attention only, one layer; "
+                             "delta_us = the step-latency increase Fig. 1 plots (PAPER.md:159)", "peaks": peaks, "rows": rows}
     with open(args.out, "w") as f:
         json.dump(out, f, indent=1)
     print(f"wrote {args.out}")
