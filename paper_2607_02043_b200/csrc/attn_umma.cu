@@ -32,7 +32,8 @@ using namespace ptx;
 
 constexpr int kSoftmaxWarps = 8;                 // 2 per TMEM lane quadrant: each takes half of the query-row columns
 constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
-constexpr int kThreads = 64 + kSoftmaxThreads;    // warp 0 producer, warp 1 MMA issuer, warps 2-9 softmax
+constexpr int kThreads = 64 + kSoftmaxThreads + 32;  // warp 0 producer, warp 1 S issuer, warps 2-9 softmax, warp 10 PV issuer
+constexpr int kPvWarp = 2 + kSoftmaxWarps;
 constexpr int kChunkTileTokens = 4;
 // one page = 73,728 B = 9 slots of 8 KB ([64 tokens][128 B], SWIZZLE_128B)
 constexpr int kSlotBytes = 8192;
@@ -82,16 +83,12 @@ __device__ __forceinline__ PageSlots page_slots(uint32_t g) {
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64
 constexpr uint32_t kColO = 128;  // O^T blocks at 128 + 64*b
-#ifndef KAIROS_S_AHEAD
-#define KAIROS_S_AHEAD 1
-#endif
-constexpr int kSAhead = KAIROS_S_AHEAD;  // pages the S MMAs may run ahead of the PV MMAs (S^T is double-buffered: <= 1)
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the max grows by more than 2^8
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
 
 struct Small {
-    uint64_t q_full[2], q_empty[2], kv_full[kPageRing], kv_empty[kPageRing], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kPageRing][5], kv_empty[kPageRing], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -366,78 +363,82 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// MMA issue for one work item (whole warp, converged).  S(s) may run one page ahead of PV; PV has priority as soon
-// as its P^T is ready, because its completion releases the KV stage to the TMA producer.
+// MMA issue for one work item: two issuing warps (each converged, one elected lane issues).  A tcgen05.mma of these
+// shapes costs its issuing warp 25-60 cycles, more than the tensor pipe needs to execute it, and an mbarrier wait ~100
+// even when complete: with ONE warp the 36 S MMAs and the 16 PV MMAs of a page serialise (~2000 cycles per page) and a
+// PV whose P^T is ready queues behind the S burst of the next page -- which lengthens the time a page holds its ring
+// slots, and with it the bytes in flight per SM.  The S warp and the PV warp only meet through the barriers the softmax
+// warps sit between (s_full -> p_full), so they run independently: S(g + 1) is issued while PV(g) is.
+// tcgen05.commit tracks the issuing thread's own MMAs: the page's slots are released by the PV warp (S(g) completed
+// before the softmax of page g started, i.e. before PV(g) was issued).
 // ------------------------------------------------------------------------------------------------------------
 template <int N, int R>
-__device__ __forceinline__ void mma_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base,
-                                         int npages, uint32_t g0, uint32_t it, uint32_t leader, const KParams& p,
-                                         uint32_t qbuf, uint32_t qfull_parity) {
+__device__ __forceinline__ void s_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base, int npages, uint32_t g0,
+                                       uint32_t qbuf, uint32_t qfull_parity) {
     constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
-    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
     const uint32_t qb_lo = smem_desc_lo(q_base, 16);
     mbar_wait(&sm->q_full[qbuf], qfull_parity);
-    int s_next = 0, pv_next = 0;
-    uint32_t spins = 0;
-    while (pv_next < npages) {
-        if (pv_next < s_next) {
-            const uint32_t gg = g0 + pv_next;
-            const uint32_t pst = gg & 1, pph = (gg >> 1) & 1;
-            const bool ready = __any_sync(0xffffffffu, mbar_test_wait(&sm->p_full[pst], pph));
-            if (ready || s_next == npages) {
-                if (!ready) mbar_wait(&sm->p_full[pst], pph);
-                if (pv_next == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
-                tc_fence_after();
-                const PageSlots ps = page_slots<R>(gg);
-                const uint32_t st = gg & (kPageRing - 1);
-                const uint32_t pb_lo = smem_desc_lo(kv_base + ps.rope * kSlotBytes, 8192);
+    for (int s = 0; s < npages; ++s) {
+        const uint32_t gg = g0 + s;
+        const uint32_t st = gg & 1;
+        mbar_wait(&sm->s_empty[st], ((gg >> 1) & 1) ^ 1);  // the softmax warps have read S^T of page gg - 2 out of this buffer
+        // The page lands box by box (4 pairs of latent chunks + the RoPE chunk): the MMAs of a box are issued as soon as it is
+        // there, so that S^T completes ~300 cycles after the last box instead of a whole issue burst (~1270) later.  This warp
+        // has nothing else to do meanwhile.
+        const PageSlots ps = page_slots<R>(gg);
+        uint64_t* full = sm->kv_full[gg & (kPageRing - 1)];
+        const uint32_t par = (gg / kPageRing) & 1;
+        auto chunk_mmas = [&](uint32_t c, uint32_t slot, bool first) {
+            const uint32_t ka_lo = smem_desc_lo(kv_base + slot * kSlotBytes, 16);
 #pragma unroll
-                for (uint32_t b4 = 0; b4 < 4; ++b4) {
-                    const uint32_t va_lo = smem_desc_lo(kv_base + ps.pair[b4] * kSlotBytes, 8192);
+            for (uint32_t j = 0; j < 4; ++j)
+                umma_bf16_ss_lohi(tmem + kColS + st * 64, ka_lo + ((j * 32) >> 4), desc_hi,
+                                  qb_lo + ((c * N * 128 + j * 32) >> 4), desc_hi, idesc_s, !(first && j == 0));
+        };
+        // Fixed accumulation order (latent chunks 0..7, then the RoPE chunk) whatever the page's slot parity: the order of
+        // the fp32 partial sums must not depend on which pages a CTA happened to pop (results are bit-reproducible).
 #pragma unroll
-                    for (uint32_t ks = 0; ks < 4; ++ks)
-                        umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + ((ks * 2048) >> 4), desc_hi,
-                                          pb_lo + ((ks * 2048) >> 4), desc_hi, idesc_o, (pv_next > 0 || ks > 0));
-                }
-                umma_commit_elect(&sm->kv_empty[st]);
-                umma_commit_elect(&sm->pv_done[pst]);
-                if (pv_next == npages - 1) umma_commit_elect(&sm->o_full);
-                ++pv_next;
-                spins = 0;
-                continue;
-            }
+        for (uint32_t b = 0; b < 4; ++b) {
+            mbar_wait(&full[b], par);
+            tc_fence_after();
+            chunk_mmas(2 * b, ps.pair[b], b == 0);
+            chunk_mmas(2 * b + 1, ps.pair[b] + 1, false);
         }
-        if (s_next < npages && s_next <= pv_next + kSAhead) {
-            const uint32_t gg = g0 + s_next;
-            const uint32_t st = gg & 1;
-            if (__any_sync(0xffffffffu, mbar_test_wait(&sm->kv_full[gg & (kPageRing - 1)], (gg / kPageRing) & 1))) {
-                // No wait on s_empty: S(g) reuses the S^T buffer of page g - 2, whose PV has been issued (s_next <= pv_next + 1,
-                // and an item returns only after its last PV), i.e. p_full(g - 2) was observed, and every softmax warp arrives
-                // on s_empty (after its tcgen05.ld of S^T) before it arrives on p_full.  A completed mbarrier wait still costs
-                // this warp ~100 cycles, and it is the serial resource of the page chain.
-                tc_fence_after();
-                const PageSlots ps = page_slots<R>(gg);
-#pragma unroll
-                for (uint32_t c = 0; c < 9; ++c) {
-                    const uint32_t slot = c < 8 ? ps.pair[c >> 1] + (c & 1) : ps.rope;
-                    const uint32_t ka_lo = smem_desc_lo(kv_base + slot * kSlotBytes, 16);
-#pragma unroll
-                    for (uint32_t j = 0; j < 4; ++j)
-                        umma_bf16_ss_lohi(tmem + kColS + st * 64, ka_lo + ((j * 32) >> 4), desc_hi,
-                                          qb_lo + ((c * N * 128 + j * 32) >> 4), desc_hi, idesc_s, (c | j) != 0);
-                }
-                umma_commit_elect(&sm->s_full[st]);
-                ++s_next;
-                if (s_next == npages) {  // Q buffer(s) free once every S-MMA retires
-                    umma_commit_elect(&sm->q_empty[qbuf]);
-                    if (N == 64) umma_commit_elect(&sm->q_empty[1]);
-                }
-                spins = 0;
-                continue;
-            }
+        mbar_wait(&full[4], par);
+        tc_fence_after();
+        chunk_mmas(8, ps.rope, false);
+        umma_commit_elect(&sm->s_full[st]);
+        if (s == npages - 1) {  // Q buffer(s) free once every S-MMA retires
+            umma_commit_elect(&sm->q_empty[qbuf]);
+            if (N == 64) umma_commit_elect(&sm->q_empty[1]);
         }
-        if (++spins > (1u << 26)) __trap();
+    }
+}
+
+template <int N, int R>
+__device__ __forceinline__ void pv_item(Small* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t g0, uint32_t it) {
+    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
+    constexpr uint32_t desc_hi = smem_desc_hi(1024);
+    for (int pv = 0; pv < npages; ++pv) {
+        const uint32_t gg = g0 + pv;
+        const uint32_t pst = gg & 1, pph = (gg >> 1) & 1;
+        mbar_wait(&sm->p_full[pst], pph);
+        if (pv == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
+        tc_fence_after();
+        const PageSlots ps = page_slots<R>(gg);
+        const uint32_t pb_lo = smem_desc_lo(kv_base + ps.rope * kSlotBytes, 8192);
+#pragma unroll
+        for (uint32_t b4 = 0; b4 < 4; ++b4) {
+            const uint32_t va_lo = smem_desc_lo(kv_base + ps.pair[b4] * kSlotBytes, 8192);
+#pragma unroll
+            for (uint32_t ks = 0; ks < 4; ++ks)
+                umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + ((ks * 2048) >> 4), desc_hi,
+                                  pb_lo + ((ks * 2048) >> 4), desc_hi, idesc_o, (pv > 0 || ks > 0));
+        }
+        umma_commit_elect(&sm->kv_empty[gg & (kPageRing - 1)]);
+        umma_commit_elect(&sm->pv_done[pst]);
+        if (pv == npages - 1) umma_commit_elect(&sm->o_full);
     }
 }
 
@@ -460,14 +461,14 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
             mbar_init(&sm->q_empty[i], 1);
         }
         for (int i = 0; i < kPageRing; ++i) {
-            mbar_init(&sm->kv_full[i], 1);
+            for (int bx = 0; bx < 5; ++bx) mbar_init(&sm->kv_full[i][bx], 1);
             mbar_init(&sm->kv_empty[i], 1);
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&sm->s_full[i], 1);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
-            mbar_init(&sm->item_empty[i], 1 + kSoftmaxWarps);
+            mbar_init(&sm->item_empty[i], 2 + kSoftmaxWarps);
             mbar_init(&sm->p_full[i], kSoftmaxWarps);
             mbar_init(&sm->pv_done[i], 1);
         }
@@ -532,7 +533,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
                         const PageSlots ps = page_slots<R>(g);
-                        uint64_t* full = &sm->kv_full[g & (kPageRing - 1)];
+                        uint64_t* full = sm->kv_full[g & (kPageRing - 1)];  // one barrier per box: [0..3] latent pairs, [4] RoPE chunk
                         const int row = pid * kPage;
                         // take slots in ring order; pages retire in order, 9 slots each
                         auto reserve = [&](int n) {
@@ -543,25 +544,28 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                             }
                             free_slots -= n;
                         };
-                        reserve(ps.odd ? 1 : 2);
-                        mbar_arrive_expect_tx(full, 9 * kSlotBytes);
-                        if (ps.odd) tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, full, row, 8, policy);
+                        if (ps.odd) {
+                            reserve(1);
+                            mbar_arrive_expect_tx(&full[4], kSlotBytes);
+                            tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, &full[4], row, 8, policy);
+                        }
 #pragma unroll
                         for (int b = 0; b < 4; ++b) {
-                            if (b > 0 || ps.odd) reserve(2);
-                            tma_load_chunks(kv_u32 + ps.pair[b] * kSlotBytes, &pool_map2, full, row, 2 * b, policy);
+                            reserve(2);
+                            mbar_arrive_expect_tx(&full[b], 2 * kSlotBytes);
+                            tma_load_chunks(kv_u32 + ps.pair[b] * kSlotBytes, &pool_map2, &full[b], row, 2 * b, policy);
                         }
                         if (!ps.odd) {
                             reserve(1);
-                            tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, full, row, 8, policy);
+                            mbar_arrive_expect_tx(&full[4], kSlotBytes);
+                            tma_load_chunks(kv_u32 + ps.rope * kSlotBytes, &pool_map1, &full[4], row, 8, policy);
                         }
                     }
                 }
             }
         }
-    } else if (warp == 1) {
-        // ================= MMA issuer: the whole warp runs converged, one elected lane issues =================
-        const uint32_t leader = elect_one();
+    } else if (warp == 1 || warp == kPvWarp) {
+        // ================= MMA issuers: warp 1 issues the S MMAs, warp kPvWarp the PV MMAs (each converged, one elected lane)
         const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV);
         uint32_t q_full0 = 0, q_full1 = 0;
         uint32_t g = 0;
@@ -575,12 +579,18 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
             const WorkItem w = load_item(p.items + idx);
             const int kind = __shfl_sync(0xffffffffu, w.kind, 0);
             const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
-            // Q buffer bookkeeping mirrors the producer's: q_full[b] completes once per item that loads into buffer b
-            const uint32_t qb = (!DEC && kind) ? 0u : (it & 1u);
-            const uint32_t qpar = (qb ? q_full1 : q_full0) & 1u;
-            if (qb) ++q_full1; else ++q_full0;
-            if (!DEC && kind) mma_item<64, R>(sm, tmem, q_base, kv_base, npages, g, it, leader, p, 0, qpar);
-            else mma_item<16, R>(sm, tmem, q_base + qb * kDecQBytes, kv_base, npages, g, it, leader, p, qb, qpar);
+            const bool chunk = !DEC && kind;
+            if (warp == 1) {
+                // Q buffer bookkeeping mirrors the producer's: q_full[b] completes once per item that loads into buffer b
+                const uint32_t qb = chunk ? 0u : (it & 1u);
+                const uint32_t qpar = (qb ? q_full1 : q_full0) & 1u;
+                if (qb) ++q_full1; else ++q_full0;
+                if (chunk) s_item<64, R>(sm, tmem, q_base, kv_base, npages, g, 0, qpar);
+                else s_item<16, R>(sm, tmem, q_base + qb * kDecQBytes, kv_base, npages, g, qb, qpar);
+            } else {
+                if (chunk) pv_item<64, R>(sm, tmem, kv_base, npages, g, it);
+                else pv_item<16, R>(sm, tmem, kv_base, npages, g, it);
+            }
             g += npages;
         }
     } else {
