@@ -43,12 +43,14 @@ constexpr int kSlotBytes = 8192;
 // the mixed instantiation holds a 64-row Q tile (72 KB) and 18 slots.  Decode items alternate between two 18 KB Q
 // buffers at the start of the Q region (item parity), so that the next item's Q is loaded while the current item still
 // streams its pages; a chunk tile takes the whole region (both buffers).
+constexpr int kDecPBytes = 2048;
 template <bool DEC>
 struct Geo {
     static constexpr int kQBytes = (DEC ? 2 * 16 : 64) * kTokenBytes;  // two decode Q buffers, or one 64-row chunk tile
     static constexpr int kSlots = DEC ? 22 : 18;  // even: a pair of latent slots (one M=128 V^T operand) never straddles the wrap
     static constexpr int kOffKV = kQBytes;
-    static constexpr int kOffSmall = kOffKV + kSlots * kSlotBytes;
+    static constexpr int kOffP = kOffKV + kSlots * kSlotBytes;  // DEC: two 2 KB P buffers ([16 query rows][64 keys], K-major)
+    static constexpr int kOffSmall = kOffP + (DEC ? 2 * kDecPBytes : 0);
     static constexpr int kSmemBytes = kOffSmall + 3072 + 1024;  // Small + alignment slack
     static_assert(kQBytes % 1024 == 0 && kSlots % 2 == 0, "ring must stay 1024-B aligned and even");
     static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
@@ -88,7 +90,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;  // finite stand-in for "no key seen yet" (keeps x - m free of inf - inf)
 
 struct Small {
-    uint64_t q_full[2], q_empty[2], kv_full[kPageRing][5], kv_empty[kPageRing], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kPageRing][5], kv_empty[kPageRing][5], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -175,7 +177,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 // 8 warps: warp sw works on TMEM lane quadrant sw & 3 (16 of its lanes hold the M=64 accumulator rows = keys) and on
 // the column half sw >> 2 (N/2 query rows).
 // ------------------------------------------------------------------------------------------------------------
-template <int N, int R>
+template <int N, int R, bool PK>
 __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkItem& w, const KParams& p, uint32_t tmem,
                                              int sw, int lane, uint32_t& g, uint32_t it) {
     constexpr int NC = N / 2;            // columns of this warp
@@ -277,7 +279,18 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
                 for (int j = 0; j < 8; ++j) dst[j] = make_uint4(0u, 0u, 0u, 0u);
             }
         }
-        if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
+        if (PK) {
+            // decode-only instantiation: P as a K-major B operand [16 query rows][64 keys] (2 KB, SWIZZLE_128B) in a buffer of
+            // its own, so that the page's RoPE slot can go back to the ring as soon as the S MMAs have read it
+            if (g >= 2) mbar_wait(&sm->pv_done[b], ((g - 2) >> 1) & 1);  // PV of page g - 2 has read this P buffer
+            if (lane_ok) {
+                uint8_t* pb = kv + R * kSlotBytes + b * kDecPBytes;
+                const uint32_t kk = uint32_t(tok_in_page);
+#pragma unroll
+                for (int c = 0; c < NC; ++c)
+                    *reinterpret_cast<__nv_bfloat16*>(pb + sw128_offset(uint32_t(cbase + c), kk >> 3) + (kk & 7u) * 2u) = __float2bfloat16_rn(x[c]);
+            }
+        } else if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
             uint8_t* ps = kv + page_slots<R>(g).rope * kSlotBytes;
 #pragma unroll
             for (int j = 0; j < NC / 8; ++j) {
@@ -372,7 +385,7 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
 // tcgen05.commit tracks the issuing thread's own MMAs: the page's slots are released by the PV warp (S(g) completed
 // before the softmax of page g started, i.e. before PV(g) was issued).
 // ------------------------------------------------------------------------------------------------------------
-template <int N, int R>
+template <int N, int R, bool PK>
 __device__ __forceinline__ void s_item(Small* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base, int npages, uint32_t g0,
                                        uint32_t qbuf, uint32_t qfull_parity) {
     constexpr uint32_t idesc_s = make_idesc_bf16(64, N, 0, 0);   // S^T = K Q^T : A K-major, B K-major
@@ -409,6 +422,7 @@ __device__ __forceinline__ void s_item(Small* sm, uint32_t tmem, uint32_t q_base
         tc_fence_after();
         chunk_mmas(8, ps.rope, false);
         umma_commit_elect(&sm->s_full[st]);
+        if (PK) umma_commit_elect(&sm->kv_empty[gg & (kPageRing - 1)][4]);  // the RoPE slot is only ever read by these MMAs
         if (s == npages - 1) {  // Q buffer(s) free once every S-MMA retires
             umma_commit_elect(&sm->q_empty[qbuf]);
             if (N == 64) umma_commit_elect(&sm->q_empty[1]);
@@ -416,9 +430,10 @@ __device__ __forceinline__ void s_item(Small* sm, uint32_t tmem, uint32_t q_base
     }
 }
 
-template <int N, int R>
+template <int N, int R, bool PK>
 __device__ __forceinline__ void pv_item(Small* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t g0, uint32_t it) {
-    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);  // O^T += V^T P^T : A MN-major, B MN-major
+    // O^T += V^T P^T : A = the page's latent slots MN-major; B = P, MN-major in the page's RoPE slot, or (PK) K-major in its own buffer
+    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, PK ? 0 : 1);
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
     for (int pv = 0; pv < npages; ++pv) {
         const uint32_t gg = g0 + pv;
@@ -427,16 +442,19 @@ __device__ __forceinline__ void pv_item(Small* sm, uint32_t tmem, uint32_t kv_ba
         if (pv == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);  // previous item's epilogue has drained O^T
         tc_fence_after();
         const PageSlots ps = page_slots<R>(gg);
-        const uint32_t pb_lo = smem_desc_lo(kv_base + ps.rope * kSlotBytes, 8192);
+        uint64_t* empty = sm->kv_empty[gg & (kPageRing - 1)];
+        const uint32_t pb_lo = PK ? smem_desc_lo(kv_base + R * kSlotBytes + pst * kDecPBytes, 16)
+                                  : smem_desc_lo(kv_base + ps.rope * kSlotBytes, 8192);
 #pragma unroll
         for (uint32_t b4 = 0; b4 < 4; ++b4) {
             const uint32_t va_lo = smem_desc_lo(kv_base + ps.pair[b4] * kSlotBytes, 8192);
 #pragma unroll
             for (uint32_t ks = 0; ks < 4; ++ks)
                 umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + ((ks * 2048) >> 4), desc_hi,
-                                  pb_lo + ((ks * 2048) >> 4), desc_hi, idesc_o, (pv > 0 || ks > 0));
+                                  pb_lo + ((PK ? ks * 32 : ks * 2048) >> 4), desc_hi, idesc_o, (pv > 0 || ks > 0));
+            umma_commit_elect(&empty[b4]);  // slot pair b4 goes back to the ring when this block's MMAs retire
         }
-        umma_commit_elect(&sm->kv_empty[gg & (kPageRing - 1)]);
+        if (!PK) umma_commit_elect(&empty[4]);  // P^T sat in the RoPE slot
         umma_commit_elect(&sm->pv_done[pst]);
         if (pv == npages - 1) umma_commit_elect(&sm->o_full);
     }
@@ -462,7 +480,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
         }
         for (int i = 0; i < kPageRing; ++i) {
             for (int bx = 0; bx < 5; ++bx) mbar_init(&sm->kv_full[i][bx], 1);
-            mbar_init(&sm->kv_empty[i], 1);
+            for (int bx = 0; bx < 5; ++bx) mbar_init(&sm->kv_empty[i][bx], 1);
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&sm->s_full[i], 1);
@@ -492,7 +510,7 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
     if (warp == 0) {
         // ================= producer: pop work items, TMA-load Q tiles and KV pages =================
         uint32_t g = 0;        // pages issued so far
-        uint32_t g_acked = 0;  // pages whose slots have been taken back (kv_empty observed)
+        uint32_t g_acked = 0, k_acked = 0;  // release cursor: page, and group within it (kv_empty observed so far)
         int free_slots = R;
         uint32_t q_use0 = 0, q_use1 = 0;  // how many items have used each Q buffer (a chunk tile uses both)
         const uint32_t kv_u32 = smem_u32(base + kOffKV);
@@ -536,11 +554,15 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                         uint64_t* full = sm->kv_full[g & (kPageRing - 1)];  // one barrier per box: [0..3] latent pairs, [4] RoPE chunk
                         const int row = pid * kPage;
                         // take slots in ring order; pages retire in order, 9 slots each
+                        // Slots come back group by group (the page's RoPE slot and its 4 slot pairs), in ring order: for a page
+                        // that starts at an odd slot the RoPE slot is first, else last.
                         auto reserve = [&](int n) {
                             while (free_slots < n) {
-                                mbar_wait(&sm->kv_empty[g_acked & (kPageRing - 1)], (g_acked / kPageRing) & 1);
-                                ++g_acked;
-                                free_slots += 9;
+                                const uint32_t odd = ((g_acked * 9u) % uint32_t(R)) & 1u;
+                                const uint32_t grp = odd ? (k_acked == 0 ? 4u : k_acked - 1u) : k_acked;
+                                mbar_wait(&sm->kv_empty[g_acked & (kPageRing - 1)][grp], (g_acked / kPageRing) & 1);
+                                free_slots += grp == 4 ? 1 : 2;
+                                if (++k_acked == 5) { k_acked = 0; ++g_acked; }
                             }
                             free_slots -= n;
                         };
@@ -585,11 +607,11 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
                 const uint32_t qb = chunk ? 0u : (it & 1u);
                 const uint32_t qpar = (qb ? q_full1 : q_full0) & 1u;
                 if (qb) ++q_full1; else ++q_full0;
-                if (chunk) s_item<64, R>(sm, tmem, q_base, kv_base, npages, g, 0, qpar);
-                else s_item<16, R>(sm, tmem, q_base + qb * kDecQBytes, kv_base, npages, g, qb, qpar);
+                if (chunk) s_item<64, R, false>(sm, tmem, q_base, kv_base, npages, g, 0, qpar);
+                else s_item<16, R, DEC>(sm, tmem, q_base + qb * kDecQBytes, kv_base, npages, g, qb, qpar);
             } else {
-                if (chunk) pv_item<64, R>(sm, tmem, kv_base, npages, g, it);
-                else pv_item<16, R>(sm, tmem, kv_base, npages, g, it);
+                if (chunk) pv_item<64, R, false>(sm, tmem, kv_base, npages, g, it);
+                else pv_item<16, R, DEC>(sm, tmem, kv_base, npages, g, it);
             }
             g += npages;
         }
@@ -605,8 +627,8 @@ kairos_mixed_kernel(const __grid_constant__ CUtensorMap pool_map2, const __grid_
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
             if (idx < 0) break;
             const WorkItem w = load_item(p.items + idx);
-            if (!DEC && w.kind) softmax_item<64, R>(sm, kv, w, p, tmem, sw, lane, g, it);
-            else softmax_item<16, R>(sm, kv, w, p, tmem, sw, lane, g, it);
+            if (!DEC && w.kind) softmax_item<64, R, false>(sm, kv, w, p, tmem, sw, lane, g, it);
+            else softmax_item<16, R, DEC>(sm, kv, w, p, tmem, sw, lane, g, it);
         }
     }
 
