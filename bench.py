@@ -305,7 +305,7 @@ def roofline_entry(pt: Point, us_per_step: float, kern_us: float, peaks) -> dict
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=HEADLINE[0], help="BASELINE.json configs index of the headline workload")
     ap.add_argument("--chunk", type=int, default=None, help="chunk size for configs[3]")
@@ -341,8 +341,18 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- headline workload first (clock / throttle reasons are sampled over its timed regions only)
+    pt = Point(args.config, args.chunk, R_.replica_seed_shift(rank), dev, K, torch)
+    inp = pt.inp
+    pt.warm(args.warmup)
+    info = pt.info
     sampler = ClockSampler(local_rank)
     sampler.start()
+    ms_head, host_head, _, _ = pt.timed(args.steps, barrier)
+    # roofline leg: the same K steps again with the attention kernels bracketed by CUDA events on their stream
+    ms_prof, _, kern_us, kern_n = pt.timed(args.steps, barrier, profile=True)
+    clocks = sampler.stop()
+
 
     # ---- the other gated workloads (rank 0's own GPU, N = 1 only): same protocol, their own step counts
     sweep = []
@@ -351,34 +361,24 @@ def main():
         for (ci, cc) in SWEEP:
             if point_key(ci, cc) == headline_key:
                 continue
-            pt = Point(ci, cc, 0, dev, K, torch)
-            pt.warm(args.warmup)
-            ms, _, _, _ = pt.timed(10, barrier)  # sizes the timed region: at least K steps and about 30 ms
+            sp = Point(ci, cc, 0, dev, K, torch)
+            sp.warm(args.warmup)
+            ms, _, _, _ = sp.timed(10, barrier)  # sizes the timed region: at least K steps and about 30 ms
             n = int(min(max(args.steps, 30e3 / max(ms * 1e3 / 10, 1.0)), 400))
-            ms, host_s, _, _ = pt.timed(n, barrier)
-            _, _, k_us, k_n = pt.timed(n, barrier, profile=True)
+            ms, host_s, _, _ = sp.timed(n, barrier)
+            _, _, k_us, k_n = sp.timed(n, barrier, profile=True)
             us, kern = ms * 1e3 / n, k_us / max(k_n, 1)
-            e = {"workload": point_key(ci, cc), "B": pt.inp.n_dec, "C": pt.inp.chunk_len, "P": pt.inp.prefix_len,
-                 "step_us": us, "kernel_us": kern, "host_enqueue_us": host_s * 1e6 / n, "steps": n, "l2": pt.l2,
-                 "chunk_pairs": pt.info["chunk_pairs"], "dec_ctas_first": pt.info["dec_ctas_first"],
-                 "kernels_per_step": pt.info["kernels"] + (1 if pt.inp.chunk_len else 0), "graph": pt.info["graph"]}
-            e.update(roofline_entry(pt, us, kern, peaks))
+            e = {"workload": point_key(ci, cc), "B": sp.inp.n_dec, "C": sp.inp.chunk_len, "P": sp.inp.prefix_len,
+                 "step_us": us, "kernel_us": kern, "host_enqueue_us": host_s * 1e6 / n, "steps": n, "l2": sp.l2,
+                 "chunk_pairs": sp.info["chunk_pairs"], "dec_ctas_first": sp.info["dec_ctas_first"],
+                 "kernels_per_step": sp.info["kernels"] + (1 if sp.inp.chunk_len else 0), "graph": sp.info["graph"]}
+            e.update(roofline_entry(sp, us, kern, peaks))
             sweep.append(e)
-            pt.close()
-            del pt
+            sp.close()
+            del sp
 
-    # ---- headline workload
-    pt = Point(args.config, args.chunk, R_.replica_seed_shift(rank), dev, K, torch)
-    inp = pt.inp
-    pt.warm(args.warmup)
-    info = pt.info
-    ms, host_s, _, _ = pt.timed(args.steps, barrier)
-    # roofline leg: the same K steps again with the attention kernels bracketed by CUDA events on their stream
-    ms_prof, _, kern_us, kern_n = pt.timed(args.steps, barrier, profile=True)
-    clocks = sampler.stop()
-
-    ms_max = R_.max_over_ranks(ms, dev)
-    us_per_step = R_.whole_job_us_per_step(ms, args.steps, world, dev)  # world replicas advance one step per iteration
+    ms_max = R_.max_over_ranks(ms_head, dev)
+    us_per_step = R_.whole_job_us_per_step(ms_head, args.steps, world, dev)  # world replicas advance one step per iteration
 
     # ---- end-to-end leg: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -433,7 +433,7 @@ def main():
                  "step_frac_of_roofline_sustained_tensor_peak": re["frac_sustained"],
                  "us_per_step_with_kernel_events": ms_prof * 1e3 / args.steps})
     head = {"workload": headline_key, "B": inp.n_dec, "C": inp.chunk_len, "P": inp.prefix_len, "step_us": own_us,
-            "kernel_us": kern_avg_us, "host_enqueue_us": host_s * 1e6 / args.steps, "steps": args.steps, "l2": pt.l2,
+            "kernel_us": kern_avg_us, "host_enqueue_us": host_head * 1e6 / args.steps, "steps": args.steps, "l2": pt.l2,
             "chunk_pairs": info["chunk_pairs"], "dec_ctas_first": info["dec_ctas_first"],
             "kernels_per_step": info["kernels"] + (1 if inp.chunk_len else 0), "graph": info["graph"]}
     head.update(re)
@@ -455,7 +455,7 @@ def main():
                    "step": "kairos_append_latent(chunk) + kairos_mixed_step (cached plan replayed as a CUDA graph: attention grid(s) + combine)",
                    "plan": info, "library": K.version()},
         "clocks": clocks,
-        "host_enqueue_us": host_s * 1e6 / args.steps,
+        "host_enqueue_us": host_head * 1e6 / args.steps,
         "e2e": e2e,
         "gpu_launches": int(args.steps * ((1 if inp.chunk_len else 0) + info["kernels"])),
         "roofline": roof,

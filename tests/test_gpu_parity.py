@@ -396,3 +396,35 @@ def test_latency_table_shape_and_monotone():
     assert med.shape == (2, 1, 3) and med[0, 0, 0] == 0.0
     assert np.all(med.ravel()[1:] > 0) and np.all(mn <= med + 1e-9)
     assert med[1, 0, 2] > med[1, 0, 0] and med[0, 0, 2] > med[0, 0, 1]
+
+
+def test_latency_table_matches_independently_timed_steps():
+    """an entry of the table produced through kairos_step_latency_table must agree with the same point
+    timed independently (CUDA events around back-to-back kairos_mixed_step calls on BASELINE.json configs[3] inputs), and
+    the table must grow with C, with K and with B within noise."""
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    from paper_2607_02043_b200 import latency_table as LT
+    ctx = LT.make_context(LT.pages_needed([256], [2048], [2048]), 256, 2048)
+    Cs = [0, 512, 2048]
+    med, mn = ctx.step_latency_table([256], [2048], Cs, warmup=5, reps=20, flush_l2=False)
+    for iC, C in enumerate(Cs):
+        inp = W.make_config(3, chunk_len=C)
+        run = Hp.GpuRun(inp)
+        run.append()
+        out = run.ctx.mixed_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, C, 0)
+        bound = run.ctx.bind_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, C, 0, *out)
+        for _ in range(5):
+            bound.run()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(20):
+            bound.run()
+        e1.record()
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / 20
+        assert abs(med[0, 0, iC] - us) <= 0.10 * us + 3.0, (C, med[0, 0, iC], us)
+    assert med[0, 0, 0] < med[0, 0, 1] < med[0, 0, 2]
+    grid, _ = ctx.step_latency_table([64, 256], [512, 2048], [0, 1024], warmup=3, reps=10, flush_l2=False)
+    assert np.all(grid[1] > grid[0] * 0.98) and np.all(grid[:, 1] > grid[:, 0] * 0.98) and np.all(grid[:, :, 1] > grid[:, :, 0])
