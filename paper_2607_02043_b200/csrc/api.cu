@@ -129,6 +129,23 @@ static int launch_step_kernels(kairos_ctx* ctx, const PlanEntry& e, const PlanBu
     return KAIROS_OK;
 }
 
+// kairos_profile_enable: the next pair of events that brackets a step's attention kernels (NULL, NULL when profiling is off)
+static int next_profile_events(kairos_ctx* ctx, cudaEvent_t* e0, cudaEvent_t* e1) {
+    *e0 = *e1 = nullptr;
+    if (!ctx->profile) return KAIROS_OK;
+    if (ctx->prof_used + 2 > ctx->prof_events.size()) {
+        for (int i = 0; i < 2; ++i) {
+            cudaEvent_t ev;
+            KAIROS_CUDA_TRY(cudaEventCreate(&ev));
+            ctx->prof_events.push_back(ev);
+        }
+    }
+    *e0 = ctx->prof_events[ctx->prof_used];
+    *e1 = ctx->prof_events[ctx->prof_used + 1];
+    ctx->prof_used += 2;
+    return KAIROS_OK;
+}
+
 static int kernels_of(const Plan& plan) {
     return (plan.n_pairs > 0 ? 1 : 0) + (plan.items.empty() ? 0 : 1) + (plan.combines.empty() ? 0 : 1);
 }
@@ -281,18 +298,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
         KAIROS_CUDA_TRY(cudaGraphLaunch(b.exec, stream));
     } else {
         cudaEvent_t e0 = nullptr, e1 = nullptr;
-        if (ctx->profile) {
-            if (ctx->prof_used + 2 > ctx->prof_events.size()) {
-                for (int i = 0; i < 2; ++i) {
-                    cudaEvent_t ev;
-                    KAIROS_CUDA_TRY(cudaEventCreate(&ev));
-                    ctx->prof_events.push_back(ev);
-                }
-            }
-            e0 = ctx->prof_events[ctx->prof_used];
-            e1 = ctx->prof_events[ctx->prof_used + 1];
-            ctx->prof_used += 2;
-        }
+        if (int rc = next_profile_events(ctx, &e0, &e1)) return rc;
         if (int rc = launch_step_kernels(ctx, *e, b, a, stream, e0, e1)) return rc;
     }
     KAIROS_CUDA_TRY(cudaEventRecord(b.last_use, stream));
@@ -373,7 +379,10 @@ static int enqueue_schedule(kairos_ctx* ctx, const ScheduleArgs& s, const std::v
             if (int rc = encode_q_map(&ctx->qp_map, a.q_chunk, uint64_t(C) * kHeads, 128)) return rc;
         PlanBuffer b;
         b.dev = const_cast<uint8_t*>(arena) + plan_off[i];
-        if (int rc = launch_step_kernels(ctx, e, b, a, stream, nullptr, nullptr)) return rc;
+        cudaEvent_t pe0 = nullptr, pe1 = nullptr;  // kairos_profile_enable brackets each step's attention kernels (never while capturing)
+        if (stream != ctx->capture_stream)
+            if (int rc = next_profile_events(ctx, &pe0, &pe1)) return rc;
+        if (int rc = launch_step_kernels(ctx, e, b, a, stream, pe0, pe1)) return rc;
         if (ev) KAIROS_CUDA_TRY(cudaEventRecord(ev[2 * i + 1], stream));
         done += C;
     }
@@ -438,9 +447,9 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
         std::memcpy(k, chunk_sizes, sizeof(int32_t) * size_t(n_steps));
     }
     ScheduleCache& sc = ctx->schedule;
-    const bool want_steps = step_us != nullptr;
-    const bool hit = sc.exec && sc.key == key && ctx->use_graph && !want_steps;
-    if (!hit) {
+    const bool want_steps = step_us != nullptr || ctx->profile;  // both launch the steps one by one (event brackets)
+    const bool planned = !sc.key.empty() && sc.key == key;  // plans of every step are in the arena already
+    if (!planned) {
         // ---- plan every step (a0) and pack the work lists and the decodes' append positions into one arena
         if (sc.exec) { cudaGraphExecDestroy(sc.exec); sc.exec = nullptr; }
         sc.key.clear();
@@ -488,8 +497,12 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
         for (int32_t i = 0; i < n_steps; ++i)
             for (int32_t j = 0; j < n_dec; ++j) pos[size_t(i) * n_dec + j] = dec_ctx_lens[j] + i;  // the slot of step i's new token
         KAIROS_CUDA_TRY(cudaMemcpyAsync(sc.dev, sc.host, off, cudaMemcpyHostToDevice, stream));
-        // ---- one CUDA graph for the whole schedule (programmatic launch edges kept)
-        if (ctx->use_graph && !want_steps && ctx->capture_stream &&
+        sc.key = key;
+    }
+    {
+        // ---- one CUDA graph for the whole schedule (programmatic launch edges kept), captured on first use without timing brackets
+        std::vector<int32_t> lens(dec_ctx_lens, dec_ctx_lens + n_dec);
+        if (!sc.exec && ctx->use_graph && !want_steps && ctx->capture_stream &&
             cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
             const int rc = enqueue_schedule(ctx, s, sc.steps, lens, chunk_sizes, n_steps, static_cast<const uint8_t*>(sc.dev), sc.plan_off,
                                             sc.pos_off, ctx->capture_stream, nullptr);
@@ -498,11 +511,10 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
             bool ok = rc == KAIROS_OK && ce == cudaSuccess && graph != nullptr;
             if (ok) ok = cudaGraphInstantiate(&sc.exec, graph, 0) == cudaSuccess;
             if (graph) cudaGraphDestroy(graph);
-            if (!ok) {
+            if (!ok) {  // not an error of the schedule: graphs are switched off for this context, the steps are launched one by one
                 cudaGetLastError();
                 sc.exec = nullptr;
-            } else {
-                sc.key = key;
+                ctx->use_graph = 0;
             }
         }
     }
@@ -513,7 +525,7 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
         std::vector<cudaEvent_t>& v;
         ~EvGuard() { for (auto e : v) cudaEventDestroy(e); }
     } guard{ev};
-    const int n_ev = timed ? 2 + (want_steps ? 2 * n_steps : 0) : 0;
+    const int n_ev = timed ? 2 + (step_us ? 2 * n_steps : 0) : 0;
     for (int i = 0; i < n_ev; ++i) {
         cudaEvent_t e;
         KAIROS_CUDA_TRY(cudaEventCreate(&e));
@@ -525,7 +537,7 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
     } else {
         std::vector<int32_t> lens(dec_ctx_lens, dec_ctx_lens + n_dec);
         if (int rc = enqueue_schedule(ctx, s, sc.steps, lens, chunk_sizes, n_steps, static_cast<const uint8_t*>(sc.dev), sc.plan_off,
-                                      sc.pos_off, stream, want_steps ? ev.data() + 2 : nullptr))
+                                      sc.pos_off, stream, step_us ? ev.data() + 2 : nullptr))
             return rc;
     }
     ctx->last_info[4] = sc.kernels;
@@ -536,7 +548,7 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
         float ms = 0.f;
         KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, ev[0], ev[1]));
         if (ttft_us) *ttft_us = double(ms) * 1e3;
-        for (int32_t i = 0; want_steps && i < n_steps; ++i) {
+        for (int32_t i = 0; step_us && i < n_steps; ++i) {
             KAIROS_CUDA_TRY(cudaEventElapsedTime(&ms, ev[2 + 2 * i], ev[3 + 2 * i]));
             step_us[i] = double(ms) * 1e3;
         }

@@ -214,8 +214,8 @@ class Kairos:
     def bind_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
                   prefix_len: int, out_dec, out_chunk, lse_dec=None, lse_chunk=None, chunk_latent=None, chunk_k_rope=None):
         """Marshals the arguments of a step ONCE (a serving loop passes the same buffers step after step) and returns a
-        BoundStep whose run() makes the two C calls -- kairos_append_latent for the chunk (when chunk_latent / chunk_k_rope are
-        given) and kairos_mixed_step -- with no per-call tensor inspection.  The tensors are kept alive by the object."""
+        BoundStep whose run() makes the C call -- kairos_mixed_step, or, when chunk_latent / chunk_k_rope are given, the
+        one-step kairos_run_schedule that appends the chunk and runs the step -- with no per-call tensor inspection.  The tensors are kept alive by the object."""
         return BoundStep(self, q_dec, dec_page_tables, dec_ctx_lens, q_chunk, chunk_page_table, chunk_len, prefix_len,
                          out_dec, out_chunk, lse_dec, lse_chunk, chunk_latent, chunk_k_rope)
 
@@ -328,18 +328,22 @@ class BoundStep:
         self._step_args = (B, _dp(q_dec), _dp(dec_page_tables), stride, self._lens.ctypes.data_as(_vp), C, int(prefix_len),
                            _dp(q_chunk), _dp(chunk_page_table), int(chunk_page_table.numel()) if C else 0, _dp(out_dec),
                            _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk))
-        self._append_args = None
+        self._sched_args = None
         if C and chunk_latent is not None:
-            self._append_args = (_dp(chunk_latent), _dp(chunk_k_rope), C, _dp(chunk_page_table), int(chunk_page_table.numel()),
-                                 int(prefix_len))
+            # append + step as a one-step chunk schedule: kairos_run_schedule captures the append, the attention grid(s) and
+            # the combine into ONE graph (one launch per step instead of an append launch plus a graph launch)
+            self._cs = np.array([C], dtype=np.int32)
+            self._sched_args = (B, _dp(q_dec), _dp(dec_page_tables), stride, self._lens.ctypes.data_as(_vp), None, None, C,
+                                self._cs.ctypes.data_as(_vp), 1, _dp(q_chunk), _dp(chunk_latent), _dp(chunk_k_rope),
+                                _dp(chunk_page_table), int(chunk_page_table.numel()), int(prefix_len), _dp(out_dec),
+                                _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk), None, None)
 
     def run(self, stream: Optional[torch.cuda.Stream] = None) -> None:
         sp = _stream_ptr(stream)
-        if self._append_args is not None:
-            rc = _lib.kairos_append_latent(self._h, *self._append_args, sp)
-            if rc:
-                raise KairosError(rc)
-        rc = _lib.kairos_mixed_step(self._h, *self._step_args, sp)
+        if self._sched_args is not None:
+            rc = _lib.kairos_run_schedule(self._h, *self._sched_args, sp)
+        else:
+            rc = _lib.kairos_mixed_step(self._h, *self._step_args, sp)
         if rc:
             raise KairosError(rc)
 
