@@ -55,11 +55,15 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
 
 
+KERNEL_SOURCES = ["append.cu", "attn_pair.cu", "attn_umma.cu", "kairos_internal.h", "plan.cpp", "umma_ptx.cuh"]
+
+
 def csrc_sha() -> str:
-    """Hash of the kernel sources: an ncu DRAM-traffic capture under profiles/ is only quoted for the sources it measured."""
+    """Hash of the device code and the planner (what decides a kernel's DRAM traffic): an ncu capture under profiles/ is
+    only quoted for the sources it measured."""
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2607_02043_b200", "csrc")
-    for f in sorted(os.listdir(d)):
+    for f in KERNEL_SOURCES:
         with open(os.path.join(d, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
