@@ -204,7 +204,8 @@ int kairos_plan_dump(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_l
                      int32_t pair_mode, int32_t* items_out, int32_t max_items, int32_t* n_items_out,
                      int32_t* n_partial_slots_out, int32_t* n_pairs_out);
 
-/* Introspection of the last kairos_mixed_step plan on this context (host-only; for tests, bench):
+/* Introspection of the last kairos_mixed_step plan on this context -- after kairos_run_schedule: the plan of the schedule's
+ * LAST step, with [4] = every kernel of the whole schedule, appends included -- (host-only; for tests, bench):
  * info[0] = work items, [1] = decode splits, [2] = chunk tiles, [3] = CTAs launched, [4] = kernels launched
  * by that call, [5] = workspace bytes used, [6] = 2-CTA clusters the chunk ran on (0 = the chunk ran as tiles of the
  * decode grid's queue), [7] = plan cache (0 planned, 1 structure re-used with patched lengths, 2 exact hit),

@@ -540,8 +540,20 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
                                       sc.pos_off, stream, step_us ? ev.data() + 2 : nullptr))
             return rc;
     }
-    ctx->last_info[4] = sc.kernels;
-    ctx->last_info[8] = (sc.exec && !want_steps) ? 1 : 0;
+    {   // kairos_last_plan_info: the LAST step's plan; [4] counts every kernel of the schedule (appends included)
+        const Plan& lp = sc.steps.back().plan;
+        std::memset(ctx->last_info, 0, sizeof(ctx->last_info));
+        ctx->last_info[0] = int64_t(lp.items.size());
+        ctx->last_info[1] = lp.n_decode_items;
+        ctx->last_info[2] = lp.n_chunk_items + int64_t(lp.pair_items.size());
+        ctx->last_info[3] = std::min<int64_t>(lp.n_pairs > 0 && lp.dec_ctas > 0 ? lp.dec_ctas : umma_resident_ctas(ctx), int64_t(lp.items.size()));
+        ctx->last_info[4] = sc.kernels;
+        ctx->last_info[5] = int64_t(kCounterBytes + size_t(lp.n_partial_slots) * kPartialSlotBytes);
+        ctx->last_info[6] = lp.n_pairs;
+        ctx->last_info[7] = planned ? 2 : 0;
+        ctx->last_info[8] = (sc.exec && !want_steps) ? 1 : 0;
+        ctx->last_info[9] = lp.dec_ctas;
+    }
     if (timed) {
         KAIROS_CUDA_TRY(cudaEventRecord(ev[1], stream));
         KAIROS_CUDA_TRY(cudaEventSynchronize(ev[1]));
