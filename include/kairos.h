@@ -306,6 +306,60 @@ int kairos_decide(const kairos_step_model* model, const kairos_prefill_model* pr
                   int32_t* schedule_out, int32_t max_schedule, kairos_decide_output* out);
 
 /*
+ * SURVEY.md 8(f) row 4 (second half) -- the paper's policy simulator ("we wrap the three predictors in an
+ * event-based simulator with support for PD disaggregation"; section 3.4, Table 4): the latency models
+ * above inside an event loop over n_prefill FIFO prefill nodes and n_decode decode nodes.  Host only.  The paper prints no
+ * pseudo-code for it; the rules (reading G22) are:
+ *   - A request that is not deflected goes to the prefill node with the fewest outstanding prompt tokens (ties: lowest
+ *     index), occupies it for T_pf (Eq. 3) in FIFO order, and is ready on a decode node transfer_per_token * l_r later
+ *     (KV transfer = bytes over bandwidth); its TTFT is that instant minus its arrival.  It joins the decode
+ *     node with the fewest in-flight + pending requests at the time its prefill ends.
+ *   - A decode node runs steps back to back while it has work.  A step admits the pending requests that are ready, then
+ *     runs B in-flight decodes caching Kd tokens plus -- if a deflected request is in its prefill phase there (at most one
+ *     per node) -- C = min(max(chi - B, 1), tokens left) of its prompt over the P already served, and lasts
+ *     T_step(B, Kd, C, P) (Eq. 4).  At its end every decode has one more token and leaves when its output is complete; a
+ *     deflected request whose prompt is complete has TTFT = step end - arrival and decodes on the same node from then on.
+ *   - A step with B > 0 longer than tbt_slo is a TBT violation of the step and of every request decoding in it.
+ *   - policy 0 Baseline: never deflect.  1 SQ(param): deflect when more than `param` requests WAIT on every prefill node.
+ *     2 SL(param): deflect when l_r < param.  Both to the decode node with the fewest in-flight decodes that hosts no
+ *     deflected request (none: prefill path), with the fixed chi = static_chi (128 in the paper).  3 Oracle: kairos_decide on
+ *     the simulator's own state (the queue of the prefill node the request would take; (B, Kd) of the eligible decode nodes);
+ *     the schedule X* is followed step by step, its last chi repeated if it runs out.
+ *   - Events at equal times: decode step ends (node order), prefill completions (node order), arrivals; then idle nodes start.
+ *   reqs      HOST [n], sorted by arrival; prompt_len >= 1, output_len >= 0 (tokens decoded after the first)
+ *   ttft_out  HOST double [n] or NULL
+ * Result: deflections, P95 (nearest rank) and mean TTFT, decode steps and those over tbt_slo, SLO attainment (TTFT <= ttft_slo
+ * and no violated step), makespan -- Table 4's columns.  Errors: INVALID_ARG.
+ */
+typedef struct {
+    double arrival;
+    int32_t prompt_len;
+    int32_t output_len;
+} kairos_sim_request;
+
+typedef struct {
+    int32_t n_prefill, n_decode;
+    int32_t chi_p;               /* prefill-node chunk size */
+    int32_t policy;              /* 0 baseline, 1 SQ(theta), 2 SL(l), 3 Oracle */
+    int32_t param;               /* theta or l */
+    int32_t static_chi;          /* chi of the static policies (total tokens per step) */
+    const int32_t* candidates;   /* Oracle: chunk-size candidates, strictly decreasing */
+    int32_t n_candidates;
+    double tbt_slo, beta, alpha, ttft_slo;
+    double transfer_per_token;   /* KV transfer time per prompt token */
+} kairos_sim_config;
+
+typedef struct {
+    int32_t n_requests, n_deflected;
+    double p95_ttft, mean_ttft;
+    int64_t decode_steps, tbt_violations;
+    double slo_attainment, makespan;
+} kairos_sim_result;
+
+int kairos_simulate(const kairos_step_model* model, const kairos_prefill_model* prefill, const kairos_sim_config* cfg,
+                    const kairos_sim_request* reqs, int32_t n, double* ttft_out, kairos_sim_result* out);
+
+/*
  * what the decode node does with a deflected request (section 4.3.2;
  * PAPER.md:363-367 section 5.4; Fig. 1's "successive chunks"): the chunk schedule X = [chi(1) ..
  * chi(m)] executed as m successive steps behind one call.  Step i (0-based):

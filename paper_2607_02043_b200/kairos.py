@@ -82,6 +82,25 @@ class DecideOutput(_c.Structure):
     _fields_ = [("decision", _i32), ("node", _i32), ("n_steps", _i32), ("ttft_pf", _c.c_double), ("ttft_dec", _c.c_double)]
 
 
+class SimRequest(_c.Structure):
+    _fields_ = [("arrival", _c.c_double), ("prompt_len", _i32), ("output_len", _i32)]
+
+
+class SimConfig(_c.Structure):
+    _fields_ = [("n_prefill", _i32), ("n_decode", _i32), ("chi_p", _i32), ("policy", _i32), ("param", _i32),
+                ("static_chi", _i32), ("candidates", _vp), ("n_candidates", _i32), ("tbt_slo", _c.c_double),
+                ("beta", _c.c_double), ("alpha", _c.c_double), ("ttft_slo", _c.c_double), ("transfer_per_token", _c.c_double)]
+
+
+class SimResult(_c.Structure):
+    _fields_ = [("n_requests", _i32), ("n_deflected", _i32), ("p95_ttft", _c.c_double), ("mean_ttft", _c.c_double),
+                ("decode_steps", _c.c_int64), ("tbt_violations", _c.c_int64), ("slo_attainment", _c.c_double),
+                ("makespan", _c.c_double)]
+
+
+_lib.kairos_simulate.argtypes = [_c.POINTER(StepModel), _c.POINTER(PrefillModel), _c.POINTER(SimConfig), _vp, _i32, _vp,
+                                 _c.POINTER(SimResult)]
+_lib.kairos_simulate.restype = _c.c_int
 _lib.kairos_fit_latency_model.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, _c.POINTER(StepModel), _vp]
 _lib.kairos_fit_latency_model.restype = _c.c_int
 _lib.kairos_predict_step.argtypes = [_c.POINTER(StepModel), _c.c_int64, _c.c_int64, _c.c_int64, _c.c_int64]
@@ -106,7 +125,7 @@ _lib.kairos_version.restype = _c.c_char_p
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
-           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out",
+           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -407,6 +426,28 @@ def decide(model: StepModel, prefill: PrefillModel, prompt_len: int, queue_lens,
     _check(_lib.kairos_decide(_c.byref(model), _c.byref(prefill), _c.byref(inp), sched.ctypes.data_as(_vp), max_schedule,
                               _c.byref(out)))
     return ("DEFLECT" if out.decision else "KEEP"), int(out.node), sched[:out.n_steps].tolist(), float(out.ttft_pf), float(out.ttft_dec)
+
+
+POLICIES = {"baseline": 0, "sq": 1, "sl": 2, "oracle": 3}
+
+
+def simulate(model: StepModel, prefill: PrefillModel, reqs, n_prefill: int, n_decode: int, chi_p: int, policy: str,
+             param: int = 0, static_chi: int = 128, candidates=(2048, 1024, 512, 256, 128), tbt_slo: float = 1e30,
+             beta: float = 1.0, alpha: float = 1.0, ttft_slo: float = 1e30, transfer_per_token: float = 0.0):
+    """kairos_simulate: reqs = sequence of (arrival, prompt_len, output_len) sorted by arrival.  Returns (dict, ttft array)."""
+    n = len(reqs)
+    arr = (SimRequest * max(n, 1))()
+    for i, (t, l, o) in enumerate(reqs):
+        arr[i] = SimRequest(float(t), int(l), int(o))
+    cand = np.ascontiguousarray(np.asarray(candidates, dtype=np.int32))
+    cfg = SimConfig(int(n_prefill), int(n_decode), int(chi_p), POLICIES[policy], int(param), int(static_chi),
+                    cand.ctypes.data_as(_vp), int(cand.size), float(tbt_slo), float(beta), float(alpha), float(ttft_slo),
+                    float(transfer_per_token))
+    ttft = np.zeros(max(n, 1), dtype=np.float64)
+    res = SimResult()
+    _check(_lib.kairos_simulate(_c.byref(model), _c.byref(prefill), _c.byref(cfg), arr, n, ttft.ctypes.data_as(_vp),
+                                _c.byref(res)))
+    return {k: getattr(res, k) for k, _ in SimResult._fields_}, ttft[:n]
 
 
 def bf16_tensor(bits: np.ndarray, device="cuda") -> torch.Tensor:

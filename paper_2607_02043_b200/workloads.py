@@ -169,3 +169,25 @@ def make_config(index: int, *, chunk_len: Optional[int] = None, q_scale: float =
     if index == 4:
         return make_inputs("long_context", 4, [32768] * 32, 4096, 28672, q_scale=q_scale)
     raise ValueError(f"no such config index {index}")
+
+
+def make_arrivals(seed: int, n: int, rate: float, burst_every: float, burst_size: int, prompt_median: float = 3569.0,
+                  prompt_sigma: float = 0.8, prompt_lo: int = 64, prompt_hi: int = 16384, out_median: float = 200.0,
+                  out_sigma: float = 0.6, out_lo: int = 1, out_hi: int = 2000):
+    """Synthetic bursty arrivals for the policy simulator: a Poisson stream of `rate` requests per time
+    unit plus `burst_size` simultaneous-ish requests every `burst_every` time units (the paper's Bursty trace is proprietary,
+    PAPER.md:86-90; its prompt lengths have median 3569, P25/P90 = 2071/10336, i.e. lognormal sigma ~ 0.8).
+    Returns a list of (arrival, prompt_len, output_len) sorted by arrival.  No method arithmetic here."""
+    rng = np.random.default_rng(seed)
+    n_burst = 0
+    t_end = n / max(rate, 1e-12)
+    if burst_every > 0 and burst_size > 0:
+        n_burst = min(n // 2, int(t_end / burst_every) * burst_size)
+    base = np.cumsum(rng.exponential(1.0 / rate, n - n_burst))
+    bursts = []
+    for k in range(n_burst):
+        bursts.append((k // burst_size + 1) * burst_every + 1e-3 * burst_every * rng.random())
+    t = np.sort(np.concatenate([base, np.asarray(bursts, dtype=np.float64)]))
+    prompts = np.clip(np.rint(np.exp(math.log(prompt_median) + prompt_sigma * rng.standard_normal(n))), prompt_lo, prompt_hi).astype(np.int64)
+    outs = np.clip(np.rint(np.exp(math.log(out_median) + out_sigma * rng.standard_normal(n))), out_lo, out_hi).astype(np.int64)
+    return [(float(t[i]), int(prompts[i]), int(outs[i])) for i in range(n)]
