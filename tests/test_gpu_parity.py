@@ -428,3 +428,24 @@ def test_latency_table_matches_independently_timed_steps():
     assert med[0, 0, 0] < med[0, 0, 1] < med[0, 0, 2]
     grid, _ = ctx.step_latency_table([64, 256], [512, 2048], [0, 1024], warmup=3, reps=10, flush_l2=False)
     assert np.all(grid[1] > grid[0] * 0.98) and np.all(grid[:, 1] > grid[:, 0] * 0.98) and np.all(grid[:, :, 1] > grid[:, :, 0])
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_host_buffer_step_matches_oracle_every_row(cfg):
+    """kairos_mixed_step_host (the end-to-end leg bench.py times): HOST buffers in, HOST buffers out, the chunk appended by
+    the call itself.  Every row against the oracle, the pool bit-exact, and the byte counts it reports."""
+    from oracle import oracle
+    inp = W.make_config(cfg)
+    run = Hp.GpuRun(inp)
+    od = np.zeros((inp.n_dec, 16, 512), np.uint16)
+    oc = np.zeros((inp.chunk_len, 16, 512), np.uint16)
+    for _ in range(2):  # the second call re-uses the context's device staging
+        h2d, d2h = run.ctx.mixed_step_host(inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.q_chunk, inp.chunk_latent,
+                                           inp.chunk_k_rope, inp.chunk_page_table, inp.chunk_len, inp.prefix_len, od, oc)
+    pool_np = Hp.oracle_pool_after_append(inp)
+    assert np.array_equal(run.pool_bits(), pool_np)
+    rd, rc, _, _ = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
+                                     inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    Hp.assert_attention_close([W.bf16_bits_to_f32(od), W.bf16_bits_to_f32(oc)], [rd, rc], f"configs[{cfg}] through host buffers")
+    assert h2d == inp.q_dec.nbytes + inp.q_chunk.nbytes + inp.dec_page_tables.nbytes + inp.chunk_page_table.nbytes + inp.chunk_latent.nbytes + inp.chunk_k_rope.nbytes
+    assert d2h == od.nbytes + oc.nbytes
