@@ -4,7 +4,7 @@ The table is the input of the latency model of Eq. 4 that `ka
 `kairos_decide` consumes.  Default grid: BASELINE.json configs[3] (B = 256, K = 2048, C in {0 .. 8192}, 20 timed reps
 after 5 warm-ups) plus a B x K x C grid around it.  The pool is synthetic (N(0,1) bf16): this is a timing tool.
 
-  python -m paper_2607_02043_b200.latency_table --out profiles/r02_latency_table.json [--grid paper] [--no-flush]
+  python -m paper_2607_02043_b200.latency_table --out profiles/r02_latency_table.json.txt [--grid paper] [--no-flush]
 """
 from __future__ import annotations
 

@@ -4,7 +4,7 @@ model fitted on THIS machine's table: kairos_step_latency_table -> kairos_fit_la
 Latencies are ONE attention layer's, in microseconds, so the SLOs are per-layer budgets and the arrival rate is scaled to
 load two prefill nodes of that speed; the paper's absolute numbers (whole model, A100, proprietary trace) are context.
 
-  python -m paper_2607_02043_b200.policy_table --table profiles/r02_latency_table.json --out profiles/r02_policy_table.md
+  python -m paper_2607_02043_b200.policy_table --table profiles/r02_latency_table.json.txt --out profiles/r02_policy_table.md
 """
 from __future__ import annotations
 

@@ -5,7 +5,7 @@
 
 Latencies are ONE attention layer's, in microseconds (include/kairos.h units note), so tau here is a per-layer TBT budget.
 
-  python -m paper_2607_02043_b200.ttft_check --out profiles/r02_ttft_vs_model.json
+  python -m paper_2607_02043_b200.ttft_check --out profiles/r02_ttft_vs_model.json.txt
 """
 from __future__ import annotations
 

@@ -157,7 +157,7 @@ def test_fit_matches_restatement():
 
 
 def _table_samples():
-    path = os.path.join(ROOT, "profiles", "r02_latency_table.json")
+    path = os.path.join(ROOT, "profiles", "r02_latency_table.json.txt")
     d = json.load(open(path))
     rows = []
     for key in ("grid", "grid_prefix", "configs3"):
@@ -176,7 +176,7 @@ def _table_samples():
 
 def test_model_fitted_on_the_measured_table_holds_out_under_10_percent():
     """'on held-out traces ... MAPE < 10 %'.  The table is the committed output of kairos_step_latency_table
-    on a B200 (profiles/r02_latency_table.json); every third point is held out of the fit."""
+    on a B200 (profiles/r02_latency_table.json.txt); every third point is held out of the fit."""
     from paper_2607_02043_b200 import kairos as K
     rows = _table_samples()
     held = np.arange(len(rows)) % 3 == 1
