@@ -418,6 +418,26 @@ int kairos_absorb_q(kairos_ctx* ctx, const void* q_nope, const void* q_rope, con
 int kairos_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, int32_t n, void* v_out, void* cuda_stream);
 
 /*
+ * Measured launch order for a step shape.  The host planner (a0) ranks the orders in which the decode grid and the chunk's
+ * clusters take the SMs with a cost model; off the workloads it was calibrated on the model can be 10-30 % off the best
+ * order (profiles/r02_planner_offpoints.md).  This call runs the step given (same arguments and preconditions as
+ * kairos_mixed_step: the chunk already appended) under each candidate order -- the planner's own, every cluster first, a
+ * few clusters first, the decode grid first beside n clusters, one queue -- `reps` times each after two warm-ups, timed with
+ * CUDA events on `cuda_stream` (it SYNCHRONISES after every run), and pins the fastest for every later kairos_mixed_step /
+ * kairos_run_schedule step of this context with the same shape (same number of decodes, same page count per decode, same
+ * chunk_len, same number of prefix pages), unless it beats the planner's order by less than 3 %.  Results of every
+ * candidate are the same attention outputs (every order is parity-tested); out_dec / out_chunk hold the last run's.
+ *   chosen_mode  HOST or NULL: the pinned order in kairos_plan_dump's pair_mode encoding, -1 = the planner's own was kept
+ *   chosen_us / default_us  HOST or NULL: median step time under the pinned order / under the planner's own
+ * A step with no decodes or no chunk has one grid and nothing to order (returns at once).  Errors as kairos_mixed_step.
+ */
+int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                     int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len,
+                     const void* q_chunk, const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec,
+                     void* out_chunk, int32_t reps, int32_t* chosen_mode, double* chosen_us, double* default_us,
+                     void* cuda_stream);
+
+/*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
  *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;

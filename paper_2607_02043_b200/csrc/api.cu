@@ -32,6 +32,26 @@ static int check_ctx(const kairos_ctx* ctx) {
     return KAIROS_OK;
 }
 
+// Shape key of a step for the tuned launch orders: what the planner's decision depends on at page granularity.
+static uint64_t shape_key(const int32_t* lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len) {
+    uint64_t h = 1469598103934665603ull;
+    auto mix = [&](uint64_t v) { h = (h ^ v) * 1099511628211ull; };
+    mix(uint64_t(n_dec));
+    for (int32_t i = 0; i < n_dec; ++i) mix(uint64_t((lens[i] + kPage - 1) / kPage));
+    mix(uint64_t(chunk_len));
+    mix(uint64_t((prefix_len + kPage - 1) / kPage));
+    return h;
+}
+
+// The launch order the planner is asked for: the test knob if set, else what kairos_tune_step measured for this shape, else -1 (decide).
+static int32_t pair_mode_for(const kairos_ctx* ctx, const int32_t* lens, int32_t n_dec, int32_t chunk_len, int32_t prefix_len) {
+    if (ctx->force_pairs != -1 || ctx->tuned.empty() || chunk_len == 0) return ctx->force_pairs;
+    const uint64_t k = shape_key(lens, n_dec, chunk_len, prefix_len);
+    for (const TunedShape& t : ctx->tuned)
+        if (t.key == k) return t.pair_mode;
+    return -1;
+}
+
 static bool same_args(const StepArgs& a, const StepArgs& b) {
     return a.n_dec == b.n_dec && a.q_dec == b.q_dec && a.dec_page_tables == b.dec_page_tables &&
            a.dec_table_stride == b.dec_table_stride && a.chunk_len == b.chunk_len && a.prefix_len == b.prefix_len &&
@@ -209,7 +229,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     const StepArgs a{n_dec, q_dec, dec_page_tables, dec_table_stride, chunk_len, prefix_len,
                      q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk};
     const int32_t target_ctas = umma_resident_ctas(ctx);
-    const int32_t pair_mode = ctx->force_pairs;
+    const int32_t pair_mode = pair_mode_for(ctx, dec_ctx_lens, n_dec, chunk_len, prefix_len);
 
     // ---- a0: find the plan (exact hit: same lengths; structural hit: same page count per request), else build it
     PlanEntry* hit = nullptr;
@@ -463,7 +483,7 @@ extern "C" int kairos_run_schedule(kairos_ctx* ctx, int32_t n_dec, const void* q
             if (grow) for (int32_t j = 0; j < n_dec; ++j) lens[j] = dec_ctx_lens[j] + i + 1;
             PlanEntry& e = sc.steps[i];
             build_plan(lens.data(), n_dec, chunk_sizes[i], prefix_len + int32_t(done), umma_resident_ctas(ctx), umma_chunk_tile_tokens(),
-                       &e.plan, ctx->force_pairs, pair_tile_tokens());
+                       &e.plan, pair_mode_for(ctx, lens.data(), n_dec, chunk_sizes[i], prefix_len + int32_t(done)), pair_tile_tokens());
             layout_entry(e);
             sc.plan_off[i] = off;
             off += (e.total_bytes + 255) / 256 * 256;
@@ -642,6 +662,81 @@ int kairos_destroy(kairos_ctx* ctx) {
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
     delete ctx;
+    return KAIROS_OK;
+}
+
+int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                     const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len, const void* q_chunk,
+                     const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk, int32_t reps,
+                     int32_t* chosen_mode, double* chosen_us, double* default_us, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (reps < 1) return fail(KAIROS_ERR_INVALID_ARG, "tune: reps < 1");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (chosen_mode) *chosen_mode = -1;
+    if (chunk_len <= 0 || n_dec <= 0) {  // one grid only: nothing to order
+        if (chosen_us) *chosen_us = 0.0;
+        if (default_us) *default_us = 0.0;
+        return KAIROS_OK;
+    }
+    const int32_t tiles = (chunk_len + pair_tile_tokens() - 1) / pair_tile_tokens();
+    const int32_t max_pairs = std::min(tiles, ctx->sm_count / 2);
+    // candidates: the planner's own choice first, then every cluster first, a few clusters first, decode grid first beside n clusters
+    std::vector<int32_t> modes{-1, -(max_pairs + 1)};
+    for (int32_t n : {8, 16, 24, 32, 48})
+        if (n < max_pairs) modes.push_back(-(n + 1));
+    for (int32_t n : {20, 28, 36, 44, 52, 60})
+        if (n < max_pairs && ctx->sm_count - 2 * n >= 2) modes.push_back(n);
+    if (tiles <= 64) modes.push_back(0);
+    const uint64_t key = shape_key(dec_ctx_lens, n_dec, chunk_len, prefix_len);
+    for (size_t i = 0; i < ctx->tuned.size(); ++i)
+        if (ctx->tuned[i].key == key) { ctx->tuned.erase(ctx->tuned.begin() + long(i)); break; }
+    const int saved_force = ctx->force_pairs, saved_graph = ctx->use_graph;
+    ctx->use_graph = 0;  // candidates are timed as direct launches: the order of the grids is what differs
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = KAIROS_OK;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = fail(KAIROS_ERR_CUDA, "tune: cudaEventCreate failed");
+    double best = 0.0, def = 0.0;
+    int32_t best_mode = -1;
+    std::vector<double> ts;
+    for (size_t m = 0; m < modes.size() && rc == KAIROS_OK; ++m) {
+        ctx->force_pairs = modes[m];
+        ts.clear();
+        for (int32_t it = 0; it < 2 + reps && rc == KAIROS_OK; ++it) {
+            if (cudaEventRecord(e0, stream) != cudaSuccess) { rc = fail(KAIROS_ERR_CUDA, "tune: cudaEventRecord failed"); break; }
+            rc = mixed_step_impl(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, chunk_len, prefix_len, q_chunk,
+                                 chunk_page_table, chunk_table_len, out_dec, out_chunk, nullptr, nullptr, stream);
+            if (rc != KAIROS_OK) break;
+            if (cudaEventRecord(e1, stream) != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess) { rc = fail(KAIROS_ERR_CUDA, "tune: step failed on the device"); break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (it >= 2) ts.push_back(double(ms) * 1e3);
+        }
+        if (rc != KAIROS_OK) break;
+        std::sort(ts.begin(), ts.end());
+        const double med = ts[ts.size() / 2];
+        if (m == 0) def = med;
+        if (m == 0 || med < best) { best = med; best_mode = modes[m]; }
+    }
+    ctx->force_pairs = saved_force;
+    ctx->use_graph = saved_graph;
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (rc != KAIROS_OK) return rc;
+    if (best_mode != -1 && best < 0.97 * def) {  // pinned only when it beats the planner's own order by more than the noise
+        if (ctx->tuned.size() >= 256) ctx->tuned.erase(ctx->tuned.begin());
+        ctx->tuned.push_back(TunedShape{key, best_mode});
+    } else {
+        best_mode = -1;
+        best = def;
+    }
+    for (PlanEntry& e : ctx->plans) {  // plans of this shape were built under forced orders: drop them
+        for (PlanBuffer& b : e.buf) drop_graph(b);
+        e.valid = false;
+    }
+    ctx->schedule.key.clear();
+    if (chosen_mode) *chosen_mode = best_mode;
+    if (chosen_us) *chosen_us = best;
+    if (default_us) *default_us = def;
     return KAIROS_OK;
 }
 

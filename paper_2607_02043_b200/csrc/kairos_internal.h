@@ -133,6 +133,12 @@ struct ScheduleCache {
     int kernels = 0;
 };
 
+// kairos_tune_step: the launch order measured fastest for a step shape (page counts per decode, C, P)
+struct TunedShape {
+    uint64_t key = 0;      // hash of (n_dec, page count of every decode, chunk_len, prefix pages)
+    int32_t pair_mode = -1;
+};
+
 struct QMapCache {  // a tensor map stays valid while (pointer, rows) do not change
     const void* ptr = nullptr;
     uint64_t rows = 0;
@@ -156,6 +162,7 @@ struct kairos_ctx {
     int force_pairs = -1;         // -1 auto, 0 never use the pair kernel, n > 0 decode grid first beside n clusters, -(n + 1) n clusters first
     int force_dec_only = -1;      // 0 = never use the decode-only instantiation
     int use_copy_stream = 1, use_graph = 1, use_plan_cache = 1;
+    std::vector<kairos::TunedShape> tuned;   // filled by kairos_tune_step; consulted when force_pairs == -1
     static constexpr int kPlanEntries = 8;
     kairos::PlanEntry plans[kPlanEntries];
     uint64_t plan_clock = 0;

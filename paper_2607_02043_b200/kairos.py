@@ -115,6 +115,8 @@ _lib.kairos_absorb_q.argtypes = [_vp, _vp, _vp, _vp, _i32, _vp, _vp]
 _lib.kairos_absorb_q.restype = _c.c_int
 _lib.kairos_project_out.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp]
 _lib.kairos_project_out.restype = _c.c_int
+_lib.kairos_tune_step.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
+_lib.kairos_tune_step.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
 _lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
@@ -125,7 +127,7 @@ _lib.kairos_version.restype = _c.c_char_p
 EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_append_latent",
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
-           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate",
+           "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate", "kairos_tune_step",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -229,6 +231,19 @@ class Kairos:
                                       _dp(chunk_page_table), int(chunk_page_table.numel()) if C else 0, _dp(out_dec),
                                       _dp(out_chunk), _dp(lse_dec), _dp(lse_chunk), _stream_ptr(stream)))
         return out_dec, out_chunk, lse_dec, lse_chunk
+
+    def tune_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
+                  prefix_len: int, out_dec, out_chunk, reps: int = 5, stream=None):
+        """kairos_tune_step: (pinned order or -1, its median us, the planner's own order's median us).  Synchronises."""
+        lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        B, C = int(lens.shape[0]), int(chunk_len)
+        stride = int(dec_page_tables.shape[1]) if B else 1
+        mode, us, dus = _i32(-1), _c.c_double(0.0), _c.c_double(0.0)
+        _check(_lib.kairos_tune_step(self._h, B, _dp(q_dec), _dp(dec_page_tables), stride, lens.ctypes.data_as(_vp), C,
+                                     int(prefix_len), _dp(q_chunk), _dp(chunk_page_table),
+                                     int(chunk_page_table.numel()) if C else 0, _dp(out_dec), _dp(out_chunk), int(reps),
+                                     _c.byref(mode), _c.byref(us), _c.byref(dus), _stream_ptr(stream)))
+        return int(mode.value), float(us.value), float(dus.value)
 
     def bind_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
                   prefix_len: int, out_dec, out_chunk, lse_dec=None, lse_chunk=None, chunk_latent=None, chunk_k_rope=None):

@@ -449,3 +449,35 @@ def test_host_buffer_step_matches_oracle_every_row(cfg):
     Hp.assert_attention_close([W.bf16_bits_to_f32(od), W.bf16_bits_to_f32(oc)], [rd, rc], f"configs[{cfg}] through host buffers")
     assert h2d == inp.q_dec.nbytes + inp.q_chunk.nbytes + inp.dec_page_tables.nbytes + inp.chunk_page_table.nbytes + inp.chunk_latent.nbytes + inp.chunk_k_rope.nbytes
     assert d2h == od.nbytes + oc.nbytes
+
+
+def test_tuned_launch_order_keeps_parity_and_is_used():
+    """kairos_tune_step pins a measured launch order for a shape; later steps of that shape use it (also through
+    kairos_run_schedule / Kairos.bind_step) and still match the oracle on every row."""
+    import torch
+    from oracle import oracle
+    inp = W.make_config(1)
+    run = Hp.GpuRun(inp)
+    run.append()
+    od, oc, ld, lc = run.ctx.mixed_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, inp.chunk_len, inp.prefix_len)
+    before = run.ctx.last_plan_info()
+    mode, us, dus = run.ctx.tune_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, inp.chunk_len, inp.prefix_len, od, oc, reps=3)
+    assert us > 0 and dus > 0 and us <= dus
+    pool_np = Hp.oracle_pool_after_append(inp)
+    rd, rc, rld, rlc = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
+                                         inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    f = lambda t: W.bf16_bits_to_f32(run.K.bf16_bits(t))
+    for _ in range(3):
+        got = run.step(reuse_outputs=True)
+        Hp.assert_attention_close(got[:2], [rd, rc], "after tuning")
+    after = run.ctx.last_plan_info()
+    if mode != -1:  # a different order was pinned: the plan reflects it
+        assert (after["chunk_pairs"], after["dec_ctas_first"]) != (before["chunk_pairs"], before["dec_ctas_first"]) or mode == 0
+    bound = run.ctx.bind_step(run.q_dec, run.dec_pt, inp.dec_ctx_lens, run.q_chunk, run.chunk_pt, inp.chunk_len, inp.prefix_len,
+                              *run.out, run.latent, run.k_rope)
+    for _ in range(3):
+        bound.run()
+    torch.cuda.synchronize()
+    Hp.assert_attention_close([f(run.out[0]), f(run.out[1])], [rd, rc], "bound step after tuning")
+    info = run.ctx.last_plan_info()
+    assert (info["chunk_pairs"], info["dec_ctas_first"]) == (after["chunk_pairs"], after["dec_ctas_first"])
