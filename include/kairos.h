@@ -438,6 +438,39 @@ int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const in
                      void* cuda_stream);
 
 /*
+ * the fp8 latent cache ("an fp8 latent-cache variant (halves the decode roofline)").  The paper has no
+ * such passage; the format is DESIGN.md reading G23:
+ *   one cached token = 512 latent values as e4m3 codes (OCP fp8: bias 7, no infinity, largest finite 448) + ONE float32 scale
+ *   + its 64 RoPE key values in bf16 = 644 bytes (bf16 cache: 1,152).  A page of 64 tokens is KAIROS_FP8_PAGE_BYTES = 41,216
+ *   bytes:  codes u8 [64][512]  |  RoPE bf16 [64][64] at byte 32,768  |  scales f32 [64] at byte 40,960.
+ *   Quantisation of token t (float32, IEEE round to nearest even): amax = max_d |c_t[d]|;  s_t = amax / 448 (1 when amax = 0);
+ *   code = e4m3_rne_satfinite(c_t[d] / s_t).  The cached latent is s_t * value(code); attention is the definition at the top of
+ *   this file over those values (q in bf16, fp32 accumulation, bf16 out).  Inside the kernel the MMAs are tcgen05 kind::f8f6f4
+ *   on the codes themselves; q and the softmax weights enter them as a sum of two e4m3 terms (a 4-bit head and the 4-bit
+ *   remainder), which keeps them at bf16's precision -- see DESIGN.md 6.7 for the error budget.
+ *
+ * kairos_fp8_attach     tells the context about an fp8 pool and the scratch the decode call stages its quantised queries in.
+ *                       pool8 DEVICE [num_pages][41,216] bytes, 128-byte aligned; scratch DEVICE, 128-byte aligned, at least
+ *                       kairos_fp8_scratch_bytes(max_decodes) bytes.  Both stay caller-owned and must outlive the context or
+ *                       the next attach.  The bf16 pool given at create time is untouched: a context can serve both.
+ * kairos_fp8_append     as kairos_append_latent (same arguments, same indexing, same errors) but quantises into the attached
+ *                       fp8 pool.  BIT-EXACT against the definition above: codes, scales and RoPE bytes.
+ * kairos_fp8_decode     as kairos_mixed_step with chunk_len = 0 over the fp8 pool: n_dec decodes, request i attends its first
+ *                       dec_ctx_lens[i] cached tokens through row i of dec_page_tables.  Same planner (a0), split partials,
+ *                       LSE combine, plan cache and graph replay as the bf16 step; one extra kernel quantises q first.
+ *                       Stale slots of a request's last page never reach a result (any bit pattern, NaN codes included).
+ *                       n_dec must not exceed the max_decodes the scratch was sized for.
+ * Errors: INVALID_ARG (NULL / misaligned / sizes / no pool attached), WORKSPACE, CUDA.
+ */
+#define KAIROS_FP8_PAGE_BYTES 41216
+size_t kairos_fp8_scratch_bytes(int32_t max_decodes);
+int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes);
+int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
+                      int32_t table_len, int32_t start_pos, void* cuda_stream);
+int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                      int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream);
+
+/*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
  *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;

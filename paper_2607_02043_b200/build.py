@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkairos.so")
-SOURCES = ["api.cu", "plan.cpp", "decide.cpp", "simulate.cpp", "append.cu", "proj.cu", "attn_umma.cu", "attn_pair.cu"]
+SOURCES = ["api.cu", "plan.cpp", "decide.cpp", "simulate.cpp", "append.cu", "proj.cu", "fp8.cu", "attn_umma.cu", "attn_pair.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "--expt-relaxed-constexpr",

@@ -56,7 +56,7 @@ static bool same_args(const StepArgs& a, const StepArgs& b) {
     return a.n_dec == b.n_dec && a.q_dec == b.q_dec && a.dec_page_tables == b.dec_page_tables &&
            a.dec_table_stride == b.dec_table_stride && a.chunk_len == b.chunk_len && a.prefix_len == b.prefix_len &&
            a.q_chunk == b.q_chunk && a.chunk_page_table == b.chunk_page_table && a.out_dec == b.out_dec &&
-           a.out_chunk == b.out_chunk && a.lse_dec == b.lse_dec && a.lse_chunk == b.lse_chunk;
+           a.out_chunk == b.out_chunk && a.lse_dec == b.lse_dec && a.lse_chunk == b.lse_chunk && a.fp8 == b.fp8;
 }
 
 static void drop_graph(PlanBuffer& b) {
@@ -125,7 +125,9 @@ static int launch_step_kernels(kairos_ctx* ctx, const PlanEntry& e, const PlanBu
     // Roofline leg of bench.py: one pair of events around the attention kernels of the step (the decode grid and, when the
     // planner uses it, the concurrent pair grid).
     if (e0) KAIROS_CUDA_TRY(cudaEventRecord(e0, stream));
-    if (n_pairs > 0 && have_queue) {
+    if (a.fp8) {
+        if (int rc = launch_fp8_decode(ctx, a, dev_items, n_items, stream)) return rc;
+    } else if (n_pairs > 0 && have_queue) {
         // The two grids share the SMs in time (plan.cpp::choose_pairs).  dec_ctas > 0: the decode grid goes first, as 2-CTA
         // clusters on dec_ctas SMs (whole TPCs), then one chunk cluster per SM pair -- those that do not fit yet start when
         // the decode CTAs exit.  dec_ctas == 0: the clusters go first and the decode CTAs follow as SMs free up.  The second
@@ -201,7 +203,7 @@ static bool capture_graph(kairos_ctx* ctx, const PlanEntry& e, PlanBuffer& b, co
 int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                     int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len,
                     const void* q_chunk, const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec,
-                    void* out_chunk, float* lse_dec, float* lse_chunk, cudaStream_t stream) {
+                    void* out_chunk, float* lse_dec, float* lse_chunk, cudaStream_t stream, int32_t fp8) {
     if (int rc = check_ctx(ctx)) return rc;
     if (n_dec < 0 || chunk_len < 0 || prefix_len < 0) return fail(KAIROS_ERR_INVALID_ARG, "negative size");
     auto misaligned = [](const void* p, uintptr_t a) { return reinterpret_cast<uintptr_t>(p) % a != 0; };
@@ -227,9 +229,9 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     if (n_dec == 0 && chunk_len == 0) return KAIROS_OK;
 
     const StepArgs a{n_dec, q_dec, dec_page_tables, dec_table_stride, chunk_len, prefix_len,
-                     q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk};
+                     q_chunk, chunk_page_table, out_dec, out_chunk, lse_dec, lse_chunk, fp8};
     const int32_t target_ctas = umma_resident_ctas(ctx);
-    const int32_t pair_mode = pair_mode_for(ctx, dec_ctx_lens, n_dec, chunk_len, prefix_len);
+    const int32_t pair_mode = fp8 ? 0 : pair_mode_for(ctx, dec_ctx_lens, n_dec, chunk_len, prefix_len);
 
     // ---- a0: find the plan (exact hit: same lengths; structural hit: same page count per request), else build it
     PlanEntry* hit = nullptr;
@@ -242,7 +244,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
             if (!e.valid) { if (victim->valid) victim = &e; continue; }
             if (victim->valid && e.stamp < victim->stamp) victim = &e;
             if (e.n_dec != n_dec || e.chunk_len != chunk_len || e.prefix_len != prefix_len || e.target_ctas != target_ctas ||
-                e.pair_mode != pair_mode)
+                e.pair_mode != pair_mode || e.fp8 != fp8)
                 continue;
             if (n_dec == 0 || std::memcmp(e.lens.data(), dec_ctx_lens, sizeof(int32_t) * size_t(n_dec)) == 0) { hit = &e; break; }
             if (!structural) {
@@ -273,7 +275,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
         const size_t ws_needed = kCounterBytes + size_t(e->plan.n_partial_slots) * kPartialSlotBytes;
         if (ws_needed > ctx->cfg.workspace_bytes)
             return fail(KAIROS_ERR_WORKSPACE, "workspace too small: need " + std::to_string(ws_needed) + " bytes");
-        e->n_dec = n_dec; e->chunk_len = chunk_len; e->prefix_len = prefix_len; e->target_ctas = target_ctas; e->pair_mode = pair_mode;
+        e->n_dec = n_dec; e->chunk_len = chunk_len; e->prefix_len = prefix_len; e->target_ctas = target_ctas; e->pair_mode = pair_mode; e->fp8 = fp8;
         e->lens.assign(dec_ctx_lens, dec_ctx_lens + n_dec);
         layout_entry(*e);
         e->cur = 0;
@@ -327,7 +329,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     ctx->last_info[1] = plan.n_decode_items;
     ctx->last_info[2] = plan.n_chunk_items + int64_t(plan.pair_items.size());
     ctx->last_info[3] = std::min<int64_t>(plan.n_pairs > 0 && plan.dec_ctas > 0 ? plan.dec_ctas : umma_resident_ctas(ctx), int64_t(plan.items.size()));
-    ctx->last_info[4] = kernels_of(plan);
+    ctx->last_info[4] = kernels_of(plan) + (fp8 ? 1 : 0);  // + the query preparation
     ctx->last_info[5] = int64_t(kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes);
     ctx->last_info[6] = plan.n_pairs;
     ctx->last_info[7] = cache_state;
@@ -818,6 +820,42 @@ int kairos_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
     return mixed_step_impl(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, chunk_len, prefix_len,
                            q_chunk, chunk_page_table, chunk_table_len, out_dec, out_chunk, lse_dec, lse_chunk,
                            static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ---- the fp8 latent cache ------------------------------------------------------------------------------
+size_t kairos_fp8_scratch_bytes(int32_t max_decodes) { return fp8_scratch_bytes(max_decodes); }
+
+int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!pool8 || !scratch || num_pages < 1) return fail(KAIROS_ERR_INVALID_ARG, "NULL pool8 / scratch or num_pages < 1");
+    if (reinterpret_cast<uintptr_t>(pool8) % 128 || reinterpret_cast<uintptr_t>(scratch) % 128)
+        return fail(KAIROS_ERR_INVALID_ARG, "pool8 / scratch must be 128-byte aligned");
+    if (scratch_bytes < fp8_scratch_bytes(1)) return fail(KAIROS_ERR_WORKSPACE, "scratch smaller than kairos_fp8_scratch_bytes(1)");
+    return fp8_attach(ctx, pool8, num_pages, scratch, scratch_bytes);
+}
+
+int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
+                      int32_t table_len, int32_t start_pos, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!ctx->fp8.attached) return fail(KAIROS_ERR_INVALID_ARG, "no fp8 pool attached (kairos_fp8_attach)");
+    if (n_tokens < 0 || start_pos < 0 || table_len < 0) return fail(KAIROS_ERR_INVALID_ARG, "negative size");
+    if (n_tokens == 0) return KAIROS_OK;
+    if (!latent || !k_rope || !page_table) return fail(KAIROS_ERR_INVALID_ARG, "NULL pointer");
+    if (int64_t(start_pos) + n_tokens > int64_t(table_len) * kPage)
+        return fail(KAIROS_ERR_INVALID_ARG, "start_pos + n_tokens beyond table_len*64");
+    if (reinterpret_cast<uintptr_t>(latent) % 16 || reinterpret_cast<uintptr_t>(k_rope) % 16)
+        return fail(KAIROS_ERR_INVALID_ARG, "latent / k_rope must be 16-byte aligned");
+    return launch_fp8_append(ctx, latent, k_rope, n_tokens, page_table, start_pos, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
+                      int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!ctx->fp8.attached) return fail(KAIROS_ERR_INVALID_ARG, "no fp8 pool attached (kairos_fp8_attach)");
+    if (n_dec > ctx->fp8.max_decodes)
+        return fail(KAIROS_ERR_WORKSPACE, "n_dec beyond the decodes the fp8 scratch was sized for: " + std::to_string(ctx->fp8.max_decodes));
+    return mixed_step_impl(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, 0, 0, nullptr, nullptr, 0, out_dec,
+                           nullptr, lse_dec, nullptr, static_cast<cudaStream_t>(cuda_stream), /*fp8=*/1);
 }
 
 int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,

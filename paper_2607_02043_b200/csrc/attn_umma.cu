@@ -780,6 +780,19 @@ int encode_2d_map(QMapCache* cache, const void* ptr, uint64_t inner, uint64_t ro
     return KAIROS_OK;
 }
 
+int encode_tiled_map(CUtensorMap* out, bool u8, int rank, const void* ptr, const uint64_t* dims, const uint64_t* strides, const uint32_t* box) {
+    if (!g_encode) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    cuuint64_t d[3], st[2];
+    cuuint32_t bx[3], es[3] = {1, 1, 1};
+    for (int i = 0; i < rank; ++i) { d[i] = dims[i]; bx[i] = box[i]; }
+    for (int i = 0; i + 1 < rank; ++i) st[i] = strides[i];
+    const CUresult r = g_encode(out, u8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, cuuint32_t(rank),
+                                const_cast<void*>(ptr), d, st, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(KAIROS_ERR_CUDA, "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)));
+    return KAIROS_OK;
+}
+
 int umma_init(kairos_ctx* ctx) {
     if (!g_encode) {
         void* fn = nullptr;

@@ -90,6 +90,7 @@ struct StepArgs {
     void* out_chunk;
     float* lse_dec;
     float* lse_chunk;
+    int32_t fp8 = 0;  // 1: kairos_fp8_decode (decodes only, over the attached fp8 pool)
 };
 
 // Device-resident copy of one plan's work lists (items | combines | pair items) with its pinned source.
@@ -112,12 +113,22 @@ struct PlanBuffer {
 struct PlanEntry {
     bool valid = false;
     uint64_t stamp = 0;                // LRU clock
-    int32_t n_dec = 0, chunk_len = 0, prefix_len = 0, target_ctas = 0, pair_mode = 0;
+    int32_t n_dec = 0, chunk_len = 0, prefix_len = 0, target_ctas = 0, pair_mode = 0, fp8 = 0;
     std::vector<int32_t> lens;
     Plan plan;
     size_t items_bytes = 0, comb_off = 0, comb_bytes = 0, pair_off = 0, pair_bytes = 0, total_bytes = 0;
     PlanBuffer buf[2];
     int cur = 0;
+};
+
+// kairos_fp8_attach: the fp8 pool, its tensor maps and the scratch of the query preparation
+struct Fp8State {
+    bool attached = false;
+    void* pool8 = nullptr;
+    int32_t num_pages = 0;
+    void* scratch = nullptr;           // q8 [max_decodes][16 KB] | ginv [max_decodes][16] f32
+    int32_t max_decodes = 0;
+    CUtensorMap lat_map, rope_map, q8_map;
 };
 
 // kairos_run_schedule: the plans of every step of the last schedule, their device copies and the captured graph
@@ -176,6 +187,7 @@ struct kairos_ctx {
     void* table_buf = nullptr;
     size_t table_bytes = 0;
     void* flush_buf = nullptr;
+    kairos::Fp8State fp8;
 };
 
 namespace kairos {
@@ -184,7 +196,7 @@ namespace kairos {
 int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
                     const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len, const void* q_chunk,
                     const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk, float* lse_dec,
-                    float* lse_chunk, cudaStream_t stream);
+                    float* lse_chunk, cudaStream_t stream, int32_t fp8 = 0);
 
 // ---- kernel launchers (each returns a kairos_status) -----------------------------------------------
 int launch_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
@@ -208,6 +220,15 @@ int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
 // projections either side of the attention (proj.cu)
 int launch_absorb_q(kairos_ctx* ctx, const void* q_nope, const void* q_rope, const void* w_uk_t, int32_t n, void* q_out, cudaStream_t stream);
 int launch_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, int32_t n, void* v_out, cudaStream_t stream);
+
+// fp8 latent cache (fp8.cu)
+// tensor map of rank 2 or 3 over bytes (u8) or bf16 elements, SWIZZLE_128B; strides in bytes for dimensions 1..rank-1
+int encode_tiled_map(CUtensorMap* out, bool u8, int rank, const void* ptr, const uint64_t* dims, const uint64_t* strides, const uint32_t* box);
+size_t fp8_scratch_bytes(int32_t max_decodes);
+int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes);
+int launch_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
+                      int32_t start_pos, cudaStream_t stream);
+int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, cudaStream_t stream);
 
 // chunk tiles on 2-CTA clusters (attn_pair.cu)
 int pair_tile_tokens();

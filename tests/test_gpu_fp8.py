@@ -1,0 +1,188 @@
+"""GPU parity of the fp8 latent cache (include/kairos.h kairos_fp8_*): the quantising append bit for bit,
+the decode attention within the bf16 path's tolerance, against oracle/fp8_oracle.py on the same seeded inputs.
+
+Both sides build their own fp8 pool from the same bf16 tokens (the workloads module's draws): the oracle with numpy, the
+library with kairos_fp8_append.  The pools start from the same random bytes, so stale slots hold arbitrary codes (NaN codes
+included) on both sides."""
+import numpy as np
+import pytest
+
+from oracle import fp8_oracle as F
+from oracle import oracle as O
+from paper_2607_02043_b200 import workloads as W
+from tests.helpers import MAX_ABS_TOL, REL_L2_TOL, errors
+
+pytestmark = pytest.mark.gpu
+
+
+class Fp8Run:
+    def __init__(self, inp: W.MixedStepInputs, oracle_requests=None, seed=99, knobs=None):
+        import torch
+        from paper_2607_02043_b200 import kairos as K
+        self.K, self.torch, self.inp = K, torch, inp
+        rng = np.random.default_rng(seed)
+        init = rng.integers(0, 256, (inp.num_pages, F.PAGE_BYTES), dtype=np.uint8)
+        self.pool8_ref = init.copy()
+        self.pool8 = torch.from_numpy(init).cuda()
+        self.pool16 = K.bf16_tensor(inp.pool)   # the context's bf16 pool (untouched by the fp8 calls)
+        self.ws = torch.empty(K.workspace_bytes(max(inp.n_dec, 1), 1), dtype=torch.uint8, device="cuda")
+        self.ctx = K.Kairos(self.pool16, self.ws, inp.softmax_scale)
+        for k, v in (knobs or {}).items():
+            self.ctx.debug_set(k, v)
+        self.ctx.fp8_attach(self.pool8, max(inp.n_dec, 1))
+        self.dec_pt = torch.from_numpy(inp.dec_page_tables).cuda()
+        self.q_dec = K.bf16_tensor(inp.q_dec)
+        self.oracle_requests = list(range(inp.n_dec)) if oracle_requests is None else list(oracle_requests)
+        # every request's tokens: gathered from the bf16 synthetic pool, quantised into both fp8 pools
+        for i in range(inp.n_dec):
+            L = int(inp.dec_ctx_lens[i])
+            tok = O.gather(inp.pool, inp.dec_page_tables[i], L)
+            lat, rope = np.ascontiguousarray(tok[:, :512]), np.ascontiguousarray(tok[:, 512:])
+            self.ctx.fp8_append(K.bf16_tensor(lat), K.bf16_tensor(rope), self.dec_pt[i], 0)
+            if i in self.oracle_requests:
+                F.append(self.pool8_ref, lat, rope, inp.dec_page_tables[i], 0)
+        torch.cuda.synchronize()
+
+    def check_pool(self):
+        got = self.pool8.cpu().numpy()
+        for i in self.oracle_requests:
+            n = (int(self.inp.dec_ctx_lens[i]) + 63) // 64
+            for pg in self.inp.dec_page_tables[i, :n]:
+                np.testing.assert_array_equal(got[pg], self.pool8_ref[pg], err_msg=f"request {i} page {pg}")
+
+    def decode(self, **kw):
+        od, lse = self.ctx.fp8_decode(self.q_dec, self.dec_pt, self.inp.dec_ctx_lens, **kw)
+        self.torch.cuda.synchronize()
+        return W.bf16_bits_to_f32(self.K.bf16_bits(od)), lse.cpu().numpy(), (od, lse)
+
+    def reference(self):
+        idx = np.asarray(self.oracle_requests)
+        return F.decode(self.pool8_ref, self.inp.q_dec[idx], self.inp.dec_page_tables[idx], self.inp.dec_ctx_lens[idx], self.inp.softmax_scale)
+
+
+def _assert_close(out, lse, ref_out, ref_lse, what):
+    ma, rl = errors(out, ref_out)
+    assert np.isfinite(out).all(), what
+    assert ma <= MAX_ABS_TOL and rl <= REL_L2_TOL, f"{what}: max-abs {ma:.3e} rel-L2 {rl:.3e}"
+    assert np.abs(lse - ref_lse).max() <= 2e-3, f"{what}: lse {np.abs(lse - ref_lse).max():.3e}"
+
+
+@pytest.mark.parametrize("lens", [[64], [1], [63, 65], [1, 63, 64, 65, 200, 333, 1000, 2500]])
+def test_append_bit_exact_and_decode_parity_small(lens):
+    inp = W.make_inputs("fp8_small", 11, lens, 0, 0)
+    r = Fp8Run(inp)
+    r.check_pool()
+    out, lse, _ = r.decode()
+    ref_out, ref_lse = r.reference()
+    _assert_close(out, lse, ref_out, ref_lse, f"lens {lens}")
+
+
+def test_append_ragged_positions_bit_exact():
+    """appends that start and end inside pages, in several calls, as a growing request does"""
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    inp = W.make_inputs("fp8_ragged", 12, [300], 0, 0)
+    r = Fp8Run(inp)
+    rng = np.random.default_rng(5)
+    pos = 300 - 300  # rewrite the request piecewise from position 0 with fresh tokens
+    pt = inp.dec_page_tables[0]
+    for n in [1, 62, 2, 64, 100, 71]:
+        lat = W.f32_to_bf16_bits(rng.standard_normal((n, 512)).astype(np.float32) * np.float32(rng.uniform(0.01, 30)))
+        rope = W.f32_to_bf16_bits(rng.standard_normal((n, 64)).astype(np.float32))
+        if n == 2:
+            lat[0] = 0  # an all-zero token: scale 1, codes 0
+        r.ctx.fp8_append(K.bf16_tensor(lat), K.bf16_tensor(rope), r.dec_pt[0], pos)
+        F.append(r.pool8_ref, lat, rope, pt, pos)
+        pos += n
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(r.pool8.cpu().numpy(), r.pool8_ref)
+
+
+def test_sharp_softmax_and_wide_scale_range():
+    """q_scale 1.0 (peaked softmax) and token magnitudes spread over 2^-10 .. 2^10: the scale rides the softmax weight"""
+    inp = W.make_inputs("fp8_sharp", 13, [500, 129, 2000, 70], 0, 0, q_scale=1.0)
+    rng = np.random.default_rng(6)
+    f = W.bf16_bits_to_f32(inp.pool)
+    f[:, :, :512] *= np.exp2(rng.integers(-10, 11, (inp.num_pages, 64, 1))).astype(np.float32)
+    inp.pool[:] = W.f32_to_bf16_bits(f)
+    r = Fp8Run(inp)
+    r.check_pool()
+    out, lse, _ = r.decode()
+    ref_out, ref_lse = r.reference()
+    ma, rl = errors(out, ref_out)
+    scale = np.abs(ref_out).max()
+    assert np.isfinite(out).all()
+    assert ma <= MAX_ABS_TOL * max(1.0, scale) and rl <= REL_L2_TOL, (ma, rl, scale)
+    assert np.abs(lse - ref_lse).max() <= 5e-3
+
+
+def test_repeated_calls_replay_the_same_result():
+    """plan cache hit, then graph replay (same buffers): bit-identical outputs; a length moved inside a page: structural hit"""
+    inp = W.make_inputs("fp8_repeat", 14, [700, 2500, 68, 135, 70], 0, 0)
+    r = Fp8Run(inp)
+    out0, lse0, bufs = r.decode()
+    infos = []
+    for _ in range(4):
+        bufs[0].fill_(float("nan"))
+        out, lse, _ = r.decode(out_dec=bufs[0], lse_dec=bufs[1])
+        infos.append(r.ctx.last_plan_info())
+        np.testing.assert_array_equal(out, out0)
+        np.testing.assert_array_equal(lse, lse0)
+    assert infos[-1]["plan_cache"] == 2 and infos[-1]["graph"] == 1, infos[-1]   # exact plan hit, replayed as a graph
+    ref_out, ref_lse = r.reference()
+    _assert_close(out0, lse0, ref_out, ref_lse, "repeat")
+    # the bf16 step of the same context still works beside it (its own plan entry)
+    e = r.torch.empty((0, 16, 576), dtype=r.torch.bfloat16, device="cuda")
+    od, _, ld, _ = r.ctx.mixed_step(r.q_dec, r.dec_pt, inp.dec_ctx_lens, e, r.torch.zeros(1, dtype=r.torch.int32, device="cuda"), 0, 0)
+    r.torch.cuda.synchronize()
+    ref16 = O.mixed_step(inp.pool, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, 0, 0, np.zeros((0, 16, 576), np.uint16), np.zeros(1, np.int32), inp.softmax_scale)
+    ma, rl = errors(W.bf16_bits_to_f32(r.K.bf16_bits(od)), ref16[0])
+    assert ma <= MAX_ABS_TOL and rl <= REL_L2_TOL
+    out, lse, _ = r.decode()
+    np.testing.assert_array_equal(out, out0)
+
+
+def test_config1_every_request():
+    inp = W.make_config(1)
+    inp = W.make_inputs("fp8_cfg1", 1, inp.dec_ctx_lens.tolist(), 0, 0)
+    r = Fp8Run(inp)
+    r.check_pool()
+    out, lse, _ = r.decode()
+    ref_out, ref_lse = r.reference()
+    _assert_close(out, lse, ref_out, ref_lse, "configs[1] decodes")
+
+
+def test_config3_sampled_requests():
+    """BASELINE.json configs[3] at C = 0 (256 x 2048 tokens), the launch configuration bench.py times: 12 sampled requests"""
+    inp = W.make_config(3, chunk_len=0)
+    idx = sorted(set([0, 255] + np.random.default_rng(7).choice(256, 10, replace=False).tolist()))
+    r = Fp8Run(inp, oracle_requests=idx)
+    r.check_pool()
+    out, lse, _ = r.decode()
+    ref_out, ref_lse = r.reference()
+    _assert_close(out[idx], lse[idx], ref_out, ref_lse, "configs[3] C=0 sampled")
+    assert np.isfinite(out).all()
+    info = r.ctx.last_plan_info()
+    assert info["kernels"] >= 3   # query preparation + attention + combine
+
+
+def test_errors():
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    inp = W.make_inputs("fp8_err", 15, [100, 100], 0, 0)
+    pool16 = K.bf16_tensor(inp.pool)
+    ws = torch.empty(K.workspace_bytes(2, 1), dtype=torch.uint8, device="cuda")
+    ctx = K.Kairos(pool16, ws, inp.softmax_scale)
+    q = K.bf16_tensor(inp.q_dec)
+    pt = torch.from_numpy(inp.dec_page_tables).cuda()
+    with pytest.raises(K.KairosError) as e:
+        ctx.fp8_decode(q, pt, inp.dec_ctx_lens)
+    assert e.value.code == -1 and "attach" in str(e.value)
+    pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device="cuda")
+    ctx.fp8_attach(pool8, 1)
+    with pytest.raises(K.KairosError) as e:
+        ctx.fp8_decode(q, pt, inp.dec_ctx_lens)   # 2 decodes, scratch sized for 1
+    assert e.value.code == -3
+    with pytest.raises(K.KairosError) as e:
+        ctx.fp8_append(q[0, 0, :512].reshape(1, 512).contiguous(), q[0, 0, 512:].reshape(1, 64).contiguous(), pt[0], 64 * pt.shape[1])
+    assert e.value.code == -1
