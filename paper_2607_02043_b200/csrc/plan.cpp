@@ -152,28 +152,26 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
         tile_pages += ceil_div(int64_t(prefix_len) + q_last + 1, kPage);
     }
     const int64_t total_cost = dec_pages * kChunkCostDen + tile_pages * kChunkCostNum;
-    // an item should not exceed about half of one CTA's fair share
-    int64_t max_item_cost = total_cost / (2 * int64_t(target_ctas));
+    // An item should not exceed about half of one CTA's fair share -- 0.6 of it in a queue of decode splits alone, where
+    // every split that is avoided saves a partial (32 KB written, read again by the combine): measured on configs[3] C = 0,
+    // 256 x 32 pages on 148 CTAs, whole requests beside 24-page bodies run 113.9 -> 109.4 us against two halves each.
+    const bool dec_queue_only = chunk_len == 0 && plan->n_pairs == 0;
+    int64_t max_item_cost = dec_queue_only ? total_cost * 3 / (5 * int64_t(target_ctas)) : total_cost / (2 * int64_t(target_ctas));
     max_item_cost = std::max<int64_t>(max_item_cost, int64_t(kMinSplitPages) * kChunkCostDen);
 
     // global caps that keep the workspace bound of kairos_workspace_bytes valid
-    // extra decode partial slots beyond one per request; a queue without chunk tiles may also spend the chunk's share
-    int32_t dec_split_budget = ((chunk_len == 0 && plan->n_pairs == 0) ? 8 : 4) * target_ctas;
+    int32_t dec_split_budget = 4 * target_ctas;   // extra decode partial slots beyond one per request
     int32_t chunk_slot_budget = 8 * target_ctas;  // chunk partial token-slots
 
     std::vector<WorkItem> dec_items, chunk_items;
 
     // ---- decode splits.  Two item sizes: "big" pieces (about half of one CTA's fair share) carry most of the
-    // pages with few partials; a tail budget of small (kMinSplitPages or half of it) pieces, peeled off the longest requests, goes
+    // pages with few partials; a tail budget of kMinSplitPages-sized pieces, peeled off the longest requests, goes
     // to the END of the queue so that the dynamic queue's finishing imbalance is a few pages, not one big piece.
     {
         const int64_t fair_pages = std::max<int64_t>(1, total_cost / (int64_t(kChunkCostDen) * target_ctas));
-        const int32_t big = int32_t(std::max<int64_t>(kMinSplitPages, std::min<int64_t>(max_item_cost / kChunkCostDen, (fair_pages + 1) / 2)));
+        const int32_t big = int32_t(std::max<int64_t>(kMinSplitPages, std::min<int64_t>(max_item_cost / kChunkCostDen, dec_queue_only ? (fair_pages * 3 + 4) / 5 : (fair_pages + 1) / 2)));
         int64_t tail_budget = fair_pages >= 4 * kMinSplitPages ? int64_t(target_ctas) * 2 * kMinSplitPages : 0;  // pages
-        // a queue of decode splits alone ends when its last piece does: halve the tail pieces (measured: configs[3] C = 0
-        // 113.2 -> 110.8 us; with a chunk beside the decodes the extra items cost more than the shorter tail gives)
-        const int32_t tail = (chunk_len == 0 && plan->n_pairs == 0) ? kMinSplitPages / 2 : kMinSplitPages;
-        const int32_t max_small = 2 * kMinSplitPages / tail;
         std::vector<int32_t> order(n_dec);
         for (int32_t i = 0; i < n_dec; ++i) order[i] = i;
         std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return dec_ctx_lens[a] > dec_ctx_lens[b]; });
@@ -184,10 +182,10 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
             // small tail pieces of this request (peeled from its end)
             int32_t n_small = 0;
             if (tail_budget > 0 && pages >= 3 * kMinSplitPages) {
-                n_small = int32_t(std::min<int64_t>({int64_t(max_small), tail_budget / tail, int64_t((pages - 2 * kMinSplitPages) / tail)}));
+                n_small = int32_t(std::min<int64_t>({int64_t(2), tail_budget / kMinSplitPages, int64_t(pages / kMinSplitPages - 2)}));
                 n_small = std::max(n_small, 0);
             }
-            const int32_t body = pages - n_small * tail;
+            const int32_t body = pages - n_small * kMinSplitPages;
             int32_t n_big = ceil_div(body, big);
             n_big = std::min(n_big, std::max(1, body / kMinSplitPages));
             int32_t n_splits = n_big + n_small;
@@ -197,7 +195,7 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
                 n_big = std::max(1, std::min(n_big, std::max(1, pages / kMinSplitPages)));
                 n_splits = n_big;
             }
-            const int32_t body2 = pages - n_small * tail;
+            const int32_t body2 = pages - n_small * kMinSplitPages;
             cuts.clear();
             cuts.push_back(0);
             const int32_t per = ceil_div(body2, n_big);
@@ -205,10 +203,10 @@ void build_plan(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len, i
                 const int32_t e = std::min(body2, s * per);
                 if (e > cuts.back()) cuts.push_back(e);
             }
-            for (int32_t s = 1; s <= n_small; ++s) cuts.push_back(body2 + s * tail);
+            for (int32_t s = 1; s <= n_small; ++s) cuts.push_back(body2 + s * kMinSplitPages);
             n_splits = int32_t(cuts.size()) - 1;
             if (n_splits > 1) dec_split_budget -= (n_splits - 1);
-            tail_budget -= int64_t(n_small) * tail;
+            tail_budget -= int64_t(n_small) * kMinSplitPages;
             int32_t first_slot = -1;
             if (n_splits > 1) {
                 first_slot = plan->n_partial_slots;
