@@ -130,13 +130,17 @@ __global__ void __launch_bounds__(512) fp8_quant_q_kernel(const uint4* __restric
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// decode attention over fp8 pages.  Warp roles as in attn_umma.cu: warp 0 producer, warp 1 S issuer + TMEM owner,
-// warps 2-9 softmax / epilogue, warp 10 PV issuer.
+// decode attention over fp8 pages.  Warp roles: warp 0 producer, warp 1 S issuer A (latent boxes 0-1) + TMEM owner, warps 2-9
+// softmax / epilogue, warp 10 PV issuer, warp 11 S issuer B (latent boxes 2-3 + RoPE).  Issuing a tcgen05.mma costs its warp
+// ~40 cycles and an mbarrier wait ~100 whether or not it blocks: one warp issuing the page's 20 S MMAs behind five waits was
+// the longest stage of the pipeline (2,250 cycles per page, measured), so the S product is cut in two halves that accumulate
+// in separate TMEM columns (summed by the softmax warps, in a fixed order) and a page has two landing barriers, not five.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kSoftmaxWarps = 8;
 constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
-constexpr int kThreads = 64 + kSoftmaxThreads + 32;
+constexpr int kThreads = 64 + kSoftmaxThreads + 64;
 constexpr int kPvWarp = 2 + kSoftmaxWarps;
+constexpr int kSbWarp = kPvWarp + 1;
 constexpr int kSlotBytes = 8192;      // one box: [64 tokens][128 B] = 128 latent codes, or the 64 bf16 RoPE values, SWIZZLE_128B
 constexpr int kStages = 4;            // pages in flight: 4 x 5 slots (4 latent boxes + RoPE) = 160 KB
 constexpr int kQBufBytes = kQ8Bytes + 16 * kRope * 2;  // 18,432: q8 (4 boxes of [32 rows][128 B]) | q_rope [16 rows][128 B]
@@ -150,9 +154,10 @@ constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;
 static_assert(kSmemBytes <= 232448, "exceeds the per-CTA shared memory limit");
 static_assert(kOffKV % 1024 == 0 && kOffP % 1024 == 0, "operand tiles must stay 1024-B aligned");
 
-constexpr uint32_t kTmemCols = 256;
-constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 64: [0,32) latent hi|lo, [32,48) RoPE
-constexpr uint32_t kColO = 128;  // O^T block b at 128 + 32 b: [0,16) from P hi, [16,32) from P lo
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 96: [0,32) boxes 0-1 hi|lo, [32,64) boxes 2-3 hi|lo, [64,80) RoPE
+constexpr uint32_t kSBuf = 96;
+constexpr uint32_t kColO = 192;  // O^T block b at 192 + 32 b: [0,16) from P hi, [16,32) from P lo
 // The reference m sits kHeadroom binades below the largest y seen when it was last refreshed, and is refreshed when some
 // y exceeds it by more than kRefresh: P8 = 2^(y - m) <= 2^8 = 256 < 448, and a weight 2^-10 below the largest still is a
 // normal e4m3 number (2^-6).
@@ -162,7 +167,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;
 
 struct Small8 {
-    uint64_t q_full[2], q_empty[2], kv_full[kStages][5], kv_empty[kStages][5], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kStages][2], kv_empty[kStages], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -267,28 +272,32 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const int b = g & 1;
         const int st = g & (kStages - 1);
-        mbar_wait(&sm->s_full[b], (g >> 1) & 1);
-        tc_fence_after();
-        float xh[NC], xl[NC], xr[NC];
-        tmem_ld8(tmem_addr(tmem, w4 * 32, kColS + b * 64 + cbase), *reinterpret_cast<uint32_t(*)[8]>(xh));
-        tmem_ld8(tmem_addr(tmem, w4 * 32, kColS + b * 64 + 16 + cbase), *reinterpret_cast<uint32_t(*)[8]>(xl));
-        tmem_ld8(tmem_addr(tmem, w4 * 32, kColS + b * 64 + 32 + cbase), *reinterpret_cast<uint32_t(*)[8]>(xr));
-        tmem_wait_ld();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&sm->s_empty[b]);
-        // the scales came with the page's first box; its barrier completed before the S MMAs were issued
+        // the token scales came with the page's first boxes, long before its S product completes: fetch them first
         mbar_wait(&sm->kv_full[st][0], (g / kStages) & 1);
         const float sc = lane_ok ? sm->scales[st][tok_in_page] : 1.f;
-
         const int page = w.page_begin + pg;
         const int key_pos = page * kPage + tok_in_page;
         const bool ok = lane_ok && key_pos < w.n_keys;
         const float lsc = lg2(sc), rs = ok ? __frcp_rn(sc) : 0.f;
+
+        mbar_wait(&sm->s_full[b], (g >> 1) & 1);
+        tc_fence_after();
+        float xa[2][NC], xb[2][NC], xr[NC];
+        const uint32_t sbase = tmem_addr(tmem, w4 * 32, kColS + b * kSBuf + cbase);
+        tmem_ld8(sbase, *reinterpret_cast<uint32_t(*)[8]>(xa[0]));
+        tmem_ld8(sbase + 16, *reinterpret_cast<uint32_t(*)[8]>(xa[1]));
+        tmem_ld8(sbase + 32, *reinterpret_cast<uint32_t(*)[8]>(xb[0]));
+        tmem_ld8(sbase + 48, *reinterpret_cast<uint32_t(*)[8]>(xb[1]));
+        tmem_ld8(sbase + 64, *reinterpret_cast<uint32_t(*)[8]>(xr));
+        tmem_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm->s_empty[b]);
         float y[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
-            const float v = fmaf((xh[c] + xl[c]) * sc, gi[c], xr[c] * p.scale_log2) + lsc;
+            const float s8 = (xa[0][c] + xa[1][c]) + (xb[0][c] + xb[1][c]);  // fixed order: the result never depends on timing
+            const float v = fmaf(s8 * sc, gi[c], xr[c] * p.scale_log2) + lsc;
             y[c] = ok ? v : -INFINITY;
         }
         float dmax = -INFINITY;
@@ -422,7 +431,9 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     if (lane == 0) mbar_arrive(&sm->o_empty);
 }
 
-// S MMAs of one decode split (warp 1).  Fixed accumulation order: latent boxes 0..3 (4 k-steps each), then the RoPE box.
+// S MMAs of one decode split, in two halves issued by two warps: half 0 = latent boxes 0-1 into columns [0,32) of the S buffer,
+// half 1 = latent boxes 2-3 into [32,64) and the RoPE box into [64,80).  Each half accumulates in a fixed order.
+template <int HALF>
 __device__ __forceinline__ void s_item8(Small8* sm, uint32_t tmem, uint32_t q_base, uint32_t kv_base, int npages, uint32_t g0, uint32_t qbuf,
                                         uint32_t qfull_parity) {
     constexpr uint32_t idesc_s8 = make_idesc_e4m3(64, 32, 0, 0);  // S8^T = K8 [Qhi;Qlo]^T: A K-major, B K-major
@@ -433,28 +444,26 @@ __device__ __forceinline__ void s_item8(Small8* sm, uint32_t tmem, uint32_t q_ba
         const uint32_t gg = g0 + s;
         const uint32_t sb = gg & 1, st = gg & (kStages - 1), par = (gg / kStages) & 1;
         mbar_wait(&sm->s_empty[sb], ((gg >> 1) & 1) ^ 1);
+        mbar_wait(&sm->kv_full[st][HALF], par);
+        tc_fence_after();
 #pragma unroll
-        for (uint32_t b = 0; b < 4; ++b) {
-            mbar_wait(&sm->kv_full[st][b], par);
-            tc_fence_after();
+        for (uint32_t bb = 0; bb < 2; ++bb) {
+            const uint32_t b = 2 * HALF + bb;
             const uint32_t ka_lo = smem_desc_lo(kv_base + (st * 5 + b) * kSlotBytes, 16);
             const uint32_t qb_lo = smem_desc_lo(q_base + b * 4096, 16);
 #pragma unroll
             for (uint32_t j = 0; j < 4; ++j)
-                umma_f8_ss_lohi(tmem + kColS + sb * 64, ka_lo + ((j * 32) >> 4), desc_hi, qb_lo + ((j * 32) >> 4), desc_hi, idesc_s8,
-                                !(b == 0 && j == 0));
+                umma_f8_ss_lohi(tmem + kColS + sb * kSBuf + 32 * HALF, ka_lo + ((j * 32) >> 4), desc_hi, qb_lo + ((j * 32) >> 4), desc_hi,
+                                idesc_s8, !(bb == 0 && j == 0));
         }
-        mbar_wait(&sm->kv_full[st][4], par);
-        tc_fence_after();
-        {
+        if (HALF == 1) {
             const uint32_t ka_lo = smem_desc_lo(kv_base + (st * 5 + 4) * kSlotBytes, 16);
             const uint32_t qb_lo = smem_desc_lo(q_base + kQ8Bytes, 16);
 #pragma unroll
             for (uint32_t j = 0; j < 4; ++j)
-                umma_bf16_ss_lohi(tmem + kColS + sb * 64 + 32, ka_lo + ((j * 32) >> 4), desc_hi, qb_lo + ((j * 32) >> 4), desc_hi, idesc_sr, j > 0);
+                umma_bf16_ss_lohi(tmem + kColS + sb * kSBuf + 64, ka_lo + ((j * 32) >> 4), desc_hi, qb_lo + ((j * 32) >> 4), desc_hi, idesc_sr, j > 0);
         }
         umma_commit_elect(&sm->s_full[sb]);
-        umma_commit_elect(&sm->kv_empty[st][4]);  // the RoPE box is only read by these MMAs
         if (s == npages - 1) umma_commit_elect(&sm->q_empty[qbuf]);
     }
 }
@@ -477,8 +486,8 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
             for (uint32_t ks = 0; ks < 2; ++ks)  // 32 keys per instruction: 32 rows of 128 B further down the box
                 umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 32) >> 4), desc_hi, idesc_o8,
                                 (pv > 0 || ks > 0));
-            umma_commit_elect(&sm->kv_empty[st][b4]);
         }
+        umma_commit_elect(&sm->kv_empty[st]);  // the whole stage (the S MMAs of this page completed before its softmax started)
         umma_commit_elect(&sm->pv_done[pst]);
         if (pv == npages - 1) umma_commit_elect(&sm->o_full);
     }
@@ -495,19 +504,19 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
             mbar_init(&sm->q_full[i], 1);
-            mbar_init(&sm->q_empty[i], 1);
-            mbar_init(&sm->s_full[i], 1);
+            mbar_init(&sm->q_empty[i], 2);
+            mbar_init(&sm->s_full[i], 2);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
-            mbar_init(&sm->item_empty[i], 2 + kSoftmaxWarps);
+            mbar_init(&sm->item_empty[i], 3 + kSoftmaxWarps);
             mbar_init(&sm->p_full[i], kSoftmaxWarps);
             mbar_init(&sm->pv_done[i], 1);
         }
-        for (int i = 0; i < kStages; ++i)
-            for (int bx = 0; bx < 5; ++bx) {
-                mbar_init(&sm->kv_full[i][bx], 1);
-                mbar_init(&sm->kv_empty[i][bx], 1);
-            }
+        for (int i = 0; i < kStages; ++i) {
+            mbar_init(&sm->kv_full[i][0], 1);
+            mbar_init(&sm->kv_full[i][1], 1);
+            mbar_init(&sm->kv_empty[i], 1);
+        }
         mbar_init(&sm->o_full, 1);
         mbar_init(&sm->o_empty, kSoftmaxWarps);
         fence_barrier_init();
@@ -562,23 +571,20 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
                         const uint32_t st = g & (kStages - 1), par = ((g / kStages) & 1) ^ 1;
+                        mbar_wait(&sm->kv_empty[st], par);
+                        mbar_arrive_expect_tx(&sm->kv_full[st][0], 2 * kSlotBytes + kPage * 4);
+                        mbar_arrive_expect_tx(&sm->kv_full[st][1], 3 * kSlotBytes);
 #pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            mbar_wait(&sm->kv_empty[st][b], par);
-                            mbar_arrive_expect_tx(&sm->kv_full[st][b], kSlotBytes + (b == 0 ? kPage * 4 : 0));
-                            tma_load_3d(kv_u32 + (st * 5 + b) * kSlotBytes, &lat_map, &sm->kv_full[st][b], b * 128, 0, pid, kEvictFirst);
-                            if (b == 0)
-                                bulk_load(smem_u32(sm->scales[st]), p.pool8 + size_t(pid) * kPage8Bytes + kOffScale8, kPage * 4,
-                                          &sm->kv_full[st][0], kEvictFirst);
-                        }
-                        mbar_wait(&sm->kv_empty[st][4], par);
-                        mbar_arrive_expect_tx(&sm->kv_full[st][4], kSlotBytes);
-                        tma_load_3d(kv_u32 + (st * 5 + 4) * kSlotBytes, &rope_map, &sm->kv_full[st][4], 0, 0, pid, kEvictFirst);
+                        for (int b = 0; b < 4; ++b)
+                            tma_load_3d(kv_u32 + (st * 5 + b) * kSlotBytes, &lat_map, &sm->kv_full[st][b >> 1], b * 128, 0, pid, kEvictFirst);
+                        tma_load_3d(kv_u32 + (st * 5 + 4) * kSlotBytes, &rope_map, &sm->kv_full[st][1], 0, 0, pid, kEvictFirst);
+                        bulk_load(smem_u32(sm->scales[st]), p.pool8 + size_t(pid) * kPage8Bytes + kOffScale8, kPage * 4, &sm->kv_full[st][0],
+                                  kEvictFirst);
                     }
                 }
             }
         }
-    } else if (warp == 1 || warp == kPvWarp) {
+    } else if (warp == 1 || warp == kPvWarp || warp == kSbWarp) {
         // ================= MMA issuers =================
         const uint32_t q_base = smem_u32(base + kOffQ), kv_base = smem_u32(base + kOffKV), p_base = smem_u32(base + kOffP);
         uint32_t g = 0;
@@ -591,7 +597,8 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             if (idx < 0) break;
             const WorkItem w = load_item8(p.items + idx);
             const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
-            if (warp == 1) s_item8(sm, tmem, q_base + (it & 1u) * kQBufBytes, kv_base, npages, g, it & 1u, (it >> 1) & 1u);
+            if (warp == 1) s_item8<0>(sm, tmem, q_base + (it & 1u) * kQBufBytes, kv_base, npages, g, it & 1u, (it >> 1) & 1u);
+            else if (warp == kSbWarp) s_item8<1>(sm, tmem, q_base + (it & 1u) * kQBufBytes, kv_base, npages, g, it & 1u, (it >> 1) & 1u);
             else pv_item8(sm, tmem, kv_base, p_base, npages, g, it);
             g += npages;
         }
