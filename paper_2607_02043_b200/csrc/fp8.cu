@@ -278,7 +278,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         const int page = w.page_begin + pg;
         const int key_pos = page * kPage + tok_in_page;
         const bool ok = lane_ok && key_pos < w.n_keys;
-        const float lsc = lg2(sc), rs = ok ? __frcp_rn(sc) : 0.f;
+        const float lsc = lg2(sc), rs = ok ? __fdividef(1.f, sc) : 0.f;
 
         mbar_wait(&sm->s_full[b], (g >> 1) & 1);
         tc_fence_after();
@@ -533,8 +533,9 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm->tmem_base;
-    // launched behind the query-preparation grid with programmatic stream serialisation: everything above overlapped it
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // Launched behind the query-preparation grid with programmatic stream serialisation: everything above overlapped it, and
+    // so do the first pages' loads (the cache does not depend on that grid).  Only what it wrote is waited for: the producer
+    // waits before the first q8 load, the softmax warps before they read the gains.
 
     if (warp == 0) {
         // ================= producer =================
@@ -555,21 +556,26 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             if (idx < 0) break;
             const WorkItem w = load_item8(p.items + idx);
             const int qb = int(it & 1);
-            if (lane == 0) {
+            const int npages = w.page_end - w.page_begin;
+            auto load_q = [&]() {  // lane 0
+                if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
                 mbar_wait(&sm->q_empty[qb], ((it >> 1) & 1) ^ 1);
                 mbar_arrive_expect_tx(&sm->q_full[qb], uint32_t(kQBufBytes));
                 uint8_t* qdst = base + kOffQ + qb * kQBufBytes;
                 for (int j = 0; j < 4; ++j) tma_load_2d(qdst + j * 4096, &q8_map, &sm->q_full[qb], 0, (w.q_index * 4 + j) * 32, kEvictFirst);
                 tma_load_2d(qdst + kQ8Bytes, &qr_map, &sm->q_full[qb], kLatent, w.q_index * kHeads, kEvictFirst);
-            }
+            };
+            // the first item's q is requested behind its first pages (they fill the empty ring without waiting)
+            const int q_at = it == 0 ? min(npages, kStages) : 0;
+            if (lane == 0 && q_at == 0) load_q();
             const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
-            const int npages = w.page_end - w.page_begin;
             for (int i = 0; i < npages; i += 32) {
                 const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
                 const int cnt = min(32, npages - i);
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
+                        if (q_at > 0 && i + j == q_at) load_q();
                         const uint32_t st = g & (kStages - 1), par = ((g / kStages) & 1) ^ 1;
                         mbar_wait(&sm->kv_empty[st], par);
                         mbar_arrive_expect_tx(&sm->kv_full[st][0], 2 * kSlotBytes + kPage * 4);
@@ -583,6 +589,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                     }
                 }
             }
+            if (lane == 0 && q_at > 0 && npages <= q_at) load_q();
         }
     } else if (warp == 1 || warp == kPvWarp || warp == kSbWarp) {
         // ================= MMA issuers =================
@@ -606,6 +613,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
         // ================= softmax / correction / epilogue warps =================
         const int sw = warp - 2;
         uint32_t g = 0;
+        asm volatile("griddepcontrol.wait;" ::: "memory");  // the gains (and nothing else these warps read) come from the query preparation
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
             const int idx = sm->item_ring[it & 1];
