@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(512) fp8_quant_q_kernel(const uint4* __restric
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kSoftmaxWarps = 8;
 constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
-constexpr int kThreads = 64 + kSoftmaxThreads + 64 + kSoftmaxThreads;  // warps 12-19: the second softmax group
+constexpr int kThreads = 64 + kSoftmaxThreads + 64;
 constexpr int kPvWarp = 2 + kSoftmaxWarps;
 constexpr int kSbWarp = kPvWarp + 1;
 constexpr int kSlotBytes = 8192;      // one box: [64 tokens][128 B] = 128 latent codes, or the 64 bf16 RoPE values, SWIZZLE_128B
@@ -157,8 +157,7 @@ static_assert(kOffKV % 1024 == 0 && kOffP % 1024 == 0, "operand tiles must stay 
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 96: [0,32) boxes 0-1 hi|lo, [32,64) boxes 2-3 hi|lo, [64,80) RoPE
 constexpr uint32_t kSBuf = 96;
-constexpr uint32_t kColO = 192;  // O^T of stream r, block b at 192 + 128 r + 32 b: [0,16) from P hi, [16,32) from P lo
-constexpr uint32_t kOBuf = 128;
+constexpr uint32_t kColO = 192;  // O^T block b at 192 + 32 b: [0,16) from P hi, [16,32) from P lo
 // The reference m sits kHeadroom binades below the largest y seen when it was last refreshed, and is refreshed when some
 // y exceeds it by more than kRefresh: P8 = 2^(y - m) <= 2^8 = 256 < 448, and a weight 2^-10 below the largest still is a
 // normal e4m3 number (2^-6).
@@ -173,13 +172,11 @@ struct Small8 {
     int32_t item_ring[2];
     uint32_t tmem_base;
     uint32_t pad;
-    alignas(16) WorkItem item_w[2];            // the popped items themselves (the consumers never go to global memory for them)
-    alignas(16) float ginv[2][16];            // 1 / g of the item's query rows (bulk-copied with its q)
     alignas(16) float scales[kStages][kPage];  // the page's token scales (bulk-copied with its first box)
-    float m_ref[2][2][16];  // [item parity][stream][head]: running reference (log2 domain); -1e30 while nothing visible yet
-    float lsum[2][2][16];   // [item parity][stream][head]: row sums at the end of the item
-    float alpha[2][16];     // [stream]: O / l rescale factor of the current refresh
-    float red[2][4][16];    // [stream][quadrant]: per-warp column maxima / sums
+    float m_ref[16];
+    float alpha[16];
+    float red[4][16];
+    float linv[16];
 };
 static_assert(sizeof(Small8) <= kSmallBytes, "Small8 does not fit");
 
@@ -252,41 +249,28 @@ __device__ __forceinline__ void st_f32_evict_last(float* p, float v) {
     asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(kEvictLast) : "memory");
 }
 
-// softmax / correction / epilogue of one decode split.  Two groups of 8 warps run two INDEPENDENT online-softmax streams:
-// group r takes the pages whose CTA-wide number g has parity r (S buffer r, P buffer r, O^T accumulator r), with its own
-// reference m_r and row sums l_r; the epilogue merges the two streams exactly as the combine kernel merges KV splits
-// (weights 2^(m_r - max m)).  One page's chain (wait, TMEM load, reference check, exp, split, store, fence, arrive) is
-// ~2,000 cycles of mostly fixed latencies; two of them in flight bring the pipeline under the HBM time per page.
-// In a group, warp sw works on TMEM lane quadrant `w4` (16 of its lanes hold the M=64 accumulator rows = keys) and heads
-// 8 (sw >> 2) .. + 8.
+// softmax / correction / epilogue of one decode split.  Warp sw: TMEM lane quadrant (sw + 2) & 3 (16 of its lanes hold the
+// M=64 accumulator rows = keys), heads 8 (sw >> 2) .. + 8.
 __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* pbuf, const WorkItem& w, const K8Params& p, uint32_t tmem,
-                                              int grp, int sw, int w4, int lane, uint32_t g0, uint32_t it) {
+                                              int sw, int lane, uint32_t& g, uint32_t it) {
     constexpr int NC = 8;
+    const int w4 = (sw + 2) & 3;
     const int cbase = (sw >> 2) * NC;
     const int tid_s = sw * 32 + lane;
     const bool lane_ok = lane < 16;
     const int tok_in_page = w4 * 16 + lane;
-    const int ip = it & 1;  // the per-item statistics are double-buffered: the other group may still be merging the previous item
-    float* m_ref = sm->m_ref[ip][grp];
-    float* alpha = sm->alpha[grp];
-    const int bar_a = 1 + 2 * grp, bar_b = 2 + 2 * grp;
     float l[NC], gi[NC];
-    mbar_wait(&sm->q_full[ip], (it >> 1) & 1);  // the gains came with the item's q
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         l[c] = 0.f;
-        gi[c] = sm->ginv[ip][cbase + c] * p.scale_log2;  // 1/g_h folded with sigma * log2(e)
+        gi[c] = __ldg(p.ginv + size_t(w.q_index) * kHeads + cbase + c) * p.scale_log2;  // 1/g_h folded with sigma * log2(e)
     }
-    if (tid_s < 16) m_ref[tid_s] = kMinusHuge;
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&sm->q_empty[ip]);  // with the S warps' commits: the q buffer (and its gains) may be refilled
-    named_sync(bar_a);
+    if (tid_s < 16) sm->m_ref[tid_s] = kMinusHuge;
+    named_sync(1);
 
     const int npages = w.page_end - w.page_begin;
-    const int b = grp;  // S / P / O buffer of this group
-    int mine = 0;       // pages of this item this group has taken
-    for (int pg = (int(g0) & 1) ^ grp; pg < npages; pg += 2, ++mine) {
-        const uint32_t g = g0 + pg;
+    for (int pg = 0; pg < npages; ++pg, ++g) {
+        const int b = g & 1;
         const int st = g & (kStages - 1);
         // the token scales came with the page's first boxes, long before its S product completes: fetch them first
         mbar_wait(&sm->kv_full[st][0], (g / kStages) & 1);
@@ -298,69 +282,67 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
 
         mbar_wait(&sm->s_full[b], (g >> 1) & 1);
         tc_fence_after();
+        float xa[2][NC], xb[2][NC], xr[NC];
+        const uint32_t sbase = tmem_addr(tmem, w4 * 32, kColS + b * kSBuf + cbase);
+        tmem_ld8(sbase, *reinterpret_cast<uint32_t(*)[8]>(xa[0]));
+        tmem_ld8(sbase + 16, *reinterpret_cast<uint32_t(*)[8]>(xa[1]));
+        tmem_ld8(sbase + 32, *reinterpret_cast<uint32_t(*)[8]>(xb[0]));
+        tmem_ld8(sbase + 48, *reinterpret_cast<uint32_t(*)[8]>(xb[1]));
+        tmem_ld8(sbase + 64, *reinterpret_cast<uint32_t(*)[8]>(xr));
+        tmem_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm->s_empty[b]);
         float y[NC];
-        {
-            float xa[2][NC], xb[2][NC], xr[NC];
-            const uint32_t sbase = tmem_addr(tmem, w4 * 32, kColS + b * kSBuf + cbase);
-            tmem_ld8(sbase, *reinterpret_cast<uint32_t(*)[8]>(xa[0]));
-            tmem_ld8(sbase + 16, *reinterpret_cast<uint32_t(*)[8]>(xa[1]));
-            tmem_ld8(sbase + 32, *reinterpret_cast<uint32_t(*)[8]>(xb[0]));
-            tmem_ld8(sbase + 48, *reinterpret_cast<uint32_t(*)[8]>(xb[1]));
-            tmem_ld8(sbase + 64, *reinterpret_cast<uint32_t(*)[8]>(xr));
-            tmem_wait_ld();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sm->s_empty[b]);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                const float s8 = (xa[0][c] + xa[1][c]) + (xb[0][c] + xb[1][c]);  // fixed order: the result never depends on timing
-                const float v = fmaf(s8 * sc, gi[c], xr[c] * p.scale_log2) + lsc;
-                y[c] = ok ? v : -INFINITY;
-            }
+        for (int c = 0; c < NC; ++c) {
+            const float s8 = (xa[0][c] + xa[1][c]) + (xb[0][c] + xb[1][c]);  // fixed order: the result never depends on timing
+            const float v = fmaf(s8 * sc, gi[c], xr[c] * p.scale_log2) + lsc;
+            y[c] = ok ? v : -INFINITY;
         }
         float dmax = -INFINITY;
 #pragma unroll
-        for (int c = 0; c < NC; ++c) dmax = fmaxf(dmax, y[c] - m_ref[cbase + c]);
-        const bool need = named_or(bar_b, dmax > kRefresh);
+        for (int c = 0; c < NC; ++c) dmax = fmaxf(dmax, y[c] - sm->m_ref[cbase + c]);
+        const bool need = named_or(2, dmax > kRefresh);
         if (need) {
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const float wm = warp_max(y[c]);
-                if (lane == c) sm->red[grp][w4][cbase + c] = wm;
+                if (lane == c) sm->red[w4][cbase + c] = wm;
             }
-            named_sync(bar_a);
+            named_sync(1);
             if (tid_s < 16) {
-                const float tm = fmaxf(fmaxf(sm->red[grp][0][tid_s], sm->red[grp][1][tid_s]), fmaxf(sm->red[grp][2][tid_s], sm->red[grp][3][tid_s]));
-                const float mo = m_ref[tid_s];
+                const float tm = fmaxf(fmaxf(sm->red[0][tid_s], sm->red[1][tid_s]), fmaxf(sm->red[2][tid_s], sm->red[3][tid_s]));
+                const float mo = sm->m_ref[tid_s];
                 const float mn = fmaxf(mo, tm - kHeadroom);
-                m_ref[tid_s] = mn;
-                alpha[tid_s] = ex2(mo - mn);
+                sm->m_ref[tid_s] = mn;
+                sm->alpha[tid_s] = ex2(mo - mn);
             }
-            named_sync(bar_a);
-            if (mine > 0) {  // this group's O^T and l are relative to the old reference: rescale (rare)
-                mbar_wait(&sm->pv_done[b], ((g - 2) >> 1) & 1);  // the group's previous page has been accumulated
+            named_sync(1);
+            if (pg > 0) {  // O^T and l are relative to the old reference: rescale (rare)
+                mbar_wait(&sm->pv_done[(g - 1) & 1], ((g - 1) >> 1) & 1);
                 tc_fence_after();
 #pragma unroll
                 for (int b4 = 0; b4 < 4; ++b4)
 #pragma unroll
                     for (int half = 0; half < 2; ++half) {
                         uint32_t r[NC];
-                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b * kOBuf + b4 * 32 + half * 16 + cbase);
+                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + half * 16 + cbase);
                         tmem_ld8(ta, *reinterpret_cast<uint32_t(*)[8]>(r));
                         tmem_wait_ld();
 #pragma unroll
-                        for (int i = 0; i < NC; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * alpha[cbase + i]);
+                        for (int i = 0; i < NC; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * sm->alpha[cbase + i]);
                         tmem_st8(ta, *reinterpret_cast<const uint32_t(*)[8]>(r));
                     }
                 tmem_wait_st();
 #pragma unroll
-                for (int c = 0; c < NC; ++c) l[c] *= alpha[cbase + c];
+                for (int c = 0; c < NC; ++c) l[c] *= sm->alpha[cbase + c];
             }
         }
         uint32_t chi[NC / 2], clo[NC / 2];
 #pragma unroll
         for (int c = 0; c < NC; c += 2) {
-            const float p0 = ex2(y[c] - m_ref[cbase + c]), p1 = ex2(y[c + 1] - m_ref[cbase + c + 1]);
+            const float p0 = ex2(y[c] - sm->m_ref[cbase + c]), p1 = ex2(y[c + 1] - sm->m_ref[cbase + c + 1]);
             l[c] = fmaf(p0, rs, l[c]);
             l[c + 1] = fmaf(p1, rs, l[c + 1]);
             chi[c / 2] = e4m3x2(p0, p1);
@@ -393,8 +375,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->p_full[b]);
     }
-
-    // ---- epilogue: all PV MMAs of the item are complete; merge the two streams
+    // ---- epilogue: all PV MMAs of the item are complete
     mbar_wait(&sm->o_full, it & 1);
     tc_fence_after();
 #pragma unroll
@@ -404,67 +385,45 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         v += __shfl_xor_sync(0xffffffffu, v, 4);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
         v += __shfl_xor_sync(0xffffffffu, v, 1);  // lanes 0..15 hold the data, lanes 16..31 zeros
-        if (lane == c) sm->red[grp][w4][cbase + c] = v;
+        if (lane == c) sm->red[w4][cbase + c] = v;
     }
-    named_sync(bar_a);
-    if (tid_s < 16) sm->lsum[ip][grp][tid_s] = sm->red[grp][0][tid_s] + sm->red[grp][1][tid_s] + sm->red[grp][2][tid_s] + sm->red[grp][3][tid_s];
-    asm volatile("bar.sync 5, %0;" ::"n"(2 * kSoftmaxThreads) : "memory");  // both groups' statistics are in shared memory
-    const bool have0 = npages >= 2 || (g0 & 1) == 0, have1 = npages >= 2 || (g0 & 1) == 1;  // which streams saw a page
-    // lane j works out the merge weights of head cbase + (j & 7) once (MUFU work: 16 warps doing all 8 heads each cost ~800 cycles)
-    // and the warp shares them by shuffle
-    float w0[NC], w1[NC], linv[NC];
-    {
-        const int h = cbase + (lane & 7);
-        const float m0 = sm->m_ref[ip][0][h], m1 = sm->m_ref[ip][1][h];
-        const float M = fmaxf(m0, m1);
-        const float mw0 = have0 ? ex2(m0 - M) : 0.f, mw1 = have1 ? ex2(m1 - M) : 0.f;
-        const float L = mw0 * sm->lsum[ip][0][h] + mw1 * sm->lsum[ip][1][h];
-        const float mli = __fdividef(1.f, L);
-        if (grp == 0 && w4 == 0 && lane < NC) {  // one thread per head writes the row statistics
-            if (w.partial_slot < 0) {
-                if (p.lse_dec) p.lse_dec[size_t(w.q_index) * kHeads + h] = (M + lg2(L)) * kLn2;
-            } else {
-                float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes + size_t(kHeads) * kLatent * 4);
-                ml[h] = M;
-                ml[kHeads + h] = L;
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            w0[c] = __shfl_sync(0xffffffffu, mw0, c);
-            w1[c] = __shfl_sync(0xffffffffu, mw1, c);
-            linv[c] = __shfl_sync(0xffffffffu, mli, c);
-        }
-    }
-    // O^T block b4 (group r takes blocks 2r, 2r + 1): lane = latent dim 128 b4 + 32 w4 + lane; per stream, columns [0,16) from P hi,
-    // [16,32) from P lo
+    named_sync(1);
     const bool is_final = w.partial_slot < 0;
-#pragma unroll
-    for (int bb = 0; bb < 2; ++bb) {
-        const int b4 = 2 * grp + bb;
-        float acc[NC];
-        uint32_t o0[2][NC], o1[2][NC];  // [hi | lo] of each stream; an accumulator no page went to holds garbage: never used
-#pragma unroll
-        for (int hl = 0; hl < 2; ++hl) {
-            tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + hl * 16 + cbase), o0[hl]);
-            tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + kOBuf + b4 * 32 + hl * 16 + cbase), o1[hl]);
+    if (tid_s < 16) {
+        const float L = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
+        sm->linv[tid_s] = __fdividef(1.f, L);
+        const float m = sm->m_ref[tid_s];
+        if (is_final) {
+            if (p.lse_dec) p.lse_dec[size_t(w.q_index) * kHeads + tid_s] = (m + lg2(L)) * kLn2;
+        } else {
+            float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes + size_t(kHeads) * kLatent * 4);
+            ml[tid_s] = m;
+            ml[kHeads + tid_s] = L;
         }
+    }
+    named_sync(2);
+    // O^T block b4: lane = latent dim 128 b4 + 32 w4 + lane; columns [0,16) from P hi, [16,32) from P lo
+    uint32_t rr[2][2 * NC];
+    auto load_block = [&](int b4, uint32_t* r) {
+        tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + cbase), *reinterpret_cast<uint32_t(*)[8]>(r));
+        tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + 16 + cbase), *reinterpret_cast<uint32_t(*)[8]>(r + NC));
+    };
+    load_block(0, rr[0]);
+#pragma unroll
+    for (int b4 = 0; b4 < 4; ++b4) {
         tmem_wait_ld();
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            const float a0 = have0 ? w0[c] * (__uint_as_float(o0[0][c]) + __uint_as_float(o0[1][c])) : 0.f;
-            const float a1 = have1 ? w1[c] * (__uint_as_float(o1[0][c]) + __uint_as_float(o1[1][c])) : 0.f;
-            acc[c] = a0 + a1;
-        }
+        if (b4 < 3) load_block(b4 + 1, rr[(b4 + 1) & 1]);
+        const uint32_t* r = rr[b4 & 1];
         const int d = b4 * 128 + w4 * 32 + lane;
         if (is_final) {
             __nv_bfloat16* o = p.out_dec + (size_t(w.q_index) * kHeads + cbase) * kLatent + d;
 #pragma unroll
-            for (int i = 0; i < NC; ++i) o[i * kLatent] = __float2bfloat16_rn(acc[i] * linv[i]);
+            for (int i = 0; i < NC; ++i)
+                o[i * kLatent] = __float2bfloat16_rn((__uint_as_float(r[i]) + __uint_as_float(r[NC + i])) * sm->linv[cbase + i]);
         } else {
             float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes) + cbase * kLatent + d;
 #pragma unroll
-            for (int i = 0; i < NC; ++i) st_f32_evict_last(o + i * kLatent, acc[i]);
+            for (int i = 0; i < NC; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[i]) + __uint_as_float(r[NC + i]));
         }
     }
     tc_fence_before();
@@ -525,8 +484,8 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
             const uint32_t va_lo = smem_desc_lo(kv_base + (st * 5 + b4) * kSlotBytes, 8192);
 #pragma unroll
             for (uint32_t ks = 0; ks < 2; ++ks)  // 32 keys per instruction: 32 rows of 128 B further down the box
-                umma_f8_ss_lohi(tmem + kColO + pst * kOBuf + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 32) >> 4), desc_hi,
-                                idesc_o8, (pv > 1 || ks > 0));  // pages 0 and 1 of the item open the two streams
+                umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 32) >> 4), desc_hi, idesc_o8,
+                                (pv > 0 || ks > 0));
         }
         umma_commit_elect(&sm->kv_empty[st]);  // the whole stage (the S MMAs of this page completed before its softmax started)
         umma_commit_elect(&sm->pv_done[pst]);
@@ -545,11 +504,11 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
             mbar_init(&sm->q_full[i], 1);
-            mbar_init(&sm->q_empty[i], 2 + 2 * kSoftmaxWarps);
+            mbar_init(&sm->q_empty[i], 2);
             mbar_init(&sm->s_full[i], 2);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
-            mbar_init(&sm->item_empty[i], 3 + 2 * kSoftmaxWarps);
+            mbar_init(&sm->item_empty[i], 3 + kSoftmaxWarps);
             mbar_init(&sm->p_full[i], kSoftmaxWarps);
             mbar_init(&sm->pv_done[i], 1);
         }
@@ -559,7 +518,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             mbar_init(&sm->kv_empty[i], 1);
         }
         mbar_init(&sm->o_full, 1);
-        mbar_init(&sm->o_empty, 2 * kSoftmaxWarps);
+        mbar_init(&sm->o_empty, kSoftmaxWarps);
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) {
@@ -576,67 +535,47 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     const uint32_t tmem = sm->tmem_base;
     // Launched behind the query-preparation grid with programmatic stream serialisation: everything above overlapped it, and
     // so do the first pages' loads (the cache does not depend on that grid).  Only what it wrote is waited for: the producer
-    // waits before the first q8 / gain load.
+    // waits before the first q8 load, the softmax warps before they read the gains.
 
     if (warp == 0) {
         // ================= producer =================
-        // Popping an item costs three dependent trips to global memory (queue counter, the item, its page ids: ~4,000 cycles
-        // under load, measured).  They are taken for item it + 1 while the pages of item it are being requested, so that the
-        // ring never drains at an item boundary.
         uint32_t g = 0;
         const uint32_t kv_u32 = smem_u32(base + kOffKV);
-        auto first_ids = [&](const WorkItem& w) {  // page ids of the item's first (up to) 32 pages, one per lane
-            const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
-            return lane < w.page_end - w.page_begin ? __ldg(pt + lane) : 0;
-        };
-        int idx = int(blockIdx.x);
-        if (!p.static_first) {
-            if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
-        }
-        if (idx >= p.n_items) idx = -1;
-        WorkItem w{};
-        int my = 0;
-        if (idx >= 0) {
-            w = load_item8(p.items + idx);
-            my = first_ids(w);
-        }
         for (uint32_t it = 0;; ++it) {
-            auto publish = [&]() {  // lane 0: hand the item to the consumer warps
+            int idx = int(blockIdx.x);
+            if (it > 0 || !p.static_first) {
+                if (lane == 0) idx = atomicAdd(&p.counters[0], 1) + (p.static_first ? int(gridDim.x) : 0);
+                idx = __shfl_sync(0xffffffffu, idx, 0);
+            }
+            if (idx >= p.n_items) idx = -1;
+            if (lane == 0) {
                 mbar_wait(&sm->item_empty[it & 1], ((it >> 1) & 1) ^ 1);
                 sm->item_ring[it & 1] = idx;
-                sm->item_w[it & 1] = w;
                 mbar_arrive(&sm->item_full[it & 1]);
-            };
-            if (idx < 0) {
-                if (lane == 0) publish();
-                break;
             }
+            if (idx < 0) break;
+            const WorkItem w = load_item8(p.items + idx);
             const int qb = int(it & 1);
             const int npages = w.page_end - w.page_begin;
             auto load_q = [&]() {  // lane 0
                 if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
                 mbar_wait(&sm->q_empty[qb], ((it >> 1) & 1) ^ 1);
-                mbar_arrive_expect_tx(&sm->q_full[qb], uint32_t(kQBufBytes + kHeads * 4));
-                bulk_load(smem_u32(sm->ginv[qb]), p.ginv + size_t(w.q_index) * kHeads, kHeads * 4, &sm->q_full[qb], kEvictFirst);
+                mbar_arrive_expect_tx(&sm->q_full[qb], uint32_t(kQBufBytes));
                 uint8_t* qdst = base + kOffQ + qb * kQBufBytes;
                 for (int j = 0; j < 4; ++j) tma_load_2d(qdst + j * 4096, &q8_map, &sm->q_full[qb], 0, (w.q_index * 4 + j) * 32, kEvictFirst);
                 tma_load_2d(qdst + kQ8Bytes, &qr_map, &sm->q_full[qb], kLatent, w.q_index * kHeads, kEvictFirst);
             };
-            // Order at an item boundary: the item's first page goes out first (its ids were fetched during the previous item), then
-            // the item is published and its q requested -- q is small and lands long before the page does.  The first item's q waits
-            // for the query-preparation grid, so it goes behind the pages that fill the empty ring.
-            const int q_after = it == 0 ? min(npages, kStages) - 1 : 0;
+            // the first item's q is requested behind its first pages (they fill the empty ring without waiting)
+            const int q_at = it == 0 ? min(npages, kStages) : 0;
+            if (lane == 0 && q_at == 0) load_q();
             const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
-            const int at_item = min(1, npages - 1), at_ids = min(3, npages - 1);  // where the next item / its page ids are fetched
-            int nraw = 0, nidx = -1, nmy = 0;
-            WorkItem nw{};
             for (int i = 0; i < npages; i += 32) {
-                const int ids = i == 0 ? my : ((i + lane < npages) ? __ldg(pt + i + lane) : 0);
+                const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
                 const int cnt = min(32, npages - i);
                 for (int j = 0; j < cnt; ++j, ++g) {
-                    const int pid = __shfl_sync(0xffffffffu, ids, j);
+                    const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
+                        if (q_at > 0 && i + j == q_at) load_q();
                         const uint32_t st = g & (kStages - 1), par = ((g / kStages) & 1) ^ 1;
                         mbar_wait(&sm->kv_empty[st], par);
                         mbar_arrive_expect_tx(&sm->kv_full[st][0], 2 * kSlotBytes + kPage * 4);
@@ -647,23 +586,10 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                         tma_load_3d(kv_u32 + (st * 5 + 4) * kSlotBytes, &rope_map, &sm->kv_full[st][1], 0, 0, pid, kEvictFirst);
                         bulk_load(smem_u32(sm->scales[st]), p.pool8 + size_t(pid) * kPage8Bytes + kOffScale8, kPage * 4, &sm->kv_full[st][0],
                                   kEvictFirst);
-                        if (i + j == 0) {
-                            publish();
-                            nraw = atomicAdd(&p.counters[0], 1);  // the next pop: in flight until `at_item`
-                        }
-                        if (i + j == q_after) load_q();
                     }
-                    if (i + j == at_item) {
-                        nidx = __shfl_sync(0xffffffffu, nraw, 0) + (p.static_first ? int(gridDim.x) : 0);
-                        if (nidx >= p.n_items) nidx = -1;
-                        if (nidx >= 0) nw = load_item8(p.items + nidx);
-                    }
-                    if (i + j == at_ids && nidx >= 0) nmy = first_ids(nw);
                 }
             }
-            idx = nidx;
-            w = nw;
-            my = nmy;
+            if (lane == 0 && q_at > 0 && npages <= q_at) load_q();
         }
     } else if (warp == 1 || warp == kPvWarp || warp == kSbWarp) {
         // ================= MMA issuers =================
@@ -672,14 +598,12 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
             const int idx = __shfl_sync(0xffffffffu, sm->item_ring[it & 1], 0);
-            if (idx < 0) {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
-                break;
-            }
-            const int npages = sm->item_w[it & 1].page_end - sm->item_w[it & 1].page_begin;
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
+            __syncwarp();
+            if (idx < 0) break;
+            const WorkItem w = load_item8(p.items + idx);
+            const int npages = __shfl_sync(0xffffffffu, w.page_end - w.page_begin, 0);
             if (warp == 1) s_item8<0>(sm, tmem, q_base + (it & 1u) * kQBufBytes, kv_base, npages, g, it & 1u, (it >> 1) & 1u);
             else if (warp == kSbWarp) s_item8<1>(sm, tmem, q_base + (it & 1u) * kQBufBytes, kv_base, npages, g, it & 1u, (it >> 1) & 1u);
             else pv_item8(sm, tmem, kv_base, p_base, npages, g, it);
@@ -687,18 +611,17 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
         }
     } else {
         // ================= softmax / correction / epilogue warps =================
-        const int grp = warp >= kSbWarp ? 1 : 0;
-        const int sw = grp ? warp - (kSbWarp + 1) : warp - 2;
+        const int sw = warp - 2;
         uint32_t g = 0;
+        asm volatile("griddepcontrol.wait;" ::: "memory");  // the gains (and nothing else these warps read) come from the query preparation
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
             const int idx = sm->item_ring[it & 1];
-            const WorkItem w = sm->item_w[it & 1];
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
             if (idx < 0) break;
-            softmax_item8(sm, base + kOffKV, base + kOffP, w, p, tmem, grp, sw, warp & 3, lane, g, it);
-            g += uint32_t(w.page_end - w.page_begin);
+            const WorkItem w = load_item8(p.items + idx);
+            softmax_item8(sm, base + kOffKV, base + kOffP, w, p, tmem, sw, lane, g, it);
         }
     }
 
