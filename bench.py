@@ -11,7 +11,7 @@ in `sweep` (step time, attention-kernel bracket, host enqueue time, fraction of 
 peak).  Inputs are seeded synthetic stand-ins for the paper's proprietary traces.  N>1: one replica per
 GPU (requests shard by sequence with no data-path collective: "replicas only"), value aggregated over ranks.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--chunk C] [--no-sweep] [--impl kairos|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--chunk C] [--no-sweep] [--fp8-only] [--impl kairos|reference]
   torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 Timing: W >= 3 warm-up steps, then exactly K steps bracketed by barrier + torch.cuda.synchronize, CUDA events on the
@@ -316,6 +316,47 @@ def roofline_entry(pt: Point, us_per_step: float, kern_us: float, peaks) -> dict
             "kernel_frac": roof / kern_us if kern_us > 0 else None}
 
 
+FP8_TOKEN_BYTES = 512 + 4 + 128  # e4m3 latent codes + one f32 scale + bf16 RoPE key (include/kairos.h, G23)
+
+
+def fp8_decode_leg(K, torch, dev, peaks, steps, warmup):
+    """the decodes of configs[3] (256 x 2,048 cached tokens, C = 0) over the fp8 latent cache.  The cache is
+    built on the device by kairos_fp8_append from the same synthetic tokens; one step reads 338 MiB (> 2x L2: no flush)."""
+    inp = W.make_config(3, chunk_len=0)
+    pool16 = K.bf16_tensor(inp.pool)
+    ws = torch.empty(K.workspace_bytes(inp.n_dec, 1), dtype=torch.uint8, device=dev)
+    ctx = K.Kairos(pool16, ws, inp.softmax_scale)
+    pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device=dev)
+    ctx.fp8_attach(pool8, inp.n_dec)
+    dpt = torch.from_numpy(inp.dec_page_tables).to(dev)
+    for i in range(inp.n_dec):
+        L = int(inp.dec_ctx_lens[i])
+        tok = ctx.gather_latent(dpt[i], L)
+        ctx.fp8_append(tok[:, :512].contiguous(), tok[:, 512:].contiguous(), dpt[i], 0)
+    qd = K.bf16_tensor(inp.q_dec)
+    od = torch.empty((inp.n_dec, 16, 512), dtype=torch.bfloat16, device=dev)
+    for _ in range(max(warmup, 3)):
+        ctx.fp8_decode(qd, dpt, inp.dec_ctx_lens, out_dec=od, want_lse=False)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n = max(steps, 200)
+    e0.record()
+    for _ in range(n):
+        ctx.fp8_decode(qd, dpt, inp.dec_ctx_lens, out_dec=od, want_lse=False)
+    e1.record()
+    torch.cuda.synchronize()
+    us = e0.elapsed_time(e1) * 1e3 / n
+    tokens = int(inp.dec_ctx_lens.astype(np.int64).sum())
+    alg = tokens * FP8_TOKEN_BYTES + inp.n_dec * (W.Q_BYTES + W.OUT_BYTES)
+    info = ctx.last_plan_info()
+    return {"workload": "configs[3] C=0 decodes over the fp8 latent cache (kairos_fp8_decode)", "B": inp.n_dec, "cached_tokens": tokens,
+            "step_us": us, "steps": n, "algorithmic_bytes": alg, "bytes_per_token": FP8_TOKEN_BYTES,
+            "roofline": {"bound": "hbm", "achieved": alg / (us * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": alg / (us * 1e-6) / 1e9 / peaks["hbm_gbs"], "roofline_us": alg / peaks["hbm_gbs"] / 1e3},
+            "kernels_per_step": info["kernels"], "graph": info["graph"], "dtype": "e4m3 cache, bf16 q / out, f32 accumulation",
+            "l2": "one step reads 338 MiB > 2x L2: no flush needed"}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -327,6 +368,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="time the headline workload only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fp8-only", action="store_true", help="run the fp8 latent-cache decode leg alone and print its entry (profiling)")
     ap.add_argument("--no-tune", action="store_true", help="keep the planner's own launch order (skip kairos_tune_step in the warm-up)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -355,6 +397,10 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.fp8_only:
+        print(json.dumps({"fp8_decode": fp8_decode_leg(K, torch, dev, peaks, args.steps, args.warmup)}), flush=True)
+        return
 
     # ---- headline workload first (clock / throttle reasons are sampled over its timed regions only)
     pt = Point(args.config, args.chunk, R_.replica_seed_shift(rank), dev, K, torch)
@@ -392,6 +438,10 @@ def main():
             sweep.append(e)
             sp.close()
             del sp
+
+    fp8 = None
+    if world == 1 and not args.no_sweep:
+        fp8 = fp8_decode_leg(K, torch, dev, peaks, args.steps, args.warmup)
 
     ms_max = R_.max_over_ranks(ms_head, dev)
     us_per_step = R_.whole_job_us_per_step(ms_head, args.steps, world, dev)  # world replicas advance one step per iteration
@@ -480,6 +530,7 @@ def main():
         "achieved": {"algorithmic_GBps": pt.alg_bytes / (us_per_step * world * 1e-6) / 1e9,
                      "algorithmic_TFLOPs": pt.alg_flops / (us_per_step * world * 1e-6) / 1e12},
         "sweep": sweep,
+        "fp8_decode": fp8,
     }
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -142,12 +142,19 @@ constexpr int kThreads = 64 + kSoftmaxThreads + 64;
 constexpr int kPvWarp = 2 + kSoftmaxWarps;
 constexpr int kSbWarp = kPvWarp + 1;
 constexpr int kSlotBytes = 8192;      // one box: [64 tokens][128 B] = 128 latent codes, or the 64 bf16 RoPE values, SWIZZLE_128B
-constexpr int kStages = 4;            // pages in flight: 4 x 5 slots (4 latent boxes + RoPE) = 160 KB
+// Pages in flight: a page's latent boxes stay in shared memory from their TMA request until its PV product completes (~8,000
+// cycles: load latency + S + the softmax chain + PV), so the page rate is that lifetime over the ring depth; four stages gave
+// 2,050 cycles per page against 1,770 of HBM time.  The RoPE box is only read by the S product: it lives in a ring of its own
+// (two slots, released as soon as the page's S MMAs retire), which leaves room for FIVE latent stages.
+constexpr int kStages = 5;            // latent stages of 4 boxes (32 KB)
+constexpr int kStageBytes = 4 * kSlotBytes;
+constexpr int kRopeSlots = 2;
 constexpr int kQBufBytes = kQ8Bytes + 16 * kRope * 2;  // 18,432: q8 (4 boxes of [32 rows][128 B]) | q_rope [16 rows][128 B]
 constexpr int kPBytes = 4096;         // P8 [32 rows: hi 16 | lo 16][64 keys], K-major, rows padded to 128 B
 constexpr int kOffQ = 0;
 constexpr int kOffKV = 2 * kQBufBytes;
-constexpr int kOffP = kOffKV + kStages * 5 * kSlotBytes;
+constexpr int kOffRopeRing = kOffKV + kStages * kStageBytes;
+constexpr int kOffP = kOffRopeRing + kRopeSlots * kSlotBytes;
 constexpr int kOffSmall = kOffP + 2 * kPBytes;
 constexpr int kSmallBytes = 4096;
 constexpr int kSmemBytes = kOffSmall + kSmallBytes + 1024;
@@ -167,7 +174,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;
 
 struct Small8 {
-    uint64_t q_full[2], q_empty[2], kv_full[kStages][2], kv_empty[kStages], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kStages][2], kv_empty[kStages], rope_full[kRopeSlots], rope_empty[kRopeSlots], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -271,7 +278,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     const int npages = w.page_end - w.page_begin;
     for (int pg = 0; pg < npages; ++pg, ++g) {
         const int b = g & 1;
-        const int st = g & (kStages - 1);
+        const int st = g % kStages;
         // the token scales came with the page's first boxes, long before its S product completes: fetch them first
         mbar_wait(&sm->kv_full[st][0], (g / kStages) & 1);
         const float sc = lane_ok ? sm->scales[st][tok_in_page] : 1.f;
@@ -354,7 +361,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
             // 0 * NaN = NaN.  Zero the token's 128 B in two of the four latent boxes (the other column half takes the rest).
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                uint4* dst = reinterpret_cast<uint4*>(kv + (st * 5 + (sw >> 2) * 2 + c) * kSlotBytes + tok_in_page * 128);
+                uint4* dst = reinterpret_cast<uint4*>(kv + st * kStageBytes + ((sw >> 2) * 2 + c) * kSlotBytes + tok_in_page * 128);
 #pragma unroll
                 for (int j = 0; j < 8; ++j) dst[j] = make_uint4(0u, 0u, 0u, 0u);
             }
@@ -442,14 +449,14 @@ __device__ __forceinline__ void s_item8(Small8* sm, uint32_t tmem, uint32_t q_ba
     mbar_wait(&sm->q_full[qbuf], qfull_parity);
     for (int s = 0; s < npages; ++s) {
         const uint32_t gg = g0 + s;
-        const uint32_t sb = gg & 1, st = gg & (kStages - 1), par = (gg / kStages) & 1;
+        const uint32_t sb = gg & 1, st = gg % kStages, par = (gg / kStages) & 1;
         mbar_wait(&sm->s_empty[sb], ((gg >> 1) & 1) ^ 1);
         mbar_wait(&sm->kv_full[st][HALF], par);
         tc_fence_after();
 #pragma unroll
         for (uint32_t bb = 0; bb < 2; ++bb) {
             const uint32_t b = 2 * HALF + bb;
-            const uint32_t ka_lo = smem_desc_lo(kv_base + (st * 5 + b) * kSlotBytes, 16);
+            const uint32_t ka_lo = smem_desc_lo(kv_base + st * kStageBytes + b * kSlotBytes, 16);
             const uint32_t qb_lo = smem_desc_lo(q_base + b * 4096, 16);
 #pragma unroll
             for (uint32_t j = 0; j < 4; ++j)
@@ -457,13 +464,16 @@ __device__ __forceinline__ void s_item8(Small8* sm, uint32_t tmem, uint32_t q_ba
                                 idesc_s8, !(bb == 0 && j == 0));
         }
         if (HALF == 1) {
-            const uint32_t ka_lo = smem_desc_lo(kv_base + (st * 5 + 4) * kSlotBytes, 16);
+            mbar_wait(&sm->rope_full[gg & 1], (gg >> 1) & 1);
+            tc_fence_after();
+            const uint32_t ka_lo = smem_desc_lo(kv_base + kStages * kStageBytes + (gg & 1) * kSlotBytes, 16);
             const uint32_t qb_lo = smem_desc_lo(q_base + kQ8Bytes, 16);
 #pragma unroll
             for (uint32_t j = 0; j < 4; ++j)
                 umma_bf16_ss_lohi(tmem + kColS + sb * kSBuf + 64, ka_lo + ((j * 32) >> 4), desc_hi, qb_lo + ((j * 32) >> 4), desc_hi, idesc_sr, j > 0);
         }
         umma_commit_elect(&sm->s_full[sb]);
+        if (HALF == 1) umma_commit_elect(&sm->rope_empty[gg & 1]);  // the RoPE box is only ever read by these MMAs
         if (s == npages - 1) umma_commit_elect(&sm->q_empty[qbuf]);
     }
 }
@@ -474,14 +484,14 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
     for (int pv = 0; pv < npages; ++pv) {
         const uint32_t gg = g0 + pv;
-        const uint32_t pst = gg & 1, pph = (gg >> 1) & 1, st = gg & (kStages - 1);
+        const uint32_t pst = gg & 1, pph = (gg >> 1) & 1, st = gg % kStages;
         mbar_wait(&sm->p_full[pst], pph);
         if (pv == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);
         tc_fence_after();
         const uint32_t pb_lo = smem_desc_lo(p_base + pst * kPBytes, 16);
 #pragma unroll
         for (uint32_t b4 = 0; b4 < 4; ++b4) {
-            const uint32_t va_lo = smem_desc_lo(kv_base + (st * 5 + b4) * kSlotBytes, 8192);
+            const uint32_t va_lo = smem_desc_lo(kv_base + st * kStageBytes + b4 * kSlotBytes, 8192);
 #pragma unroll
             for (uint32_t ks = 0; ks < 2; ++ks)  // 32 keys per instruction: 32 rows of 128 B further down the box
                 umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 32) >> 4), desc_hi, idesc_o8,
@@ -516,6 +526,10 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             mbar_init(&sm->kv_full[i][0], 1);
             mbar_init(&sm->kv_full[i][1], 1);
             mbar_init(&sm->kv_empty[i], 1);
+        }
+        for (int i = 0; i < kRopeSlots; ++i) {
+            mbar_init(&sm->rope_full[i], 1);
+            mbar_init(&sm->rope_empty[i], 1);
         }
         mbar_init(&sm->o_full, 1);
         mbar_init(&sm->o_empty, kSoftmaxWarps);
@@ -566,7 +580,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                 tma_load_2d(qdst + kQ8Bytes, &qr_map, &sm->q_full[qb], kLatent, w.q_index * kHeads, kEvictFirst);
             };
             // the first item's q is requested behind its first pages (they fill the empty ring without waiting)
-            const int q_at = it == 0 ? min(npages, kStages) : 0;
+            const int q_at = it == 0 ? min(npages, kRopeSlots) : 0;  // not later: page 2's RoPE slot frees when S(0) retires, and S needs q
             if (lane == 0 && q_at == 0) load_q();
             const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
             for (int i = 0; i < npages; i += 32) {
@@ -576,14 +590,16 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
                         if (q_at > 0 && i + j == q_at) load_q();
-                        const uint32_t st = g & (kStages - 1), par = ((g / kStages) & 1) ^ 1;
+                        const uint32_t st = g % kStages, par = ((g / kStages) & 1) ^ 1;
                         mbar_wait(&sm->kv_empty[st], par);
                         mbar_arrive_expect_tx(&sm->kv_full[st][0], 2 * kSlotBytes + kPage * 4);
-                        mbar_arrive_expect_tx(&sm->kv_full[st][1], 3 * kSlotBytes);
+                        mbar_arrive_expect_tx(&sm->kv_full[st][1], 2 * kSlotBytes);
 #pragma unroll
                         for (int b = 0; b < 4; ++b)
-                            tma_load_3d(kv_u32 + (st * 5 + b) * kSlotBytes, &lat_map, &sm->kv_full[st][b >> 1], b * 128, 0, pid, kEvictFirst);
-                        tma_load_3d(kv_u32 + (st * 5 + 4) * kSlotBytes, &rope_map, &sm->kv_full[st][1], 0, 0, pid, kEvictFirst);
+                            tma_load_3d(kv_u32 + st * kStageBytes + b * kSlotBytes, &lat_map, &sm->kv_full[st][b >> 1], b * 128, 0, pid, kEvictFirst);
+                        mbar_wait(&sm->rope_empty[g & 1], ((g >> 1) & 1) ^ 1);  // S of page g - 2 retired long before a latent stage frees
+                        mbar_arrive_expect_tx(&sm->rope_full[g & 1], kSlotBytes);
+                        tma_load_3d(kv_u32 + kStages * kStageBytes + (g & 1) * kSlotBytes, &rope_map, &sm->rope_full[g & 1], 0, 0, pid, kEvictFirst);
                         bulk_load(smem_u32(sm->scales[st]), p.pool8 + size_t(pid) * kPage8Bytes + kOffScale8, kPage * 4, &sm->kv_full[st][0],
                                   kEvictFirst);
                     }
