@@ -55,7 +55,7 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
 
 
-KERNEL_SOURCES = ["append.cu", "attn_pair.cu", "attn_umma.cu", "plan.cpp", "umma_ptx.cuh"]
+KERNEL_SOURCES = ["append.cu", "attn_pair.cu", "attn_umma.cu", "plan.cpp", "umma_ptx.cuh", "fp8.cu"]
 
 
 def csrc_sha() -> str:
@@ -352,7 +352,9 @@ def fp8_decode_leg(K, torch, dev, peaks, steps, warmup):
     return {"workload": "configs[3] C=0 decodes over the fp8 latent cache (kairos_fp8_decode)", "B": inp.n_dec, "cached_tokens": tokens,
             "step_us": us, "steps": n, "algorithmic_bytes": alg, "bytes_per_token": FP8_TOKEN_BYTES,
             "roofline": {"bound": "hbm", "achieved": alg / (us * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                         "frac": alg / (us * 1e-6) / 1e9 / peaks["hbm_gbs"], "roofline_us": alg / peaks["hbm_gbs"] / 1e3},
+                         "frac": alg / (us * 1e-6) / 1e9 / peaks["hbm_gbs"], "roofline_us": alg / peaks["hbm_gbs"] / 1e3,
+                         "note": "whole step (query split + attention + combine) over the HBM time of its algorithmic bytes"},
+            "traffic": measured_traffic("fp8_config3_C0")[0],
             "kernels_per_step": info["kernels"], "graph": info["graph"], "dtype": "e4m3 cache, bf16 q / out, f32 accumulation",
             "l2": "one step reads 338 MiB > 2x L2: no flush needed"}
 
