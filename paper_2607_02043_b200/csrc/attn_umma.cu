@@ -280,15 +280,16 @@ __device__ __forceinline__ void softmax_item(Small* sm, uint8_t* kv, const WorkI
             }
         }
         if (PK) {
-            // decode-only instantiation: P as a K-major B operand [16 query rows][64 keys] (2 KB, SWIZZLE_128B) in a buffer of
-            // its own, so that the page's RoPE slot can go back to the ring as soon as the S MMAs have read it
+            // decode-only instantiation: P as the MN-major B operand [64 keys][16 query rows x 2 B] (2 KB, SWIZZLE_32B: the 16-byte
+            // chunk index is XORed with bit 2 of the row) in a buffer of its own, so that the page's RoPE slot can go back to the
+            // ring as soon as the S MMAs have read it.  This thread's key row takes ONE 16-byte store for its 8 heads.
             if (g >= 2) mbar_wait(&sm->pv_done[b], ((g - 2) >> 1) & 1);  // PV of page g - 2 has read this P buffer
             if (lane_ok) {
                 uint8_t* pb = kv + R * kSlotBytes + b * kDecPBytes;
                 const uint32_t kk = uint32_t(tok_in_page);
-#pragma unroll
-                for (int c = 0; c < NC; ++c)
-                    *reinterpret_cast<__nv_bfloat16*>(pb + sw128_offset(uint32_t(cbase + c), kk >> 3) + (kk & 7u) * 2u) = __float2bfloat16_rn(x[c]);
+                static_assert(!PK || NC == 8, "one 16-byte chunk per column half");
+                *reinterpret_cast<uint4*>(pb + kk * 32u + (((uint32_t(cbase) >> 3) ^ ((kk >> 2) & 1u)) << 4)) =
+                    make_uint4(pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]), pack_bf16(x[4], x[5]), pack_bf16(x[6], x[7]));
             }
         } else if (lane_ok) {  // P^T as the MN-major B operand: row = key, N bf16 along the row, SWIZZLE_128B
             uint8_t* ps = kv + page_slots<R>(g).rope * kSlotBytes;
@@ -432,9 +433,11 @@ __device__ __forceinline__ void s_item(Small* sm, uint32_t tmem, uint32_t q_base
 
 template <int N, int R, bool PK>
 __device__ __forceinline__ void pv_item(Small* sm, uint32_t tmem, uint32_t kv_base, int npages, uint32_t g0, uint32_t it) {
-    // O^T += V^T P^T : A = the page's latent slots MN-major; B = P, MN-major in the page's RoPE slot, or (PK) K-major in its own buffer
-    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, PK ? 0 : 1);
+    // O^T += V^T P^T : A = the page's latent slots MN-major; B = P, MN-major in the page's RoPE slot (SWIZZLE_128B), or (PK) in its own
+    // 2 KB buffer (SWIZZLE_32B)
+    constexpr uint32_t idesc_o = make_idesc_bf16(128, N, 1, 1);
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
+    constexpr uint32_t pdesc_hi = PK ? smem_desc_hi_sw32(256) : desc_hi;  // PK: P in atoms of 8 key rows x 32 B
     for (int pv = 0; pv < npages; ++pv) {
         const uint32_t gg = g0 + pv;
         const uint32_t pst = gg & 1, pph = (gg >> 1) & 1;
@@ -451,7 +454,7 @@ __device__ __forceinline__ void pv_item(Small* sm, uint32_t tmem, uint32_t kv_ba
 #pragma unroll
             for (uint32_t ks = 0; ks < 4; ++ks)
                 umma_bf16_ss_lohi(tmem + kColO + b4 * 64, va_lo + ((ks * 2048) >> 4), desc_hi,
-                                  pb_lo + ((PK ? ks * 32 : ks * 2048) >> 4), desc_hi, idesc_o, (pv > 0 || ks > 0));
+                                  pb_lo + ((PK ? ks * 512 : ks * 2048) >> 4), pdesc_hi, idesc_o, (pv > 0 || ks > 0));
             umma_commit_elect(&empty[b4]);  // slot pair b4 goes back to the ring when this block's MMAs retire
         }
         if (!PK) umma_commit_elect(&empty[4]);  // P^T sat in the RoPE slot

@@ -8,7 +8,7 @@
 //   SR^T[64 keys x 16] = KR_page[64 x 64]  . QR^T                kind::f16 (bf16), M=64 N=16 K=16, 4 per page
 //   x[t,h] = ((S8hi + S8lo) * s_t / g_h + SR) * sigma*log2(e)      s_t = the token's scale, g_h = the query row's gain (2^k)
 //   y = x + log2(s_t):  P8[t,h] = 2^(y - m_h), split into two e4m3 terms;  l_h += P8 / s_t   (= 2^(x - m_h))
-//   O^T[512 x 32]     += V8^T[512 x 64] . [Phi ; Plo]^T           kind::f8f6f4, M=128 N=32 K=32, A MN-major = the same page
+//   O^T[512 x 32]     += V8^T[512 x 64] . [Phi ; Plo]^T           kind::f8f6f4, M=128 N=32 K=32, A and B MN-major (A = the same page)
 //   out[h] = (O[:,h] + O[:,16+h]) / l_h
 //
 // The token scale rides the softmax weight (P8 = p * s_t), so that O accumulates real dequantised values without touching
@@ -150,7 +150,7 @@ constexpr int kStages = 5;            // latent stages of 4 boxes (32 KB)
 constexpr int kStageBytes = 4 * kSlotBytes;
 constexpr int kRopeSlots = 2;
 constexpr int kQBufBytes = kQ8Bytes + 16 * kRope * 2;  // 18,432: q8 (4 boxes of [32 rows][128 B]) | q_rope [16 rows][128 B]
-constexpr int kPBytes = 4096;         // P8 [32 rows: hi 16 | lo 16][64 keys], K-major, rows padded to 128 B
+constexpr int kPBytes = 2048;         // P8 [64 keys][32 B: hi 16 heads | lo 16 heads], MN-major, SWIZZLE_32B
 constexpr int kOffQ = 0;
 constexpr int kOffKV = 2 * kQBufBytes;
 constexpr int kOffRopeRing = kOffKV + kStages * kStageBytes;
@@ -370,12 +370,12 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         if (lane_ok) {
             uint8_t* pb = pbuf + b * kPBytes;
             const uint32_t kk = uint32_t(tok_in_page);
-#pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                const uint32_t hi = (chi[c / 2] >> (8 * (c & 1))) & 0xffu, lo = (clo[c / 2] >> (8 * (c & 1))) & 0xffu;
-                pb[sw128_offset(uint32_t(cbase + c), kk >> 4) + (kk & 15u)] = uint8_t(hi);
-                pb[sw128_offset(uint32_t(16 + cbase + c), kk >> 4) + (kk & 15u)] = uint8_t(lo);
-            }
+            // P8 is the MN-major B operand [64 keys][32 B: hi terms of heads 0-15 | lo terms], SWIZZLE_32B (the 16-byte chunk index
+            // is XORed with bit 2 of the row): this thread's key row takes two 8-byte stores (sixteen byte stores into a K-major
+            // tile cost 144 bank conflicts per page and 4 us of the step)
+            const uint32_t sx = (kk >> 2) & 1u;
+            *reinterpret_cast<uint2*>(pb + kk * 32u + ((0u ^ sx) << 4) + uint32_t(cbase)) = make_uint2(chi[0] | (chi[1] << 16), chi[2] | (chi[3] << 16));
+            *reinterpret_cast<uint2*>(pb + kk * 32u + ((1u ^ sx) << 4) + uint32_t(cbase)) = make_uint2(clo[0] | (clo[1] << 16), clo[2] | (clo[3] << 16));
         }
         fence_proxy_async_smem();
         tc_fence_before();
@@ -480,7 +480,8 @@ __device__ __forceinline__ void s_item8(Small8* sm, uint32_t tmem, uint32_t q_ba
 
 // PV MMAs (warp kPvWarp): O^T block b4 += V8^T block b4 [128 dims x 64 keys] (MN-major view of latent box b4) . P8^T
 __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_base, uint32_t p_base, int npages, uint32_t g0, uint32_t it) {
-    constexpr uint32_t idesc_o8 = make_idesc_e4m3(128, 32, 1, 0);
+    constexpr uint32_t idesc_o8 = make_idesc_e4m3(128, 32, 1, 1);
+    constexpr uint32_t pdesc_hi = smem_desc_hi_sw32(256);  // P8: 8 key rows of 32 B per swizzle atom
     constexpr uint32_t desc_hi = smem_desc_hi(1024);
     for (int pv = 0; pv < npages; ++pv) {
         const uint32_t gg = g0 + pv;
@@ -494,7 +495,7 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
             const uint32_t va_lo = smem_desc_lo(kv_base + st * kStageBytes + b4 * kSlotBytes, 8192);
 #pragma unroll
             for (uint32_t ks = 0; ks < 2; ++ks)  // 32 keys per instruction: 32 rows of 128 B further down the box
-                umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 32) >> 4), desc_hi, idesc_o8,
+                umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 1024) >> 4), pdesc_hi, idesc_o8,
                                 (pv > 0 || ks > 0));
         }
         umma_commit_elect(&sm->kv_empty[st]);  // the whole stage (the S MMAs of this page completed before its softmax started)

@@ -158,6 +158,8 @@ __device__ __forceinline__ void umma_commit_elect(uint64_t* bar) {
 }
 // halves of make_smem_desc: lo = start address | LBO, hi = SBO | version 1 | SWIZZLE_128B
 __host__ __device__ constexpr uint32_t smem_desc_hi(uint32_t sbo_bytes) { return ((sbo_bytes >> 4) & 0x3FFFu) | (1u << 14) | (2u << 29); }
+// the same with SWIZZLE_32B (layout type 6): atoms of 8 rows x 32 B, 16-byte chunk index XORed with bit 2 of the row
+__host__ __device__ constexpr uint32_t smem_desc_hi_sw32(uint32_t sbo_bytes) { return ((sbo_bytes >> 4) & 0x3FFFu) | (1u << 14) | (6u << 29); }
 __device__ __forceinline__ uint32_t smem_desc_lo(uint32_t saddr, uint32_t lbo_bytes) { return ((saddr >> 4) & 0x3FFFu) | (((lbo_bytes >> 4) & 0x3FFFu) << 16); }
 
 // mbarrier arrives once all tcgen05.mma issued so far by the leader lane have completed (implies
