@@ -131,16 +131,18 @@ __global__ void __launch_bounds__(512) fp8_quant_q_kernel(const uint4* __restric
 
 // ------------------------------------------------------------------------------------------------------------
 // decode attention over fp8 pages.  Warp roles: warp 0 producer, warp 1 S issuer A (latent boxes 0-1) + TMEM owner, warps 2-9
-// softmax / epilogue, warp 10 PV issuer, warp 11 S issuer B (latent boxes 2-3 + RoPE).  Issuing a tcgen05.mma costs its warp
+// softmax / correction, warp 10 PV issuer, warp 11 S issuer B (latent boxes 2-3 + RoPE), warps 12-15 epilogue (O^T is
+// double-buffered by item parity, so an item's output is written while the next item's pages stream).  Issuing a tcgen05.mma costs its warp
 // ~40 cycles and an mbarrier wait ~100 whether or not it blocks: one warp issuing the page's 20 S MMAs behind five waits was
 // the longest stage of the pipeline (2,250 cycles per page, measured), so the S product is cut in two halves that accumulate
 // in separate TMEM columns (summed by the softmax warps, in a fixed order) and a page has two landing barriers, not five.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kSoftmaxWarps = 8;
 constexpr int kSoftmaxThreads = kSoftmaxWarps * 32;
-constexpr int kThreads = 64 + kSoftmaxThreads + 64;
 constexpr int kPvWarp = 2 + kSoftmaxWarps;
 constexpr int kSbWarp = kPvWarp + 1;
+constexpr int kEpiWarp = kSbWarp + 1;  // 12..15: epilogue warps (TMEM lane quadrant = warp & 3)
+constexpr int kThreads = 64 + kSoftmaxThreads + 64 + 128;
 constexpr int kSlotBytes = 8192;      // one box: [64 tokens][128 B] = 128 latent codes, or the 64 bf16 RoPE values, SWIZZLE_128B
 // Pages in flight: a page's latent boxes stay in shared memory from their TMA request until its PV product completes (~8,000
 // cycles: load latency + S + the softmax chain + PV), so the page rate is that lifetime over the ring depth; four stages gave
@@ -164,7 +166,8 @@ static_assert(kOffKV % 1024 == 0 && kOffP % 1024 == 0, "operand tiles must stay 
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0;    // S^T buffers at columns 0 and 96: [0,32) boxes 0-1 hi|lo, [32,64) boxes 2-3 hi|lo, [64,80) RoPE
 constexpr uint32_t kSBuf = 96;
-constexpr uint32_t kColO = 192;  // O^T block b at 192 + 32 b: [0,16) from P hi, [16,32) from P lo
+constexpr uint32_t kColO = 192;  // O^T of item parity r, block b at 192 + 128 r + 32 b: [0,16) from P hi, [16,32) from P lo
+constexpr uint32_t kOBuf = 128;
 // The reference m sits kHeadroom binades below the largest y seen when it was last refreshed, and is refreshed when some
 // y exceeds it by more than kRefresh: P8 = 2^(y - m) <= 2^8 = 256 < 448, and a weight 2^-10 below the largest still is a
 // normal e4m3 number (2^-6).
@@ -174,7 +177,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kMinusHuge = -1.0e30f;
 
 struct Small8 {
-    uint64_t q_full[2], q_empty[2], kv_full[kStages][2], kv_empty[kStages], rope_full[kRopeSlots], rope_empty[kRopeSlots], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full, o_empty;
+    uint64_t q_full[2], q_empty[2], kv_full[kStages][2], kv_empty[kStages], rope_full[kRopeSlots], rope_empty[kRopeSlots], s_full[2], s_empty[2], p_full[2], pv_done[2], o_full[2], o_empty[2], stat_full[2], stat_empty[2];
     uint64_t item_full[2], item_empty[2];
     int32_t item_ring[2];
     uint32_t tmem_base;
@@ -183,7 +186,8 @@ struct Small8 {
     float m_ref[16];
     float alpha[16];
     float red[4][16];
-    float linv[16];
+    float stat_m[2][16];  // [item parity]: the item's final reference and row sums, handed to the epilogue warps
+    float stat_l[2][16];
 };
 static_assert(sizeof(Small8) <= kSmallBytes, "Small8 does not fit");
 
@@ -266,6 +270,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     const int tid_s = sw * 32 + lane;
     const bool lane_ok = lane < 16;
     const int tok_in_page = w4 * 16 + lane;
+    const int ip = it & 1;  // O^T accumulator and statistics rows of this item
     float l[NC], gi[NC];
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
@@ -334,7 +339,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
 #pragma unroll
                     for (int half = 0; half < 2; ++half) {
                         uint32_t r[NC];
-                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + half * 16 + cbase);
+                        const uint32_t ta = tmem_addr(tmem, w4 * 32, kColO + ip * kOBuf + b4 * 32 + half * 16 + cbase);
                         tmem_ld8(ta, *reinterpret_cast<uint32_t(*)[8]>(r));
                         tmem_wait_ld();
 #pragma unroll
@@ -382,9 +387,7 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm->p_full[b]);
     }
-    // ---- epilogue: all PV MMAs of the item are complete
-    mbar_wait(&sm->o_full, it & 1);
-    tc_fence_after();
+    // ---- hand the row statistics to the epilogue warps (they drain this item's O^T while these warps start the next item)
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         float v = l[c];
@@ -395,25 +398,48 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         if (lane == c) sm->red[w4][cbase + c] = v;
     }
     named_sync(1);
-    const bool is_final = w.partial_slot < 0;
     if (tid_s < 16) {
-        const float L = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
-        sm->linv[tid_s] = __fdividef(1.f, L);
-        const float m = sm->m_ref[tid_s];
-        if (is_final) {
-            if (p.lse_dec) p.lse_dec[size_t(w.q_index) * kHeads + tid_s] = (m + lg2(L)) * kLn2;
-        } else {
-            float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes + size_t(kHeads) * kLatent * 4);
-            ml[tid_s] = m;
-            ml[kHeads + tid_s] = L;
-        }
+        mbar_wait(&sm->stat_empty[ip], ((it >> 1) & 1) ^ 1);  // the epilogue of item it - 2 has read this pair of rows
+        sm->stat_l[ip][tid_s] = sm->red[0][tid_s] + sm->red[1][tid_s] + sm->red[2][tid_s] + sm->red[3][tid_s];
+        sm->stat_m[ip][tid_s] = sm->m_ref[tid_s];
     }
-    named_sync(2);
-    // O^T block b4: lane = latent dim 128 b4 + 32 w4 + lane; columns [0,16) from P hi, [16,32) from P lo
-    uint32_t rr[2][2 * NC];
+    named_sync(2);  // m_ref / red are free for the next item; the statistics are written
+    if (tid_s == 0) mbar_arrive(&sm->stat_full[ip]);
+}
+
+// Epilogue of one decode split (warps 12-15, one per TMEM lane quadrant): O^T of the item's accumulator -> bf16 output rows, or the
+// unnormalised fp32 partial of a KV split.  Runs beside the next item's pages (O^T is double-buffered by item parity).
+__device__ __forceinline__ void epilogue_item8(Small8* sm, const WorkItem& w, const K8Params& p, uint32_t tmem, int w4, int lane, uint32_t it) {
+    const int ip = it & 1;
+    mbar_wait(&sm->stat_full[ip], (it >> 1) & 1);
+    const bool is_final = w.partial_slot < 0;
+    float linv[kHeads];
+    {
+        const int h = lane & 15;
+        const float L = sm->stat_l[ip][h], m = sm->stat_m[ip][h];
+        const float mli = __fdividef(1.f, L);
+        if (w4 == 0 && lane < kHeads) {
+            if (is_final) {
+                if (p.lse_dec) p.lse_dec[size_t(w.q_index) * kHeads + h] = (m + lg2(L)) * kLn2;
+            } else {
+                float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes + size_t(kHeads) * kLatent * 4);
+                ml[h] = m;
+                ml[kHeads + h] = L;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < kHeads; ++c) linv[c] = __shfl_sync(0xffffffffu, mli, c);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm->stat_empty[ip]);
+    mbar_wait(&sm->o_full[ip], (it >> 1) & 1);  // all PV MMAs of the item are complete
+    tc_fence_after();
+    // O^T block b4: lane = latent dim 128 b4 + 32 w4 + lane; columns [0,16) from P hi, [16,32) from P lo.  The loads of block
+    // b4 + 1 are in flight while block b4 is converted and stored.
+    uint32_t rr[2][2 * kHeads];
     auto load_block = [&](int b4, uint32_t* r) {
-        tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + cbase), *reinterpret_cast<uint32_t(*)[8]>(r));
-        tmem_ld8(tmem_addr(tmem, w4 * 32, kColO + b4 * 32 + 16 + cbase), *reinterpret_cast<uint32_t(*)[8]>(r + NC));
+        tmem_ld16(tmem_addr(tmem, w4 * 32, kColO + ip * kOBuf + b4 * 32), *reinterpret_cast<uint32_t(*)[16]>(r));
+        tmem_ld16(tmem_addr(tmem, w4 * 32, kColO + ip * kOBuf + b4 * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(r + kHeads));
     };
     load_block(0, rr[0]);
 #pragma unroll
@@ -423,19 +449,18 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
         const uint32_t* r = rr[b4 & 1];
         const int d = b4 * 128 + w4 * 32 + lane;
         if (is_final) {
-            __nv_bfloat16* o = p.out_dec + (size_t(w.q_index) * kHeads + cbase) * kLatent + d;
+            __nv_bfloat16* o = p.out_dec + size_t(w.q_index) * kHeads * kLatent + d;
 #pragma unroll
-            for (int i = 0; i < NC; ++i)
-                o[i * kLatent] = __float2bfloat16_rn((__uint_as_float(r[i]) + __uint_as_float(r[NC + i])) * sm->linv[cbase + i]);
+            for (int i = 0; i < kHeads; ++i) o[i * kLatent] = __float2bfloat16_rn((__uint_as_float(r[i]) + __uint_as_float(r[kHeads + i])) * linv[i]);
         } else {
-            float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes) + cbase * kLatent + d;
+            float* o = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes) + d;
 #pragma unroll
-            for (int i = 0; i < NC; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[i]) + __uint_as_float(r[NC + i]));
+            for (int i = 0; i < kHeads; ++i) st_f32_evict_last(o + i * kLatent, __uint_as_float(r[i]) + __uint_as_float(r[kHeads + i]));
         }
     }
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(&sm->o_empty);
+    if (lane == 0) mbar_arrive(&sm->o_empty[ip]);
 }
 
 // S MMAs of one decode split, in two halves issued by two warps: half 0 = latent boxes 0-1 into columns [0,32) of the S buffer,
@@ -487,7 +512,7 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
         const uint32_t gg = g0 + pv;
         const uint32_t pst = gg & 1, pph = (gg >> 1) & 1, st = gg % kStages;
         mbar_wait(&sm->p_full[pst], pph);
-        if (pv == 0) mbar_wait(&sm->o_empty, (it & 1) ^ 1);
+        if (pv == 0) mbar_wait(&sm->o_empty[it & 1], ((it >> 1) & 1) ^ 1);  // the epilogue of item it - 2 has drained this accumulator
         tc_fence_after();
         const uint32_t pb_lo = smem_desc_lo(p_base + pst * kPBytes, 16);
 #pragma unroll
@@ -495,12 +520,12 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
             const uint32_t va_lo = smem_desc_lo(kv_base + st * kStageBytes + b4 * kSlotBytes, 8192);
 #pragma unroll
             for (uint32_t ks = 0; ks < 2; ++ks)  // 32 keys per instruction: 32 rows of 128 B further down the box
-                umma_f8_ss_lohi(tmem + kColO + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 1024) >> 4), pdesc_hi, idesc_o8,
+                umma_f8_ss_lohi(tmem + kColO + (it & 1) * kOBuf + b4 * 32, va_lo + ((ks * 4096) >> 4), desc_hi, pb_lo + ((ks * 1024) >> 4), pdesc_hi, idesc_o8,
                                 (pv > 0 || ks > 0));
         }
         umma_commit_elect(&sm->kv_empty[st]);  // the whole stage (the S MMAs of this page completed before its softmax started)
         umma_commit_elect(&sm->pv_done[pst]);
-        if (pv == npages - 1) umma_commit_elect(&sm->o_full);
+        if (pv == npages - 1) umma_commit_elect(&sm->o_full[it & 1]);
     }
 }
 
@@ -519,7 +544,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             mbar_init(&sm->s_full[i], 2);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
-            mbar_init(&sm->item_empty[i], 3 + kSoftmaxWarps);
+            mbar_init(&sm->item_empty[i], 3 + kSoftmaxWarps + 4);
             mbar_init(&sm->p_full[i], kSoftmaxWarps);
             mbar_init(&sm->pv_done[i], 1);
         }
@@ -532,8 +557,12 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             mbar_init(&sm->rope_full[i], 1);
             mbar_init(&sm->rope_empty[i], 1);
         }
-        mbar_init(&sm->o_full, 1);
-        mbar_init(&sm->o_empty, kSoftmaxWarps);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&sm->o_full[i], 1);
+            mbar_init(&sm->o_empty[i], 4);
+            mbar_init(&sm->stat_full[i], 1);
+            mbar_init(&sm->stat_empty[i], 4);
+        }
         fence_barrier_init();
     }
     if (warp == 0 && lane == 0) {
@@ -626,8 +655,19 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             else pv_item8(sm, tmem, kv_base, p_base, npages, g, it);
             g += npages;
         }
+    } else if (warp >= kEpiWarp) {
+        // ================= epilogue warps =================
+        for (uint32_t it = 0;; ++it) {
+            mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
+            const int idx = sm->item_ring[it & 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
+            if (idx < 0) break;
+            const WorkItem w = load_item8(p.items + idx);
+            epilogue_item8(sm, w, p, tmem, warp & 3, lane, it);
+        }
     } else {
-        // ================= softmax / correction / epilogue warps =================
+        // ================= softmax / correction warps =================
         const int sw = warp - 2;
         uint32_t g = 0;
         asm volatile("griddepcontrol.wait;" ::: "memory");  // the gains (and nothing else these warps read) come from the query preparation
