@@ -327,7 +327,7 @@ def fp8_decode_leg(K, torch, dev, peaks, steps, warmup):
     ws = torch.empty(K.workspace_bytes(inp.n_dec, 1), dtype=torch.uint8, device=dev)
     ctx = K.Kairos(pool16, ws, inp.softmax_scale)
     pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device=dev)
-    ctx.fp8_attach(pool8, inp.n_dec)
+    ctx.fp8_attach(pool8)
     dpt = torch.from_numpy(inp.dec_page_tables).to(dev)
     for i in range(inp.n_dec):
         L = int(inp.dec_ctx_lens[i])

@@ -449,22 +449,20 @@ int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const in
  *   on the codes themselves; q and the softmax weights enter them as a sum of two e4m3 terms (a 4-bit head and the 4-bit
  *   remainder), which keeps them at bf16's precision -- see DESIGN.md 6.7 for the error budget.
  *
- * kairos_fp8_attach     tells the context about an fp8 pool and the scratch the decode call stages its quantised queries in.
- *                       pool8 DEVICE [num_pages][41,216] bytes, 128-byte aligned; scratch DEVICE, 128-byte aligned, at least
- *                       kairos_fp8_scratch_bytes(max_decodes) bytes.  Both stay caller-owned and must outlive the context or
- *                       the next attach.  The bf16 pool given at create time is untouched: a context can serve both.
+ * kairos_fp8_attach     tells the context about an fp8 pool: pool8 DEVICE [num_pages][41,216] bytes, 128-byte aligned.  It stays
+ *                       caller-owned and must outlive the context or the next attach.  The bf16 pool given at create time is
+ *                       untouched: a context can serve both.
  * kairos_fp8_append     as kairos_append_latent (same arguments, same indexing, same errors) but quantises into the attached
  *                       fp8 pool.  BIT-EXACT against the definition above: codes, scales and RoPE bytes.
  * kairos_fp8_decode     as kairos_mixed_step with chunk_len = 0 over the fp8 pool: n_dec decodes, request i attends its first
  *                       dec_ctx_lens[i] cached tokens through row i of dec_page_tables.  Same planner (a0), split partials,
- *                       LSE combine, plan cache and graph replay as the bf16 step; one extra kernel quantises q first.
- *                       Stale slots of a request's last page never reach a result (any bit pattern, NaN codes included).
- *                       n_dec must not exceed the max_decodes the scratch was sized for.
+ *                       LSE combine, plan cache and graph replay as the bf16 step; q is split into its two e4m3 terms inside
+ *                       the kernel (no extra launch, no scratch).  Stale slots of a request's last page never reach a result
+ *                       (any bit pattern, NaN codes included).
  * Errors: INVALID_ARG (NULL / misaligned / sizes / no pool attached), WORKSPACE, CUDA.
  */
 #define KAIROS_FP8_PAGE_BYTES 41216
-size_t kairos_fp8_scratch_bytes(int32_t max_decodes);
-int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes);
+int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages);
 int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                       int32_t table_len, int32_t start_pos, void* cuda_stream);
 int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,

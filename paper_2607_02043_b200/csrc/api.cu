@@ -329,7 +329,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
     ctx->last_info[1] = plan.n_decode_items;
     ctx->last_info[2] = plan.n_chunk_items + int64_t(plan.pair_items.size());
     ctx->last_info[3] = std::min<int64_t>(plan.n_pairs > 0 && plan.dec_ctas > 0 ? plan.dec_ctas : umma_resident_ctas(ctx), int64_t(plan.items.size()));
-    ctx->last_info[4] = kernels_of(plan) + (fp8 ? 1 : 0);  // + the query preparation
+    ctx->last_info[4] = kernels_of(plan);
     ctx->last_info[5] = int64_t(kCounterBytes + size_t(plan.n_partial_slots) * kPartialSlotBytes);
     ctx->last_info[6] = plan.n_pairs;
     ctx->last_info[7] = cache_state;
@@ -823,15 +823,11 @@ int kairos_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
 }
 
 // ---- the fp8 latent cache ------------------------------------------------------------------------------
-size_t kairos_fp8_scratch_bytes(int32_t max_decodes) { return fp8_scratch_bytes(max_decodes); }
-
-int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes) {
+int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages) {
     if (int rc = check_ctx(ctx)) return rc;
-    if (!pool8 || !scratch || num_pages < 1) return fail(KAIROS_ERR_INVALID_ARG, "NULL pool8 / scratch or num_pages < 1");
-    if (reinterpret_cast<uintptr_t>(pool8) % 128 || reinterpret_cast<uintptr_t>(scratch) % 128)
-        return fail(KAIROS_ERR_INVALID_ARG, "pool8 / scratch must be 128-byte aligned");
-    if (scratch_bytes < fp8_scratch_bytes(1)) return fail(KAIROS_ERR_WORKSPACE, "scratch smaller than kairos_fp8_scratch_bytes(1)");
-    return fp8_attach(ctx, pool8, num_pages, scratch, scratch_bytes);
+    if (!pool8 || num_pages < 1) return fail(KAIROS_ERR_INVALID_ARG, "NULL pool8 or num_pages < 1");
+    if (reinterpret_cast<uintptr_t>(pool8) % 128) return fail(KAIROS_ERR_INVALID_ARG, "pool8 must be 128-byte aligned");
+    return fp8_attach(ctx, pool8, num_pages);
 }
 
 int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
@@ -852,8 +848,6 @@ int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
                       int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream) {
     if (int rc = check_ctx(ctx)) return rc;
     if (!ctx->fp8.attached) return fail(KAIROS_ERR_INVALID_ARG, "no fp8 pool attached (kairos_fp8_attach)");
-    if (n_dec > ctx->fp8.max_decodes)
-        return fail(KAIROS_ERR_WORKSPACE, "n_dec beyond the decodes the fp8 scratch was sized for: " + std::to_string(ctx->fp8.max_decodes));
     return mixed_step_impl(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, 0, 0, nullptr, nullptr, 0, out_dec,
                            nullptr, lse_dec, nullptr, static_cast<cudaStream_t>(cuda_stream), /*fp8=*/1);
 }

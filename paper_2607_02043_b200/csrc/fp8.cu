@@ -83,53 +83,6 @@ __global__ void __launch_bounds__(256) fp8_append_kernel(uint8_t* __restrict__ p
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// query preparation: one CTA per request, one warp per head.  Row (i, h) of the latent part is scaled by the power of two
-// g that puts its largest magnitude in [128, 256), then split into two e4m3 numbers: hi = rne(q g), lo = rne(q g - hi).
-// q8 layout (what the attention kernel's TMA boxes read): [request][128-dim block j 0..3][row 0..31][128 B], rows 0-15 the
-// hi terms of heads 0-15, rows 16-31 the lo terms.  ginv[i][h] = 1 / g.
-// ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512) fp8_quant_q_kernel(const uint4* __restrict__ q, uint8_t* __restrict__ q8, float* __restrict__ ginv) {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the attention grid may pre-launch; it waits for this one
-    const int lane = threadIdx.x & 31, h = threadIdx.x >> 5, i = blockIdx.x;
-    const uint4* row = q + (size_t(i) * kHeads + h) * (kTokenBytes / 16);
-    const uint4 a = __ldg(row + lane * 2), b = __ldg(row + lane * 2 + 1);
-    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-    float v[16];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        v[2 * k] = bf16_lo(w[k]);
-        v[2 * k + 1] = bf16_hi(w[k]);
-    }
-    float amax = 0.f;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) amax = fmaxf(amax, fabsf(v[k]));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-    int ex = 8;
-    if (amax > 0.f) (void)frexpf(amax, &ex);        // amax = f * 2^ex, f in [0.5, 1)
-    const int ge = min(8 - ex, 100);                // gain exponent: amax * 2^ge in [128, 256) (capped for denormal-small rows)
-    const float g = ldexpf(1.f, ge);
-    uint32_t chi[4], clo[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        uint32_t ch[2], cl[2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const float x0 = v[4 * k + 2 * u] * g, x1 = v[4 * k + 2 * u + 1] * g;
-            ch[u] = e4m3x2(x0, x1);
-            const float2 hv = e4m3x2_value(ch[u]);
-            cl[u] = e4m3x2(x0 - hv.x, x1 - hv.y);
-        }
-        chi[k] = ch[0] | (ch[1] << 16);
-        clo[k] = cl[0] | (cl[1] << 16);
-    }
-    uint8_t* dst = q8 + size_t(i) * kQ8Bytes + (lane >> 3) * 4096 + (lane & 7) * 16;
-    *reinterpret_cast<uint4*>(dst + h * 128) = make_uint4(chi[0], chi[1], chi[2], chi[3]);
-    *reinterpret_cast<uint4*>(dst + (16 + h) * 128) = make_uint4(clo[0], clo[1], clo[2], clo[3]);
-    if (lane == 0) ginv[size_t(i) * kHeads + h] = ldexpf(1.f, -ge);
-}
-
-// ------------------------------------------------------------------------------------------------------------
 // decode attention over fp8 pages.  Warp roles: warp 0 producer, warp 1 S issuer A (latent boxes 0-1) + TMEM owner, warps 2-9
 // softmax / correction, warp 10 PV issuer, warp 11 S issuer B (latent boxes 2-3 + RoPE), warps 12-15 epilogue (O^T is
 // double-buffered by item parity, so an item's output is written while the next item's pages stream).  Issuing a tcgen05.mma costs its warp
@@ -182,6 +135,7 @@ struct Small8 {
     int32_t item_ring[2];
     uint32_t tmem_base;
     uint32_t pad;
+    alignas(16) float ginv[2][16];             // 1 / g of the item's query rows (written with its q by the epilogue warps)
     alignas(16) float scales[kStages][kPage];  // the page's token scales (bulk-copied with its first box)
     float m_ref[16];
     float alpha[16];
@@ -198,7 +152,7 @@ struct K8Params {
     const int32_t* dec_pt;
     int32_t dec_stride;
     const uint8_t* pool8;
-    const float* ginv;
+    const uint4* q;      // q_dec, bf16 [n_dec][16][576]
     __nv_bfloat16* out_dec;
     float* lse_dec;
     uint8_t* partials;
@@ -272,12 +226,15 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     const int tok_in_page = w4 * 16 + lane;
     const int ip = it & 1;  // O^T accumulator and statistics rows of this item
     float l[NC], gi[NC];
+    mbar_wait(&sm->q_full[ip], (it >> 1) & 1);  // the gains are written with the item's q
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         l[c] = 0.f;
-        gi[c] = __ldg(p.ginv + size_t(w.q_index) * kHeads + cbase + c) * p.scale_log2;  // 1/g_h folded with sigma * log2(e)
+        gi[c] = sm->ginv[ip][cbase + c] * p.scale_log2;  // 1/g_h folded with sigma * log2(e)
     }
     if (tid_s < 16) sm->m_ref[tid_s] = kMinusHuge;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm->q_empty[ip]);  // with the S warps' commits: the q buffer (and its gains) may be refilled
     named_sync(1);
 
     const int npages = w.page_end - w.page_begin;
@@ -407,6 +364,65 @@ __device__ __forceinline__ void softmax_item8(Small8* sm, uint8_t* kv, uint8_t* 
     if (tid_s == 0) mbar_arrive(&sm->stat_full[ip]);
 }
 
+// Query preparation of one item by the four epilogue warps (warp r: heads 4r .. 4r + 3).  Row (item, h) of the latent part is scaled
+// by the power of two g that puts its largest magnitude in [128, 256) and split into two e4m3 numbers, hi = rne(q g) and
+// lo = rne(q g - hi), written straight into the B-operand tiles of the S MMAs: four [32 rows][128 B] SWIZZLE_128B boxes (rows 0-15
+// the hi terms of heads 0-15, rows 16-31 the lo terms), the bf16 RoPE part as a [16 rows][128 B] box, and 1 / g per head.
+__device__ __forceinline__ void prepare_q8(Small8* sm, uint8_t* qdst, int qb, const uint4* rows, int r, int lane) {
+    constexpr int kRowVecs = kTokenBytes / 16;  // 72
+    {   // RoPE part: 8 x 16 B per head, this warp's four heads in one pass
+        const int h = 4 * r + (lane >> 3), c = lane & 7;
+        *reinterpret_cast<uint4*>(qdst + kQ8Bytes + sw128_offset(uint32_t(h), uint32_t(c))) = __ldg(rows + h * kRowVecs + 64 + c);
+    }
+    uint4 ra[4], rb[4];  // lane L owns elements [16 L, 16 L + 16) of a row; the four rows are in flight together
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        ra[u] = __ldg(rows + (4 * r + u) * kRowVecs + lane * 2);
+        rb[u] = __ldg(rows + (4 * r + u) * kRowVecs + lane * 2 + 1);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int h = 4 * r + u;
+        const uint32_t wv[8] = {ra[u].x, ra[u].y, ra[u].z, ra[u].w, rb[u].x, rb[u].y, rb[u].z, rb[u].w};
+        float v[16];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            v[2 * k] = bf16_lo(wv[k]);
+            v[2 * k + 1] = bf16_hi(wv[k]);
+        }
+        float amax = 0.f;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) amax = fmaxf(amax, fabsf(v[k]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        int ex = 8;
+        if (amax > 0.f) (void)frexpf(amax, &ex);  // amax = f * 2^ex, f in [0.5, 1)
+        const int ge = min(8 - ex, 100);          // gain exponent: amax * 2^ge in [128, 256) (capped for denormal-small rows)
+        const float gn = ldexpf(1.f, ge);
+        uint32_t chi[4], clo[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t ch[2], cl[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const float x0 = v[4 * k + 2 * t] * gn, x1 = v[4 * k + 2 * t + 1] * gn;
+                ch[t] = e4m3x2(x0, x1);
+                const float2 hv = e4m3x2_value(ch[t]);
+                cl[t] = e4m3x2(x0 - hv.x, x1 - hv.y);
+            }
+            chi[k] = ch[0] | (ch[1] << 16);
+            clo[k] = cl[0] | (cl[1] << 16);
+        }
+        uint8_t* box = qdst + (lane >> 3) * 4096;
+        *reinterpret_cast<uint4*>(box + sw128_offset(uint32_t(h), uint32_t(lane & 7))) = make_uint4(chi[0], chi[1], chi[2], chi[3]);
+        *reinterpret_cast<uint4*>(box + sw128_offset(uint32_t(16 + h), uint32_t(lane & 7))) = make_uint4(clo[0], clo[1], clo[2], clo[3]);
+        if (lane == 0) sm->ginv[qb][h] = ldexpf(1.f, -ge);
+    }
+    fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm->q_full[qb]);
+}
+
 // Epilogue of one decode split (warps 12-15, one per TMEM lane quadrant): O^T of the item's accumulator -> bf16 output rows, or the
 // unnormalised fp32 partial of a KV split.  Runs beside the next item's pages (O^T is double-buffered by item parity).
 __device__ __forceinline__ void epilogue_item8(Small8* sm, const WorkItem& w, const K8Params& p, uint32_t tmem, int w4, int lane, uint32_t it) {
@@ -531,7 +547,7 @@ __device__ __forceinline__ void pv_item8(Small8* sm, uint32_t tmem, uint32_t kv_
 
 __global__ void __launch_bounds__(kThreads, 1)
 kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __grid_constant__ CUtensorMap rope_map,
-                         const __grid_constant__ CUtensorMap q8_map, const __grid_constant__ CUtensorMap qr_map, const K8Params p) {
+                         const K8Params p) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     Small8* sm = reinterpret_cast<Small8*>(base + kOffSmall);
@@ -539,8 +555,8 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
-            mbar_init(&sm->q_full[i], 1);
-            mbar_init(&sm->q_empty[i], 2);
+            mbar_init(&sm->q_full[i], 4);
+            mbar_init(&sm->q_empty[i], 2 + kSoftmaxWarps);
             mbar_init(&sm->s_full[i], 2);
             mbar_init(&sm->s_empty[i], kSoftmaxWarps);
             mbar_init(&sm->item_full[i], 1);
@@ -568,8 +584,6 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     if (warp == 0 && lane == 0) {
         prefetch_tensormap(&lat_map);
         prefetch_tensormap(&rope_map);
-        prefetch_tensormap(&q8_map);
-        prefetch_tensormap(&qr_map);
     }
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the combine grid may pre-launch
     if (warp == 1) tmem_alloc(&sm->tmem_base, kTmemCols);
@@ -577,9 +591,6 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm->tmem_base;
-    // Launched behind the query-preparation grid with programmatic stream serialisation: everything above overlapped it, and
-    // so do the first pages' loads (the cache does not depend on that grid).  Only what it wrote is waited for: the producer
-    // waits before the first q8 load, the softmax warps before they read the gains.
 
     if (warp == 0) {
         // ================= producer =================
@@ -599,19 +610,7 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             }
             if (idx < 0) break;
             const WorkItem w = load_item8(p.items + idx);
-            const int qb = int(it & 1);
             const int npages = w.page_end - w.page_begin;
-            auto load_q = [&]() {  // lane 0
-                if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
-                mbar_wait(&sm->q_empty[qb], ((it >> 1) & 1) ^ 1);
-                mbar_arrive_expect_tx(&sm->q_full[qb], uint32_t(kQBufBytes));
-                uint8_t* qdst = base + kOffQ + qb * kQBufBytes;
-                for (int j = 0; j < 4; ++j) tma_load_2d(qdst + j * 4096, &q8_map, &sm->q_full[qb], 0, (w.q_index * 4 + j) * 32, kEvictFirst);
-                tma_load_2d(qdst + kQ8Bytes, &qr_map, &sm->q_full[qb], kLatent, w.q_index * kHeads, kEvictFirst);
-            };
-            // the first item's q is requested behind its first pages (they fill the empty ring without waiting)
-            const int q_at = it == 0 ? min(npages, kRopeSlots) : 0;  // not later: page 2's RoPE slot frees when S(0) retires, and S needs q
-            if (lane == 0 && q_at == 0) load_q();
             const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
             for (int i = 0; i < npages; i += 32) {
                 const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
@@ -619,7 +618,6 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                 for (int j = 0; j < cnt; ++j, ++g) {
                     const int pid = __shfl_sync(0xffffffffu, my, j);
                     if (lane == 0) {
-                        if (q_at > 0 && i + j == q_at) load_q();
                         const uint32_t st = g % kStages, par = ((g / kStages) & 1) ^ 1;
                         mbar_wait(&sm->kv_empty[st], par);
                         mbar_arrive_expect_tx(&sm->kv_full[st][0], 2 * kSlotBytes + kPage * 4);
@@ -635,7 +633,6 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                     }
                 }
             }
-            if (lane == 0 && q_at > 0 && npages <= q_at) load_q();
         }
     } else if (warp == 1 || warp == kPvWarp || warp == kSbWarp) {
         // ================= MMA issuers =================
@@ -657,20 +654,29 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
         }
     } else if (warp >= kEpiWarp) {
         // ================= epilogue warps =================
+        // Per item: first its query rows (the S warps need them as soon as the item's first page has landed; the producer publishes an
+        // item about five pages ahead of that), then the output of the PREVIOUS item, whose last PV retires about now.
+        WorkItem prev{};
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
             const int idx = sm->item_ring[it & 1];
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm->item_empty[it & 1]);
+            WorkItem w{};
+            if (idx >= 0) {
+                w = load_item8(p.items + idx);
+                const int qb = int(it & 1);
+                mbar_wait(&sm->q_empty[qb], ((it >> 1) & 1) ^ 1);
+                prepare_q8(sm, base + kOffQ + qb * kQBufBytes, qb, p.q + size_t(w.q_index) * kHeads * (kTokenBytes / 16), warp - kEpiWarp, lane);
+            }
+            if (it > 0) epilogue_item8(sm, prev, p, tmem, warp & 3, lane, it - 1);
             if (idx < 0) break;
-            const WorkItem w = load_item8(p.items + idx);
-            epilogue_item8(sm, w, p, tmem, warp & 3, lane, it);
+            prev = w;
         }
     } else {
         // ================= softmax / correction warps =================
         const int sw = warp - 2;
         uint32_t g = 0;
-        asm volatile("griddepcontrol.wait;" ::: "memory");  // the gains (and nothing else these warps read) come from the query preparation
         for (uint32_t it = 0;; ++it) {
             mbar_wait(&sm->item_full[it & 1], (it >> 1) & 1);
             const int idx = sm->item_ring[it & 1];
@@ -697,15 +703,9 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
 
 }  // namespace
 
-size_t fp8_scratch_bytes(int32_t max_decodes) {
-    const size_t n = size_t(std::max(max_decodes, 1));
-    return (n * (kQ8Bytes + kHeads * 4) + 127) / 128 * 128;
-}
-
-int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes) {
+int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages) {
     Fp8State& f = ctx->fp8;
     f.attached = false;
-    const int32_t max_dec = int32_t(std::min<size_t>(scratch_bytes / (kQ8Bytes + kHeads * 4), size_t(1) << 20));
     {   // latent codes: [page][64 tokens][512 B], boxes of 128 codes x 64 tokens
         const uint64_t dims[3] = {uint64_t(kLatent), uint64_t(kPage), uint64_t(num_pages)};
         const uint64_t strides[2] = {uint64_t(kLatent), uint64_t(kPage8Bytes)};
@@ -718,17 +718,9 @@ int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, s
         const uint32_t box[3] = {uint32_t(kRope), uint32_t(kPage), 1};
         if (int rc = encode_tiled_map(&f.rope_map, /*u8=*/false, 3, static_cast<uint8_t*>(pool8) + kOffRope8, dims, strides, box)) return rc;
     }
-    {   // quantised queries: [request][block 4][row 32][128 B], one box = one block of one request
-        const uint64_t dims[2] = {128, uint64_t(max_dec) * 128};
-        const uint64_t strides[1] = {128};
-        const uint32_t box[2] = {128, 32};
-        if (int rc = encode_tiled_map(&f.q8_map, /*u8=*/true, 2, scratch, dims, strides, box)) return rc;
-    }
     KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_fp8_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     f.pool8 = pool8;
     f.num_pages = num_pages;
-    f.scratch = scratch;
-    f.max_decodes = max_dec;
     f.attached = true;
     return KAIROS_OK;
 }
@@ -741,13 +733,8 @@ int launch_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, i
     return KAIROS_OK;
 }
 
-// query preparation, then the attention grid behind it (programmatic stream serialisation: its prologue overlaps)
 int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, cudaStream_t stream) {
     Fp8State& f = ctx->fp8;
-    uint8_t* q8 = static_cast<uint8_t*>(f.scratch);
-    float* ginv = reinterpret_cast<float*>(q8 + size_t(f.max_decodes) * kQ8Bytes);
-    fp8_quant_q_kernel<<<a.n_dec, 512, 0, stream>>>(reinterpret_cast<const uint4*>(a.q_dec), q8, ginv);
-    KAIROS_CUDA_TRY(cudaGetLastError());
     K8Params p;
     p.items = dev_items;
     p.n_items = n_items;
@@ -755,7 +742,7 @@ int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_it
     p.dec_pt = a.dec_page_tables;
     p.dec_stride = a.dec_table_stride;
     p.pool8 = static_cast<const uint8_t*>(f.pool8);
-    p.ginv = ginv;
+    p.q = reinterpret_cast<const uint4*>(a.q_dec);
     p.out_dec = reinterpret_cast<__nv_bfloat16*>(a.out_dec);
     p.lse_dec = a.lse_dec;
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;
@@ -766,12 +753,9 @@ int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_it
     cfg.blockDim = dim3(kThreads, 1, 1);
     cfg.dynamicSmemBytes = kSmemBytes;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_fp8_decode_kernel, f.lat_map, f.rope_map, f.q8_map, ctx->qd_map.map, p));
+    cfg.attrs = nullptr;
+    cfg.numAttrs = 0;
+    KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_fp8_decode_kernel, f.lat_map, f.rope_map, p));
     return KAIROS_OK;
 }
 

@@ -121,14 +121,12 @@ struct PlanEntry {
     int cur = 0;
 };
 
-// kairos_fp8_attach: the fp8 pool, its tensor maps and the scratch of the query preparation
+// kairos_fp8_attach: the fp8 pool and its tensor maps
 struct Fp8State {
     bool attached = false;
     void* pool8 = nullptr;
     int32_t num_pages = 0;
-    void* scratch = nullptr;           // q8 [max_decodes][16 KB] | ginv [max_decodes][16] f32
-    int32_t max_decodes = 0;
-    CUtensorMap lat_map, rope_map, q8_map;
+    CUtensorMap lat_map, rope_map;
 };
 
 // kairos_run_schedule: the plans of every step of the last schedule, their device copies and the captured graph
@@ -224,8 +222,7 @@ int launch_project_out(kairos_ctx* ctx, const void* o_lat, const void* w_uv_t, i
 // fp8 latent cache (fp8.cu)
 // tensor map of rank 2 or 3 over bytes (u8) or bf16 elements, SWIZZLE_128B; strides in bytes for dimensions 1..rank-1
 int encode_tiled_map(CUtensorMap* out, bool u8, int rank, const void* ptr, const uint64_t* dims, const uint64_t* strides, const uint32_t* box);
-size_t fp8_scratch_bytes(int32_t max_decodes);
-int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages, void* scratch, size_t scratch_bytes);
+int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages);
 int launch_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                       int32_t start_pos, cudaStream_t stream);
 int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, cudaStream_t stream);

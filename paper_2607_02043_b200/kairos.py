@@ -117,9 +117,7 @@ _lib.kairos_project_out.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp]
 _lib.kairos_project_out.restype = _c.c_int
 _lib.kairos_tune_step.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.kairos_tune_step.restype = _c.c_int
-_lib.kairos_fp8_scratch_bytes.argtypes = [_i32]
-_lib.kairos_fp8_scratch_bytes.restype = _c.c_size_t
-_lib.kairos_fp8_attach.argtypes = [_vp, _vp, _i32, _vp, _c.c_size_t]
+_lib.kairos_fp8_attach.argtypes = [_vp, _vp, _i32]
 _lib.kairos_fp8_attach.restype = _c.c_int
 _lib.kairos_fp8_append.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _i32, _vp]
 _lib.kairos_fp8_append.restype = _c.c_int
@@ -136,7 +134,7 @@ EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
            "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate", "kairos_tune_step",
-           "kairos_fp8_scratch_bytes", "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_decode",
+           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_decode",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -159,10 +157,6 @@ def version() -> str:
 
 
 FP8_PAGE_BYTES = 41216  # KAIROS_FP8_PAGE_BYTES
-
-
-def fp8_scratch_bytes(max_decodes: int) -> int:
-    return int(_lib.kairos_fp8_scratch_bytes(int(max_decodes)))
 
 
 def workspace_bytes(max_decodes: int, max_chunk: int) -> int:
@@ -249,12 +243,11 @@ class Kairos:
         return out_dec, out_chunk, lse_dec, lse_chunk
 
     # -- fp8 latent cache
-    def fp8_attach(self, pool8: torch.Tensor, max_decodes: int) -> None:
-        """pool8: uint8 [num_pages, 41216] on the device.  Allocates the query scratch and keeps both alive."""
+    def fp8_attach(self, pool8: torch.Tensor) -> None:
+        """pool8: uint8 [num_pages, 41216] on the device (kept alive by this object)."""
         assert pool8.dtype == torch.uint8 and pool8.dim() == 2 and pool8.shape[1] == FP8_PAGE_BYTES
         self._pool8 = pool8
-        self._fp8_scratch = torch.empty(fp8_scratch_bytes(max_decodes), dtype=torch.uint8, device=pool8.device)
-        _check(_lib.kairos_fp8_attach(self._h, _dp(pool8), int(pool8.shape[0]), _dp(self._fp8_scratch), int(self._fp8_scratch.numel())))
+        _check(_lib.kairos_fp8_attach(self._h, _dp(pool8), int(pool8.shape[0])))
 
     def fp8_append(self, latent: torch.Tensor, k_rope: torch.Tensor, page_table: torch.Tensor, start_pos: int, stream=None) -> None:
         _check(_lib.kairos_fp8_append(self._h, _dp(latent), _dp(k_rope), int(latent.shape[0]), _dp(page_table),

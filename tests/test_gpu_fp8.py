@@ -29,7 +29,7 @@ class Fp8Run:
         self.ctx = K.Kairos(self.pool16, self.ws, inp.softmax_scale)
         for k, v in (knobs or {}).items():
             self.ctx.debug_set(k, v)
-        self.ctx.fp8_attach(self.pool8, max(inp.n_dec, 1))
+        self.ctx.fp8_attach(self.pool8)
         self.dec_pt = torch.from_numpy(inp.dec_page_tables).cuda()
         self.q_dec = K.bf16_tensor(inp.q_dec)
         self.oracle_requests = list(range(inp.n_dec)) if oracle_requests is None else list(oracle_requests)
@@ -163,7 +163,7 @@ def test_config3_sampled_requests():
     _assert_close(out[idx], lse[idx], ref_out, ref_lse, "configs[3] C=0 sampled")
     assert np.isfinite(out).all()
     info = r.ctx.last_plan_info()
-    assert info["kernels"] >= 3   # query preparation + attention + combine
+    assert info["kernels"] == 2   # attention + combine
 
 
 def test_errors():
@@ -179,10 +179,7 @@ def test_errors():
         ctx.fp8_decode(q, pt, inp.dec_ctx_lens)
     assert e.value.code == -1 and "attach" in str(e.value)
     pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device="cuda")
-    ctx.fp8_attach(pool8, 1)
-    with pytest.raises(K.KairosError) as e:
-        ctx.fp8_decode(q, pt, inp.dec_ctx_lens)   # 2 decodes, scratch sized for 1
-    assert e.value.code == -3
+    ctx.fp8_attach(pool8)
     with pytest.raises(K.KairosError) as e:
         ctx.fp8_append(q[0, 0, :512].reshape(1, 512).contiguous(), q[0, 0, 512:].reshape(1, 64).contiguous(), pt[0], 64 * pt.shape[1])
     assert e.value.code == -1
