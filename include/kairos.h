@@ -454,6 +454,8 @@ int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const in
  *                       untouched: a context can serve both.
  * kairos_fp8_append     as kairos_append_latent (same arguments, same indexing, same errors) but quantises into the attached
  *                       fp8 pool.  BIT-EXACT against the definition above: codes, scales and RoPE bytes.
+ * kairos_fp8_append_decode_tokens  as kairos_append_decode_tokens: request i caches its newest token at positions[i] through row i of
+ *                       page_tables (quantised as above; positions are trusted, device-side only).
  * kairos_fp8_decode     as kairos_mixed_step with chunk_len = 0 over the fp8 pool: n_dec decodes, request i attends its first
  *                       dec_ctx_lens[i] cached tokens through row i of dec_page_tables.  Same planner (a0), split partials,
  *                       LSE combine, plan cache and graph replay as the bf16 step; q is split into its two e4m3 terms inside
@@ -465,6 +467,8 @@ int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const in
 int kairos_fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages);
 int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                       int32_t table_len, int32_t start_pos, void* cuda_stream);
+int kairos_fp8_append_decode_tokens(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                                    int32_t table_stride, const int32_t* positions, void* cuda_stream);
 int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                       int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream);
 

@@ -844,6 +844,18 @@ int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, i
     return launch_fp8_append(ctx, latent, k_rope, n_tokens, page_table, start_pos, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int kairos_fp8_append_decode_tokens(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                                    int32_t table_stride, const int32_t* positions, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!ctx->fp8.attached) return fail(KAIROS_ERR_INVALID_ARG, "no fp8 pool attached (kairos_fp8_attach)");
+    if (n < 0 || table_stride < 1) return fail(KAIROS_ERR_INVALID_ARG, "n < 0 or table_stride < 1");
+    if (n == 0) return KAIROS_OK;
+    if (!latent || !k_rope || !page_tables || !positions) return fail(KAIROS_ERR_INVALID_ARG, "NULL pointer");
+    if (reinterpret_cast<uintptr_t>(latent) % 16 || reinterpret_cast<uintptr_t>(k_rope) % 16)
+        return fail(KAIROS_ERR_INVALID_ARG, "latent / k_rope must be 16-byte aligned");
+    return launch_fp8_append_decode(ctx, latent, k_rope, n, page_tables, table_stride, positions, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                       int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream) {
     if (int rc = check_ctx(ctx)) return rc;

@@ -47,9 +47,12 @@ __device__ __forceinline__ float2 e4m3x2_value(uint32_t c) {
 // ------------------------------------------------------------------------------------------------------------
 // quantising append: one warp per token, lane L owns latent elements [16 L, 16 L + 16)
 // ------------------------------------------------------------------------------------------------------------
+// positions == nullptr: token j of ONE request goes to position start_pos + j through `page_table`; otherwise token j is the newest
+// token of request j and goes to positions[j] through row j of `page_table` (stride table_stride).
 __global__ void __launch_bounds__(256) fp8_append_kernel(uint8_t* __restrict__ pool8, const uint4* __restrict__ latent,
                                                          const uint4* __restrict__ k_rope, const int32_t* __restrict__ page_table,
-                                                         int32_t n_tokens, int32_t start_pos) {
+                                                         int32_t n_tokens, int32_t start_pos, const int32_t* __restrict__ positions,
+                                                         int32_t table_stride) {
     const int lane = threadIdx.x & 31;
     const int j = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (j >= n_tokens) return;
@@ -74,8 +77,9 @@ __global__ void __launch_bounds__(256) fp8_append_kernel(uint8_t* __restrict__ p
         const uint32_t hi = e4m3x2(__fdiv_rn(v[4 * i + 2], s), __fdiv_rn(v[4 * i + 3], s));
         c[i] = lo | (hi << 16);
     }
-    const int32_t pos = start_pos + j;
-    uint8_t* page = pool8 + size_t(__ldg(page_table + pos / kPage)) * kPage8Bytes;
+    const int32_t pos = positions ? __ldg(positions + j) : start_pos + j;
+    const int32_t* row = positions ? page_table + size_t(j) * table_stride : page_table;
+    uint8_t* page = pool8 + size_t(__ldg(row + pos / kPage)) * kPage8Bytes;
     const int slot = pos % kPage;
     *reinterpret_cast<uint4*>(page + slot * kLatent + lane * 16) = make_uint4(c[0], c[1], c[2], c[3]);
     if (lane < 8) *reinterpret_cast<uint4*>(page + kOffRope8 + slot * (kRope * 2) + lane * 16) = __ldg(k_rope + size_t(j) * 8 + lane);
@@ -728,7 +732,15 @@ int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages) {
 int launch_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                       int32_t start_pos, cudaStream_t stream) {
     fp8_append_kernel<<<(n_tokens + 7) / 8, 256, 0, stream>>>(static_cast<uint8_t*>(ctx->fp8.pool8), reinterpret_cast<const uint4*>(latent),
-                                                              reinterpret_cast<const uint4*>(k_rope), page_table, n_tokens, start_pos);
+                                                              reinterpret_cast<const uint4*>(k_rope), page_table, n_tokens, start_pos, nullptr, 0);
+    KAIROS_CUDA_TRY(cudaGetLastError());
+    return KAIROS_OK;
+}
+
+int launch_fp8_append_decode(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                             int32_t table_stride, const int32_t* positions, cudaStream_t stream) {
+    fp8_append_kernel<<<(n + 7) / 8, 256, 0, stream>>>(static_cast<uint8_t*>(ctx->fp8.pool8), reinterpret_cast<const uint4*>(latent),
+                                                       reinterpret_cast<const uint4*>(k_rope), page_tables, n, 0, positions, table_stride);
     KAIROS_CUDA_TRY(cudaGetLastError());
     return KAIROS_OK;
 }

@@ -225,6 +225,8 @@ int encode_tiled_map(CUtensorMap* out, bool u8, int rank, const void* ptr, const
 int fp8_attach(kairos_ctx* ctx, void* pool8, int32_t num_pages);
 int launch_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n_tokens, const int32_t* page_table,
                       int32_t start_pos, cudaStream_t stream);
+int launch_fp8_append_decode(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
+                             int32_t table_stride, const int32_t* positions, cudaStream_t stream);
 int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_items, int32_t n_items, cudaStream_t stream);
 
 // chunk tiles on 2-CTA clusters (attn_pair.cu)

@@ -121,6 +121,8 @@ _lib.kairos_fp8_attach.argtypes = [_vp, _vp, _i32]
 _lib.kairos_fp8_attach.restype = _c.c_int
 _lib.kairos_fp8_append.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _i32, _vp]
 _lib.kairos_fp8_append.restype = _c.c_int
+_lib.kairos_fp8_append_decode_tokens.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp]
+_lib.kairos_fp8_append_decode_tokens.restype = _c.c_int
 _lib.kairos_fp8_decode.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.kairos_fp8_decode.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
@@ -134,7 +136,7 @@ EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
            "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate", "kairos_tune_step",
-           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_decode",
+           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_append_decode_tokens", "kairos_fp8_decode",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -252,6 +254,11 @@ class Kairos:
     def fp8_append(self, latent: torch.Tensor, k_rope: torch.Tensor, page_table: torch.Tensor, start_pos: int, stream=None) -> None:
         _check(_lib.kairos_fp8_append(self._h, _dp(latent), _dp(k_rope), int(latent.shape[0]), _dp(page_table),
                                       int(page_table.numel()), int(start_pos), _stream_ptr(stream)))
+
+    def fp8_append_decode_tokens(self, latent, k_rope, page_tables, positions, stream=None) -> None:
+        n = int(latent.shape[0])
+        _check(_lib.kairos_fp8_append_decode_tokens(self._h, _dp(latent), _dp(k_rope), n, _dp(page_tables),
+                                                    int(page_tables.shape[1]) if n else 1, _dp(positions), _stream_ptr(stream)))
 
     def fp8_decode(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], out_dec=None, lse_dec=None, want_lse: bool = True,
                    stream=None):

@@ -60,10 +60,11 @@ class Fp8Run:
         return F.decode(self.pool8_ref, self.inp.q_dec[idx], self.inp.dec_page_tables[idx], self.inp.dec_ctx_lens[idx], self.inp.softmax_scale)
 
 
-def _assert_close(out, lse, ref_out, ref_lse, what):
+def _assert_close(out, lse, ref_out, ref_lse, what, scale=1.0):
+    """`scale`: the absolute bound is stated for unit-scale latents; a case that scales them passes its largest |reference|"""
     ma, rl = errors(out, ref_out)
     assert np.isfinite(out).all(), what
-    assert ma <= MAX_ABS_TOL and rl <= REL_L2_TOL, f"{what}: max-abs {ma:.3e} rel-L2 {rl:.3e}"
+    assert ma <= MAX_ABS_TOL * max(1.0, scale) and rl <= REL_L2_TOL, f"{what}: max-abs {ma:.3e} rel-L2 {rl:.3e}"
     assert np.abs(lse - ref_lse).max() <= 2e-3, f"{what}: lse {np.abs(lse - ref_lse).max():.3e}"
 
 
@@ -183,3 +184,28 @@ def test_errors():
     with pytest.raises(K.KairosError) as e:
         ctx.fp8_append(q[0, 0, :512].reshape(1, 512).contiguous(), q[0, 0, 512:].reshape(1, 64).contiguous(), pt[0], 64 * pt.shape[1])
     assert e.value.code == -1
+
+
+def test_append_decode_tokens_then_decode_a_growing_batch():
+    """three decode steps: every request caches its newest token (batched fp8 append), then attends one token further"""
+    import torch
+    from paper_2607_02043_b200 import kairos as K
+    lens0 = [63, 64, 127, 500, 1]
+    inp = W.make_inputs("fp8_grow", 16, [L + 3 for L in lens0], 0, 0)   # page tables sized for the growth
+    r = Fp8Run(inp)                                                      # both pools hold every request's first lens0 + 3 tokens
+    rng = np.random.default_rng(8)
+    lens = np.asarray(lens0, np.int32)
+    for step in range(3):
+        lat = W.f32_to_bf16_bits(rng.standard_normal((len(lens), 512)).astype(np.float32) * np.float32(2.0 ** rng.integers(-3, 4)))
+        rope = W.f32_to_bf16_bits(rng.standard_normal((len(lens), 64)).astype(np.float32))
+        pos = torch.from_numpy(lens.copy()).cuda()
+        r.ctx.fp8_append_decode_tokens(K.bf16_tensor(lat), K.bf16_tensor(rope), r.dec_pt, pos)
+        for i in range(len(lens)):
+            F.append(r.pool8_ref, lat[i:i + 1], rope[i:i + 1], inp.dec_page_tables[i], int(lens[i]))
+        lens = lens + 1
+        od, lse = r.ctx.fp8_decode(r.q_dec, r.dec_pt, lens)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(r.pool8.cpu().numpy(), r.pool8_ref)
+        ref_out, ref_lse = F.decode(r.pool8_ref, inp.q_dec, inp.dec_page_tables, lens, inp.softmax_scale)
+        _assert_close(W.bf16_bits_to_f32(K.bf16_bits(od)), lse.cpu().numpy(), ref_out, ref_lse, f"growing batch step {step}",
+                      scale=float(np.abs(ref_out).max()))
