@@ -461,6 +461,13 @@ int kairos_tune_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const in
  *                       LSE combine, plan cache and graph replay as the bf16 step; q is split into its two e4m3 terms inside
  *                       the kernel (no extra launch, no scratch).  Stale slots of a request's last page never reach a result
  *                       (any bit pattern, NaN codes included).
+ * kairos_fp8_mixed_step the mixed step itself over the fp8 pool (same arguments as kairos_mixed_step; the chunk's tokens must already be
+ *                       in the cache: kairos_fp8_append at start_pos = prefix_len).  There is no fp8 chunk-tile kernel: token j of
+ *                       the chunk runs as a one-token request over the chunk's own sequence (n_keys = prefix_len + j + 1) in the same
+ *                       grid as the decodes, its pages kept in L2 (evict-last) for the later tokens.  That serves the chunk sizes
+ *                       the paper deflects with (chi = 128 .. 2048 beside a decode batch); a long chunk over a
+ *                       long prefix re-reads the prefix once per token and belongs on the bf16 path's cluster kernel.  The
+ *                       workspace must cover max_decodes + max_chunk requests: kairos_workspace_bytes(max_decodes + max_chunk, 0).
  * Errors: INVALID_ARG (NULL / misaligned / sizes / no pool attached), WORKSPACE, CUDA.
  */
 #define KAIROS_FP8_PAGE_BYTES 41216
@@ -469,6 +476,10 @@ int kairos_fp8_append(kairos_ctx* ctx, const void* latent, const void* k_rope, i
                       int32_t table_len, int32_t start_pos, void* cuda_stream);
 int kairos_fp8_append_decode_tokens(kairos_ctx* ctx, const void* latent, const void* k_rope, int32_t n, const int32_t* page_tables,
                                     int32_t table_stride, const int32_t* positions, void* cuda_stream);
+int kairos_fp8_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                          const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len, const void* q_chunk,
+                          const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk, float* lse_dec,
+                          float* lse_chunk, void* cuda_stream);
 int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                       int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream);
 

@@ -264,14 +264,27 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
         cache_state = 1;
         e->lens.assign(dec_ctx_lens, dec_ctx_lens + n_dec);
         for (WorkItem& w : e->plan.items)
-            if (w.kind == 0) w.n_keys = dec_ctx_lens[w.q_index];
+            if (w.kind == 0 && w.q_index < n_dec) w.n_keys = dec_ctx_lens[w.q_index];  // (fp8: q_index >= n_dec is a chunk token)
         e->cur ^= 1;
         if (int rc = upload_plan(ctx, *e, e->cur, stream)) return rc;
     } else {
         e = victim;
         for (PlanBuffer& b : e->buf) drop_graph(b);
         e->valid = false;
-        build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, target_ctas, umma_chunk_tile_tokens(), &e->plan, pair_mode, pair_tile_tokens());
+        if (fp8 && chunk_len > 0) {
+            // the fp8 kernel has no chunk tiles: token j of the chunk runs as a one-token request over the chunk's own sequence
+            // (n_keys = P + j + 1), planned with the decodes; its items and combine entries are mapped to the chunk's buffers
+            std::vector<int32_t> all(dec_ctx_lens, dec_ctx_lens + n_dec);
+            for (int32_t j = 0; j < chunk_len; ++j) all.push_back(prefix_len + j + 1);
+            build_plan(all.data(), n_dec + chunk_len, 0, 0, target_ctas, umma_chunk_tile_tokens(), &e->plan, 0, pair_tile_tokens());
+            for (CombineItem& c : e->plan.combines)
+                if (c.q_index >= n_dec) {
+                    c.q_index -= n_dec;
+                    c.kind_stride |= 1;  // output rows of the chunk
+                }
+        } else {
+            build_plan(dec_ctx_lens, n_dec, chunk_len, prefix_len, target_ctas, umma_chunk_tile_tokens(), &e->plan, pair_mode, pair_tile_tokens());
+        }
         const size_t ws_needed = kCounterBytes + size_t(e->plan.n_partial_slots) * kPartialSlotBytes;
         if (ws_needed > ctx->cfg.workspace_bytes)
             return fail(KAIROS_ERR_WORKSPACE, "workspace too small: need " + std::to_string(ws_needed) + " bytes");
@@ -288,7 +301,7 @@ int mixed_step_impl(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int
 
     // ---- q tensor maps (kept while the caller passes the same buffers); everything that can fail on the host happens
     // before the first enqueue on the caller's stream
-    if (n_dec > 0 && !plan.items.empty())
+    if (!fp8 && n_dec > 0 && !plan.items.empty())
         if (int rc = encode_q_map(&ctx->qd_map, q_dec, uint64_t(n_dec) * kHeads, 16)) return rc;
     if (chunk_len > 0 && plan.n_chunk_items > 0)
         if (int rc = encode_q_map(&ctx->qc_map, q_chunk, uint64_t(chunk_len) * kHeads, 64)) return rc;
@@ -854,6 +867,17 @@ int kairos_fp8_append_decode_tokens(kairos_ctx* ctx, const void* latent, const v
     if (reinterpret_cast<uintptr_t>(latent) % 16 || reinterpret_cast<uintptr_t>(k_rope) % 16)
         return fail(KAIROS_ERR_INVALID_ARG, "latent / k_rope must be 16-byte aligned");
     return launch_fp8_append_decode(ctx, latent, k_rope, n, page_tables, table_stride, positions, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int kairos_fp8_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                          const int32_t* dec_ctx_lens, int32_t chunk_len, int32_t prefix_len, const void* q_chunk,
+                          const int32_t* chunk_page_table, int32_t chunk_table_len, void* out_dec, void* out_chunk, float* lse_dec,
+                          float* lse_chunk, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (!ctx->fp8.attached) return fail(KAIROS_ERR_INVALID_ARG, "no fp8 pool attached (kairos_fp8_attach)");
+    return mixed_step_impl(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, chunk_len, prefix_len, q_chunk,
+                           chunk_page_table, chunk_table_len, out_dec, out_chunk, lse_dec, lse_chunk, static_cast<cudaStream_t>(cuda_stream),
+                           /*fp8=*/1);
 }
 
 int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,

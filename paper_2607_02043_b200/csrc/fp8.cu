@@ -157,6 +157,13 @@ struct K8Params {
     int32_t dec_stride;
     const uint8_t* pool8;
     const uint4* q;      // q_dec, bf16 [n_dec][16][576]
+    // kairos_fp8_mixed_step: items with q_index >= n_dec are the chunk's tokens, each run as a one-token request over the chunk's own
+    // sequence (n_keys = P + j + 1): same kernel, the chunk's page table, query and output buffers
+    int32_t n_dec;
+    const int32_t* chunk_pt;
+    const uint4* q_chunk;
+    __nv_bfloat16* out_chunk;
+    float* lse_chunk;
     __nv_bfloat16* out_dec;
     float* lse_dec;
     uint8_t* partials;
@@ -440,7 +447,9 @@ __device__ __forceinline__ void epilogue_item8(Small8* sm, const WorkItem& w, co
         const float mli = __fdividef(1.f, L);
         if (w4 == 0 && lane < kHeads) {
             if (is_final) {
-                if (p.lse_dec) p.lse_dec[size_t(w.q_index) * kHeads + h] = (m + lg2(L)) * kLn2;
+                float* lse = w.q_index < p.n_dec ? p.lse_dec : p.lse_chunk;
+                const int row = w.q_index < p.n_dec ? w.q_index : w.q_index - p.n_dec;
+                if (lse) lse[size_t(row) * kHeads + h] = (m + lg2(L)) * kLn2;
             } else {
                 float* ml = reinterpret_cast<float*>(p.partials + size_t(w.partial_slot) * kPartialSlotBytes + size_t(kHeads) * kLatent * 4);
                 ml[h] = m;
@@ -469,7 +478,8 @@ __device__ __forceinline__ void epilogue_item8(Small8* sm, const WorkItem& w, co
         const uint32_t* r = rr[b4 & 1];
         const int d = b4 * 128 + w4 * 32 + lane;
         if (is_final) {
-            __nv_bfloat16* o = p.out_dec + size_t(w.q_index) * kHeads * kLatent + d;
+            __nv_bfloat16* o = (w.q_index < p.n_dec ? p.out_dec + size_t(w.q_index) * kHeads * kLatent
+                                                    : p.out_chunk + size_t(w.q_index - p.n_dec) * kHeads * kLatent) + d;
 #pragma unroll
             for (int i = 0; i < kHeads; ++i) o[i * kLatent] = __float2bfloat16_rn((__uint_as_float(r[i]) + __uint_as_float(r[kHeads + i])) * linv[i]);
         } else {
@@ -615,7 +625,9 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
             if (idx < 0) break;
             const WorkItem w = load_item8(p.items + idx);
             const int npages = w.page_end - w.page_begin;
-            const int32_t* pt = p.dec_pt + size_t(w.q_index) * p.dec_stride + w.page_begin;
+            const bool is_chunk = w.q_index >= p.n_dec;
+            const int32_t* pt = (is_chunk ? p.chunk_pt : p.dec_pt + size_t(w.q_index) * p.dec_stride) + w.page_begin;
+            const uint64_t policy = is_chunk ? kEvictLast : kEvictFirst;  // the chunk's pages are re-read by every later token of the chunk
             for (int i = 0; i < npages; i += 32) {
                 const int my = (i + lane < npages) ? __ldg(pt + i + lane) : 0;
                 const int cnt = min(32, npages - i);
@@ -628,12 +640,12 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                         mbar_arrive_expect_tx(&sm->kv_full[st][1], 2 * kSlotBytes);
 #pragma unroll
                         for (int b = 0; b < 4; ++b)
-                            tma_load_3d(kv_u32 + st * kStageBytes + b * kSlotBytes, &lat_map, &sm->kv_full[st][b >> 1], b * 128, 0, pid, kEvictFirst);
+                            tma_load_3d(kv_u32 + st * kStageBytes + b * kSlotBytes, &lat_map, &sm->kv_full[st][b >> 1], b * 128, 0, pid, policy);
                         mbar_wait(&sm->rope_empty[g & 1], ((g >> 1) & 1) ^ 1);  // S of page g - 2 retired long before a latent stage frees
                         mbar_arrive_expect_tx(&sm->rope_full[g & 1], kSlotBytes);
-                        tma_load_3d(kv_u32 + kStages * kStageBytes + (g & 1) * kSlotBytes, &rope_map, &sm->rope_full[g & 1], 0, 0, pid, kEvictFirst);
+                        tma_load_3d(kv_u32 + kStages * kStageBytes + (g & 1) * kSlotBytes, &rope_map, &sm->rope_full[g & 1], 0, 0, pid, policy);
                         bulk_load(smem_u32(sm->scales[st]), p.pool8 + size_t(pid) * kPage8Bytes + kOffScale8, kPage * 4, &sm->kv_full[st][0],
-                                  kEvictFirst);
+                                  policy);
                     }
                 }
             }
@@ -671,7 +683,9 @@ kairos_fp8_decode_kernel(const __grid_constant__ CUtensorMap lat_map, const __gr
                 w = load_item8(p.items + idx);
                 const int qb = int(it & 1);
                 mbar_wait(&sm->q_empty[qb], ((it >> 1) & 1) ^ 1);
-                prepare_q8(sm, base + kOffQ + qb * kQBufBytes, qb, p.q + size_t(w.q_index) * kHeads * (kTokenBytes / 16), warp - kEpiWarp, lane);
+                const uint4* qrows = w.q_index < p.n_dec ? p.q + size_t(w.q_index) * kHeads * (kTokenBytes / 16)
+                                                         : p.q_chunk + size_t(w.q_index - p.n_dec) * kHeads * (kTokenBytes / 16);
+                prepare_q8(sm, base + kOffQ + qb * kQBufBytes, qb, qrows, warp - kEpiWarp, lane);
             }
             if (it > 0) epilogue_item8(sm, prev, p, tmem, warp & 3, lane, it - 1);
             if (idx < 0) break;
@@ -755,6 +769,11 @@ int launch_fp8_decode(kairos_ctx* ctx, const StepArgs& a, const WorkItem* dev_it
     p.dec_stride = a.dec_table_stride;
     p.pool8 = static_cast<const uint8_t*>(f.pool8);
     p.q = reinterpret_cast<const uint4*>(a.q_dec);
+    p.n_dec = a.n_dec;
+    p.chunk_pt = a.chunk_page_table;
+    p.q_chunk = reinterpret_cast<const uint4*>(a.q_chunk);
+    p.out_chunk = reinterpret_cast<__nv_bfloat16*>(a.out_chunk);
+    p.lse_chunk = a.lse_chunk;
     p.out_dec = reinterpret_cast<__nv_bfloat16*>(a.out_dec);
     p.lse_dec = a.lse_dec;
     p.partials = reinterpret_cast<uint8_t*>(ctx->cfg.workspace) + 256;

@@ -123,6 +123,8 @@ _lib.kairos_fp8_append.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _i32, _vp]
 _lib.kairos_fp8_append.restype = _c.c_int
 _lib.kairos_fp8_append_decode_tokens.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, _vp, _vp]
 _lib.kairos_fp8_append_decode_tokens.restype = _c.c_int
+_lib.kairos_fp8_mixed_step.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp]
+_lib.kairos_fp8_mixed_step.restype = _c.c_int
 _lib.kairos_fp8_decode.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.kairos_fp8_decode.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
@@ -136,7 +138,7 @@ EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
            "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate", "kairos_tune_step",
-           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_append_decode_tokens", "kairos_fp8_decode",
+           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_append_decode_tokens", "kairos_fp8_mixed_step", "kairos_fp8_decode",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -259,6 +261,26 @@ class Kairos:
         n = int(latent.shape[0])
         _check(_lib.kairos_fp8_append_decode_tokens(self._h, _dp(latent), _dp(k_rope), n, _dp(page_tables),
                                                     int(page_tables.shape[1]) if n else 1, _dp(positions), _stream_ptr(stream)))
+
+    def fp8_mixed_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
+                       prefix_len: int, out_dec=None, out_chunk=None, lse_dec=None, lse_chunk=None, want_lse: bool = True, stream=None):
+        """kairos_fp8_mixed_step: as mixed_step, over the attached fp8 pool."""
+        lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        B, C = int(lens.shape[0]), int(chunk_len)
+        dev = self._pool8.device
+        if out_dec is None:
+            out_dec = torch.empty((B, 16, 512), dtype=torch.bfloat16, device=dev)
+        if out_chunk is None:
+            out_chunk = torch.empty((C, 16, 512), dtype=torch.bfloat16, device=dev)
+        if want_lse and lse_dec is None:
+            lse_dec = torch.empty((B, 16), dtype=torch.float32, device=dev)
+        if want_lse and lse_chunk is None:
+            lse_chunk = torch.empty((C, 16), dtype=torch.float32, device=dev)
+        _check(_lib.kairos_fp8_mixed_step(self._h, B, _dp(q_dec), _dp(dec_page_tables), int(dec_page_tables.shape[1]) if B else 1,
+                                          lens.ctypes.data_as(_vp), C, int(prefix_len), _dp(q_chunk), _dp(chunk_page_table),
+                                          int(chunk_page_table.numel()) if C else 0, _dp(out_dec), _dp(out_chunk), _dp(lse_dec),
+                                          _dp(lse_chunk), _stream_ptr(stream)))
+        return out_dec, out_chunk, lse_dec, lse_chunk
 
     def fp8_decode(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], out_dec=None, lse_dec=None, want_lse: bool = True,
                    stream=None):

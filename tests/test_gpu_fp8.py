@@ -209,3 +209,54 @@ def test_append_decode_tokens_then_decode_a_growing_batch():
         ref_out, ref_lse = F.decode(r.pool8_ref, inp.q_dec, inp.dec_page_tables, lens, inp.softmax_scale)
         _assert_close(W.bf16_bits_to_f32(K.bf16_bits(od)), lse.cpu().numpy(), ref_out, ref_lse, f"growing batch step {step}",
                       scale=float(np.abs(ref_out).max()))
+
+
+def _mixed_case(inp, r):
+    """Cache the chunk's sequence (prefix from the synthetic pool, then the chunk's own tokens) on both sides; returns the chunk rows'
+    reference inputs for F.decode: every chunk token is a one-token request over the chunk's page table (n_keys = P + j + 1)."""
+    import torch
+    K = r.K
+    C, P = inp.chunk_len, inp.prefix_len
+    cpt = torch.from_numpy(inp.chunk_page_table).cuda()
+    if P:
+        tok = O.gather(inp.pool, inp.chunk_page_table, P)
+        lat, rope = np.ascontiguousarray(tok[:, :512]), np.ascontiguousarray(tok[:, 512:])
+        r.ctx.fp8_append(K.bf16_tensor(lat), K.bf16_tensor(rope), cpt, 0)
+        F.append(r.pool8_ref, lat, rope, inp.chunk_page_table, 0)
+    r.ctx.fp8_append(K.bf16_tensor(inp.chunk_latent), K.bf16_tensor(inp.chunk_k_rope), cpt, P)
+    F.append(r.pool8_ref, inp.chunk_latent, inp.chunk_k_rope, inp.chunk_page_table, P)
+    rows_pt = np.tile(inp.chunk_page_table[None, :], (C, 1))
+    rows_len = (P + 1 + np.arange(C)).astype(np.int32)
+    return cpt, rows_pt, rows_len
+
+
+@pytest.mark.parametrize("lens,C,P", [([64, 128, 200, 256], 64, 128), ([300, 70], 100, 0), ([], 130, 61), ([1000, 2500, 65], 257, 700)])
+def test_mixed_step_over_the_fp8_cache(lens, C, P):
+    """kairos_fp8_mixed_step: decodes + a causal chunk, every row against the float64 definition over the dequantised cache"""
+    inp = W.make_inputs("fp8_mixed", 17, lens, C, P)
+    r = Fp8Run(inp)
+    cpt, rows_pt, rows_len = _mixed_case(inp, r)
+    q_chunk = r.K.bf16_tensor(inp.q_chunk)
+    r.ws = r.torch.empty(r.K.workspace_bytes(inp.n_dec + C, 0), dtype=r.torch.uint8, device="cuda")
+    ctx = r.K.Kairos(r.pool16, r.ws, inp.softmax_scale)
+    ctx.fp8_attach(r.pool8)
+    q_dec = r.q_dec if inp.n_dec else r.torch.empty((0, 16, 576), dtype=r.torch.bfloat16, device="cuda")
+    dpt = r.dec_pt if inp.n_dec else r.torch.zeros((1, 1), dtype=r.torch.int32, device="cuda")
+    outs = None
+    for rep in range(3):   # plan miss, exact hit, graph replay: the same bits
+        od, oc, ld, lc = ctx.fp8_mixed_step(q_dec, dpt, inp.dec_ctx_lens, q_chunk, cpt, C, P) if outs is None else \
+            ctx.fp8_mixed_step(q_dec, dpt, inp.dec_ctx_lens, q_chunk, cpt, C, P, out_dec=outs[0], out_chunk=outs[1], lse_dec=outs[2], lse_chunk=outs[3])
+        r.torch.cuda.synchronize()
+        cur = [r.K.bf16_bits(od), r.K.bf16_bits(oc), ld.cpu().numpy(), lc.cpu().numpy()]
+        if outs is not None:
+            for a, b in zip(cur, first):
+                np.testing.assert_array_equal(a, b)
+        else:
+            first = cur
+        outs = (od, oc, ld, lc)
+    np.testing.assert_array_equal(r.pool8.cpu().numpy(), r.pool8_ref)
+    ref_c, ref_lc = F.decode(r.pool8_ref, inp.q_chunk, rows_pt, rows_len, inp.softmax_scale)
+    _assert_close(W.bf16_bits_to_f32(first[1]), first[3], ref_c, ref_lc, f"chunk rows C={C} P={P}")
+    if inp.n_dec:
+        ref_d, ref_ld = F.decode(r.pool8_ref, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.softmax_scale)
+        _assert_close(W.bf16_bits_to_f32(first[0]), first[2], ref_d, ref_ld, f"decode rows beside C={C}")
