@@ -320,43 +320,62 @@ FP8_TOKEN_BYTES = 512 + 4 + 128  # e4m3 latent codes + one f32 scale + bf16 RoPE
 
 
 def fp8_decode_leg(K, torch, dev, peaks, steps, warmup):
-    """the decodes of configs[3] (256 x 2,048 cached tokens, C = 0) over the fp8 latent cache.  The cache is
-    built on the device by kairos_fp8_append from the same synthetic tokens; one step reads 338 MiB (> 2x L2: no flush)."""
-    inp = W.make_config(3, chunk_len=0)
-    pool16 = K.bf16_tensor(inp.pool)
-    ws = torch.empty(K.workspace_bytes(inp.n_dec, 1), dtype=torch.uint8, device=dev)
-    ctx = K.Kairos(pool16, ws, inp.softmax_scale)
-    pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device=dev)
-    ctx.fp8_attach(pool8)
-    dpt = torch.from_numpy(inp.dec_page_tables).to(dev)
-    for i in range(inp.n_dec):
-        L = int(inp.dec_ctx_lens[i])
-        tok = ctx.gather_latent(dpt[i], L)
-        ctx.fp8_append(tok[:, :512].contiguous(), tok[:, 512:].contiguous(), dpt[i], 0)
-    qd = K.bf16_tensor(inp.q_dec)
-    od = torch.empty((inp.n_dec, 16, 512), dtype=torch.bfloat16, device=dev)
-    for _ in range(max(warmup, 3)):
-        ctx.fp8_decode(qd, dpt, inp.dec_ctx_lens, out_dec=od, want_lse=False)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n = max(steps, 200)
-    e0.record()
-    for _ in range(n):
-        ctx.fp8_decode(qd, dpt, inp.dec_ctx_lens, out_dec=od, want_lse=False)
-    e1.record()
-    torch.cuda.synchronize()
-    us = e0.elapsed_time(e1) * 1e3 / n
-    tokens = int(inp.dec_ctx_lens.astype(np.int64).sum())
-    alg = tokens * FP8_TOKEN_BYTES + inp.n_dec * (W.Q_BYTES + W.OUT_BYTES)
-    info = ctx.last_plan_info()
-    return {"workload": "configs[3] C=0 decodes over the fp8 latent cache (kairos_fp8_decode)", "B": inp.n_dec, "cached_tokens": tokens,
-            "step_us": us, "steps": n, "algorithmic_bytes": alg, "bytes_per_token": FP8_TOKEN_BYTES,
-            "roofline": {"bound": "hbm", "achieved": alg / (us * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                         "frac": alg / (us * 1e-6) / 1e9 / peaks["hbm_gbs"], "roofline_us": alg / peaks["hbm_gbs"] / 1e3,
-                         "note": "whole step (query split + attention + combine) over the HBM time of its algorithmic bytes"},
-            "traffic": measured_traffic("fp8_config3_C0")[0],
-            "kernels_per_step": info["kernels"], "graph": info["graph"], "dtype": "e4m3 cache, bf16 q / out, f32 accumulation",
-            "l2": "one step reads 338 MiB > 2x L2: no flush needed"}
+    """configs[3] over the fp8 latent cache -- the decodes alone (C = 0, kairos_fp8_decode) and, under "mixed",
+    the step with a chunk of 256 / 512 tokens (kairos_fp8_append of the chunk + kairos_fp8_mixed_step).  The cache is built on the
+    device by kairos_fp8_append from the same synthetic tokens; one step reads >= 338 MiB (> 2x L2: no flush)."""
+    def one(C):
+        inp = W.make_config(3, chunk_len=C)
+        pool16 = K.bf16_tensor(inp.pool)
+        ws = torch.empty(K.workspace_bytes(inp.n_dec + C, 0), dtype=torch.uint8, device=dev)
+        ctx = K.Kairos(pool16, ws, inp.softmax_scale)
+        pool8 = torch.zeros((inp.num_pages, K.FP8_PAGE_BYTES), dtype=torch.uint8, device=dev)
+        ctx.fp8_attach(pool8)
+        dpt = torch.from_numpy(inp.dec_page_tables).to(dev)
+        for i in range(inp.n_dec):
+            tok = ctx.gather_latent(dpt[i], int(inp.dec_ctx_lens[i]))
+            ctx.fp8_append(tok[:, :512].contiguous(), tok[:, 512:].contiguous(), dpt[i], 0)
+        qd = K.bf16_tensor(inp.q_dec)
+        od = torch.empty((inp.n_dec, 16, 512), dtype=torch.bfloat16, device=dev)
+        if C:
+            cpt = torch.from_numpy(inp.chunk_page_table).to(dev)
+            lat, rope, qc = K.bf16_tensor(inp.chunk_latent), K.bf16_tensor(inp.chunk_k_rope), K.bf16_tensor(inp.q_chunk)
+            oc = torch.empty((C, 16, 512), dtype=torch.bfloat16, device=dev)
+
+            def step():
+                ctx.fp8_append(lat, rope, cpt, inp.prefix_len)
+                ctx.fp8_mixed_step(qd, dpt, inp.dec_ctx_lens, qc, cpt, C, inp.prefix_len, out_dec=od, out_chunk=oc, want_lse=False)
+        else:
+            def step():
+                ctx.fp8_decode(qd, dpt, inp.dec_ctx_lens, out_dec=od, want_lse=False)
+        for _ in range(max(warmup, 3)):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = max(steps, 200)
+        e0.record()
+        for _ in range(n):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / n
+        tokens = int(inp.dec_ctx_lens.astype(np.int64).sum())
+        alg = (tokens + (inp.prefix_len + C if C else 0)) * FP8_TOKEN_BYTES + (inp.n_dec + C) * (W.Q_BYTES + W.OUT_BYTES)
+        roof_us = max(alg / peaks["hbm_gbs"] / 1e3, inp.algorithmic_flops() / peaks["bf16_tflops"] / 1e6)
+        info = ctx.last_plan_info()
+        return {"workload": f"configs[3] C={C} over the fp8 latent cache", "B": inp.n_dec, "C": C, "P": inp.prefix_len, "cached_tokens": tokens,
+                "step_us": us, "steps": n, "algorithmic_bytes": alg, "bytes_per_token": FP8_TOKEN_BYTES,
+                "roofline": {"bound": "hbm", "achieved": alg / (us * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": roof_us / us, "roofline_us": roof_us,
+                             "note": "whole step over max(HBM time of its algorithmic bytes, tensor time of its FLOPs at the bf16 peak)"},
+                "kernels_per_step": info["kernels"] + (1 if C else 0), "graph": info["graph"], "work_items": info["work_items"]}
+
+    head = one(0)
+    head["workload"] = "configs[3] C=0 decodes over the fp8 latent cache (kairos_fp8_decode)"
+    head["traffic"] = measured_traffic("fp8_config3_C0")[0]
+    head["dtype"] = "e4m3 cache, bf16 q / out, f32 accumulation"
+    head["l2"] = "one step reads 338 MiB > 2x L2: no flush needed"
+    head["mixed"] = [one(256), one(512)]
+    return head
 
 
 def main():
