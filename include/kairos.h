@@ -484,6 +484,27 @@ int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
                       int32_t dec_table_stride, const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream);
 
 /*
+ * Decode attention for callers that MAY NOT ALLOCATE (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc).  kairos_mixed_step grows pinned and device plan buffers on demand and takes its split-KV scratch from the caller's
+ * workspace; this entry point does neither: the queue counters, the work list, the combine list and the fp32 split partials live in
+ * ONE fixed array of device memory that is part of the library image (`static __device__`, about 9.3 MiB; every GPU that loads
+ * libkairos.so holds it until the process exits), and the work list is written by a small kernel on the device.  The call makes
+ * three launches (plan, decode splits, LSE combine) and no cudaMalloc / cudaFree / allocating library call.
+ *   Same operation and argument meaning as kairos_mixed_step with chunk_len = 0: request i attends its first dec_ctx_lens[i] cached
+ *   tokens of the bf16 pool through row i of dec_page_tables; out_dec bf16 [n_dec][16][512], lse_dec fp32 [n_dec][16] or NULL.
+ *   Results agree with kairos_mixed_step within the attention tolerance (the KV split points differ, so not bit for bit).
+ * Limits: n_dec <= KAIROS_STATIC_MAX_DECODES (128); any context length the page tables cover.  More decodes: KAIROS_ERR_WORKSPACE
+ * with a message that names the limit -- use kairos_mixed_step.
+ * Sharing: every call on a device, from every context, uses the SAME array, and the array keeps the last call's contents.  Each
+ * call clears the counters and rewrites both lists before it reads them, so back-to-back calls on one stream are safe; calls that
+ * overlap on the GPU (two streams, two contexts, two threads) race and corrupt each other -- serialise them.
+ * Asynchronous on `cuda_stream`; dec_ctx_lens (HOST) is read before the call returns.  Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+#define KAIROS_STATIC_MAX_DECODES 128
+int kairos_decode_static(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                         const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream);
+
+/*
  * TEST-ONLY knobs (parity tests force every launch order and code path through them; sweeps under profiles/ use them;
  * a deployment never calls this).  Takes effect from the next kairos_mixed_step.
  *   "pairs"       -1 planner decides (default); 0 never use the cluster kernel; n > 0 decode grid first beside n clusters;

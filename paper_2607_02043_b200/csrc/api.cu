@@ -888,6 +888,28 @@ int kairos_fp8_decode(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
                            nullptr, lse_dec, nullptr, static_cast<cudaStream_t>(cuda_stream), /*fp8=*/1);
 }
 
+// ---- decode attention for callers that may not allocate (scratch = a fixed __device__ array in attn_umma.cu) ------------------
+int kairos_decode_static(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                         const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, void* cuda_stream) {
+    if (int rc = check_ctx(ctx)) return rc;
+    if (n_dec < 0) return fail(KAIROS_ERR_INVALID_ARG, "negative size");
+    if (n_dec == 0) return KAIROS_OK;
+    if (!q_dec || !dec_page_tables || !dec_ctx_lens || !out_dec) return fail(KAIROS_ERR_INVALID_ARG, "NULL decode argument");
+    if (dec_table_stride < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_table_stride < 1");
+    if (reinterpret_cast<uintptr_t>(q_dec) % 16 || reinterpret_cast<uintptr_t>(out_dec) % 16 || reinterpret_cast<uintptr_t>(lse_dec) % 4)
+        return fail(KAIROS_ERR_INVALID_ARG, "q_dec / out_dec must be 16-byte aligned (lse_dec: 4)");
+    if (n_dec > KAIROS_STATIC_MAX_DECODES)
+        return fail(KAIROS_ERR_WORKSPACE, "kairos_decode_static takes at most " + std::to_string(KAIROS_STATIC_MAX_DECODES) +
+                                              " decodes per call (got " + std::to_string(n_dec) + "): its scratch is a fixed array");
+    for (int32_t i = 0; i < n_dec; ++i) {
+        if (dec_ctx_lens[i] < 1) return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens[" + std::to_string(i) + "] < 1");
+        if (int64_t(dec_ctx_lens[i]) > int64_t(dec_table_stride) * kPage)
+            return fail(KAIROS_ERR_INVALID_ARG, "dec_ctx_lens[" + std::to_string(i) + "] beyond its page table");
+    }
+    return launch_decode_static(ctx, n_dec, q_dec, dec_page_tables, dec_table_stride, dec_ctx_lens, out_dec, lse_dec,
+                                static_cast<cudaStream_t>(cuda_stream));
+}
+
 int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                            int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len,
                            int32_t prefix_len, const void* q_chunk, const void* chunk_latent, const void* chunk_k_rope,

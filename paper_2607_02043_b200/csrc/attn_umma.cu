@@ -753,6 +753,75 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
 
+// ------------------------------------------------------------------------------------------------------------
+// kairos_decode_static: decode attention with NO allocation anywhere (include/kairos.h).  Everything the split-KV decode needs
+// beyond the caller's inputs and outputs -- the work-queue counters, the work list, the combine list and the fp32 split partials --
+// lives in this file-scope array, which every GPU that loads the library holds until the process exits (about 9.3 MiB).
+// In HOST code the name `g_static_scratch` is a host-side stand-in, not a device address: umma_init asks cudaGetSymbolAddress for
+// the real one, once per device with that device current, and the launches below are given that pointer.  Device code may name
+// the array directly (static_plan_kernel does).  Every call on a device shares the array and it keeps the last call's contents:
+// the plan kernel clears the counters and rewrites both lists at the start of every call; calls that overlap on the GPU race.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kStaticMaxDecodes = KAIROS_STATIC_MAX_DECODES;  // 128
+constexpr int kStaticTargetPieces = 148;                       // a request longer than total_pages / 148 (min 4 pages) is split
+constexpr int kStaticMaxSlots = 2 * kStaticTargetPieces;       // split pieces <= total/per + #split requests <= 2 * 148
+constexpr int kStaticMaxItems = kStaticMaxDecodes + kStaticMaxSlots;
+constexpr size_t kStaticOffItems = 256;                        // [0, 256): queue counters
+constexpr size_t kStaticOffCombines = kStaticOffItems + size_t(kStaticMaxItems) * sizeof(WorkItem);
+constexpr size_t kStaticOffPartials = (kStaticOffCombines + size_t(kStaticMaxDecodes) * sizeof(CombineItem) + 255) / 256 * 256;
+constexpr size_t kStaticScratchBytes = kStaticOffPartials + size_t(kStaticMaxSlots) * kPartialSlotBytes;
+static __device__ __align__(256) uint8_t g_static_scratch[kStaticScratchBytes];
+uint8_t* g_static_ptr[64] = {};  // device address of g_static_scratch per device ordinal (filled by umma_init)
+
+struct StaticLens {
+    int32_t v[kStaticMaxDecodes];
+};
+
+// pages per piece for a step with `total_pages` pages in all: the ONE rule both the host (grid sizes) and the device (lists) apply
+__host__ __device__ inline int32_t static_piece_pages(int64_t total_pages) {
+    const int64_t per = (total_pages + kStaticTargetPieces - 1) / kStaticTargetPieces;
+    return int32_t(per < 4 ? 4 : per);
+}
+
+// One block: request i = thread i.  Clears the counters, writes the work list (request order, pieces of `per` pages) and the combine
+// list (one entry per request that was split) into g_static_scratch.
+__global__ void __launch_bounds__(kStaticMaxDecodes) static_plan_kernel(const StaticLens lens, int32_t n_dec, int32_t per) {
+    __shared__ int32_t s_item0[kStaticMaxDecodes + 1], s_slot0[kStaticMaxDecodes + 1], s_comb0[kStaticMaxDecodes + 1];
+    const int i = threadIdx.x;
+    if (i < 64) reinterpret_cast<int32_t*>(g_static_scratch)[i] = 0;  // queue counters: must start at zero
+    const int32_t pages = i < n_dec ? (lens.v[i] + kPage - 1) / kPage : 0;
+    const int32_t n_splits = i < n_dec ? max(1, (pages + per - 1) / per) : 0;
+    s_item0[i + 1] = n_splits;
+    s_slot0[i + 1] = n_splits > 1 ? n_splits : 0;
+    s_comb0[i + 1] = n_splits > 1 ? 1 : 0;
+    __syncthreads();
+    if (i == 0) {
+        s_item0[0] = s_slot0[0] = s_comb0[0] = 0;
+        for (int k = 1; k <= n_dec; ++k) {
+            s_item0[k] += s_item0[k - 1];
+            s_slot0[k] += s_slot0[k - 1];
+            s_comb0[k] += s_comb0[k - 1];
+        }
+    }
+    __syncthreads();
+    if (i >= n_dec) return;
+    WorkItem* items = reinterpret_cast<WorkItem*>(g_static_scratch + kStaticOffItems);
+    CombineItem* combines = reinterpret_cast<CombineItem*>(g_static_scratch + kStaticOffCombines);
+    for (int32_t sp = 0; sp < n_splits; ++sp) {
+        WorkItem w;
+        w.kind = 0;
+        w.q_index = i;
+        w.page_begin = sp * per;
+        w.page_end = min(pages, (sp + 1) * per);
+        w.n_keys = lens.v[i];
+        w.n_q = 1;
+        w.partial_slot = n_splits > 1 ? s_slot0[i] + sp : -1;
+        w.cost = 0;
+        items[s_item0[i] + sp] = w;
+    }
+    if (n_splits > 1) combines[s_comb0[i]] = CombineItem{i, s_slot0[i], n_splits, 0 /*decode*/ | (1 << 8) /*slot stride 1*/};
+}
+
 }  // namespace
 
 int umma_chunk_tile_tokens() { return kChunkTileTokens; }
@@ -824,6 +893,14 @@ int umma_init(kairos_ctx* ctx) {
     KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<false>::kSmemBytes));
     KAIROS_CUDA_TRY(cudaFuncSetAttribute(kairos_mixed_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<true>::kSmemBytes));
     KAIROS_CUDA_TRY(cudaMemset(ctx->cfg.workspace, 0, 256));  // work-queue counters
+    // kairos_decode_static: the device address of the file-scope scratch, once per device, with that device current (kairos_create
+    // has made it so).  The host-side name of a __device__ array must never be handed to a kernel.
+    const int dev = ctx->cfg.device;
+    if (dev >= 0 && dev < 64 && !g_static_ptr[dev]) {
+        void* ptr = nullptr;
+        KAIROS_CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_scratch));
+        g_static_ptr[dev] = static_cast<uint8_t*>(ptr);
+    }
     return KAIROS_OK;
 }
 
@@ -903,6 +980,84 @@ int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_co
         // with two attention kernels in flight the second one waits for the first before it exits, so following it is enough
         cfg.numAttrs = 1;
         KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, combine_kernel, dev_combines, partials, out_dec, out_chunk, lse_dec, lse_chunk));
+    }
+    return KAIROS_OK;
+}
+
+// kairos_decode_static (include/kairos.h): plan on the device, decode splits, LSE combine -- three launches, no allocation.
+int launch_decode_static(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                         const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, cudaStream_t stream) {
+    const int dev = ctx->cfg.device;
+    uint8_t* scratch = (dev >= 0 && dev < 64) ? g_static_ptr[dev] : nullptr;
+    if (!scratch) return fail(KAIROS_ERR_CUDA, "static scratch has no device address on this device (kairos_create looks it up)");
+    if (n_dec > kStaticMaxDecodes)
+        return fail(KAIROS_ERR_WORKSPACE, "kairos_decode_static takes at most " + std::to_string(kStaticMaxDecodes) + " decodes per call (got " +
+                                              std::to_string(n_dec) + "): its scratch is a fixed array");
+    // the same arithmetic as static_plan_kernel, for the grid sizes only
+    StaticLens lens{};
+    int64_t total_pages = 0;
+    for (int32_t i = 0; i < n_dec; ++i) {
+        lens.v[i] = dec_ctx_lens[i];
+        total_pages += (dec_ctx_lens[i] + kPage - 1) / kPage;
+    }
+    const int32_t per = static_piece_pages(total_pages);
+    int32_t n_items = 0, n_slots = 0, n_combines = 0;
+    for (int32_t i = 0; i < n_dec; ++i) {
+        const int32_t pages = (dec_ctx_lens[i] + kPage - 1) / kPage;
+        const int32_t n_splits = std::max(1, (pages + per - 1) / per);
+        n_items += n_splits;
+        if (n_splits > 1) {
+            n_slots += n_splits;
+            ++n_combines;
+        }
+    }
+    if (n_items > kStaticMaxItems || n_slots > kStaticMaxSlots)
+        return fail(KAIROS_ERR_WORKSPACE, "kairos_decode_static: the step needs more split pieces than its fixed scratch holds");
+    if (int rc = encode_q_map(&ctx->qs_map, q_dec, uint64_t(n_dec) * kHeads, 16)) return rc;
+
+    static_plan_kernel<<<1, kStaticMaxDecodes, 0, stream>>>(lens, n_dec, per);
+    KAIROS_CUDA_TRY(cudaGetLastError());
+
+    KParams p;
+    p.items = reinterpret_cast<const WorkItem*>(scratch + kStaticOffItems);
+    p.n_items = n_items;
+    p.counters = reinterpret_cast<int32_t*>(scratch);
+    p.dec_pt = dec_page_tables;
+    p.dec_stride = dec_table_stride;
+    p.chunk_pt = nullptr;
+    p.out_dec = reinterpret_cast<__nv_bfloat16*>(out_dec);
+    p.out_chunk = nullptr;
+    p.lse_dec = lse_dec;
+    p.lse_chunk = nullptr;
+    p.partials = scratch + kStaticOffPartials;
+    p.scale_log2 = ctx->cfg.softmax_scale * 1.4426950408889634f;
+    p.static_first = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(unsigned(std::max(1, std::min(n_items, umma_resident_ctas(ctx)))), 1, 1);
+    cfg.blockDim = dim3(kThreads, 1, 1);
+    cfg.dynamicSmemBytes = Geo<true>::kSmemBytes;
+    cfg.stream = stream;
+    cfg.attrs = nullptr;
+    cfg.numAttrs = 0;
+    // qc_map is a placeholder (the decode-only instantiation never reads it)
+    KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kairos_mixed_kernel<true>, ctx->pool_map2, ctx->pool_map1, ctx->qs_map.map, ctx->pool_map, p));
+    if (n_combines > 0) {
+        const CombineItem* dev_combines = reinterpret_cast<const CombineItem*>(scratch + kStaticOffCombines);
+        const uint8_t* partials = scratch + kStaticOffPartials;
+        __nv_bfloat16* od = reinterpret_cast<__nv_bfloat16*>(out_dec);
+        __nv_bfloat16* oc = nullptr;
+        float* lc = nullptr;
+        cudaLaunchConfig_t cc{};
+        cc.gridDim = dim3(unsigned(n_combines), kCombineSlices, 1);
+        cc.blockDim = dim3(kCombineThreads, 1, 1);
+        cc.dynamicSmemBytes = 0;
+        cc.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cc.attrs = attr;
+        cc.numAttrs = 1;
+        KAIROS_CUDA_TRY(cudaLaunchKernelEx(&cc, combine_kernel, dev_combines, partials, od, oc, lse_dec, lc));
     }
     return KAIROS_OK;
 }

@@ -164,6 +164,7 @@ struct kairos_ctx {
     CUtensorMap pool_map_c;       // a group of 64-dim chunks of a page: K ring of the pair kernel's S-CTA
     CUtensorMap pool_map_v;       // latent part of a page (box of 8 chunks): V operand of the pair kernel
     kairos::QMapCache proj_a[2], proj_b[2];    // operand maps of kairos_absorb_q [0] and kairos_project_out [1]
+    kairos::QMapCache qs_map;                  // decode q of kairos_decode_static (its own cache: the other paths' maps stay as they are)
     kairos::QMapCache qd_map, qc_map, qp_map;  // decode q (box 16 rows), chunk q for gen-1 tiles (64 rows), for the pair kernel (128 rows)
     cudaStream_t copy_stream = nullptr;   // plan H2D copies run here, beside whatever precedes the step on the caller's stream
     cudaStream_t capture_stream = nullptr;  // the step's launches are captured here when a plan is replayed as a CUDA graph
@@ -212,6 +213,8 @@ int encode_2d_map(QMapCache* cache, const void* ptr, uint64_t inner, uint64_t ro
                   uint32_t box_rows);
 int launch_attn_umma(kairos_ctx* ctx, const Plan& plan, const StepArgs& a, const WorkItem* dev_items, int32_t n_items,
                      cudaStream_t stream, int max_ctas, bool as_clusters, bool pdl);
+int launch_decode_static(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables, int32_t dec_table_stride,
+                         const int32_t* dec_ctx_lens, void* out_dec, float* lse_dec, cudaStream_t stream);
 int launch_combine(kairos_ctx* ctx, const StepArgs& a, const CombineItem* dev_combines, int32_t n_combines, cudaStream_t stream);
 int umma_init(kairos_ctx* ctx);  // builds tensor maps, sets kernel attributes
 

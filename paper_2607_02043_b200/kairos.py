@@ -127,6 +127,8 @@ _lib.kairos_fp8_mixed_step.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _i32, _i3
 _lib.kairos_fp8_mixed_step.restype = _c.c_int
 _lib.kairos_fp8_decode.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.kairos_fp8_decode.restype = _c.c_int
+_lib.kairos_decode_static.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp]
+_lib.kairos_decode_static.restype = _c.c_int
 _lib.kairos_debug_set.argtypes = [_vp, _c.c_char_p, _i32]
 _lib.kairos_debug_set.restype = _c.c_int
 _lib.kairos_last_error.argtypes = []
@@ -138,7 +140,7 @@ EXPORTS = ["kairos_workspace_bytes", "kairos_create", "kairos_destroy", "kairos_
            "kairos_append_decode_tokens", "kairos_gather_latent", "kairos_mixed_step", "kairos_mixed_step_host",
            "kairos_step_latency_table", "kairos_plan_dump", "kairos_last_plan_info", "kairos_profile_enable", "kairos_profile_read", "kairos_debug_set",
            "kairos_fit_latency_model", "kairos_predict_step", "kairos_decide", "kairos_run_schedule", "kairos_absorb_q", "kairos_project_out", "kairos_simulate", "kairos_tune_step",
-           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_append_decode_tokens", "kairos_fp8_mixed_step", "kairos_fp8_decode",
+           "kairos_fp8_attach", "kairos_fp8_append", "kairos_fp8_append_decode_tokens", "kairos_fp8_mixed_step", "kairos_decode_static", "kairos_fp8_decode",
            "kairos_last_error", "kairos_version"]
 
 STATUS = {0: "KAIROS_OK", -1: "KAIROS_ERR_INVALID_ARG", -2: "KAIROS_ERR_UNSUPPORTED", -3: "KAIROS_ERR_WORKSPACE",
@@ -161,6 +163,7 @@ def version() -> str:
 
 
 FP8_PAGE_BYTES = 41216  # KAIROS_FP8_PAGE_BYTES
+STATIC_MAX_DECODES = 128  # KAIROS_STATIC_MAX_DECODES
 
 
 def workspace_bytes(max_decodes: int, max_chunk: int) -> int:
@@ -294,6 +297,14 @@ class Kairos:
         _check(_lib.kairos_fp8_decode(self._h, B, _dp(q_dec), _dp(dec_page_tables), int(dec_page_tables.shape[1]) if B else 1,
                                       lens.ctypes.data_as(_vp), _dp(out_dec), _dp(lse_dec), _stream_ptr(stream)))
         return out_dec, lse_dec
+
+    def decode_static(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], out_dec, lse_dec=None, stream=None) -> None:
+        """kairos_decode_static: decode attention with no allocation (scratch is a fixed device array of the library; at most
+        STATIC_MAX_DECODES requests; calls that overlap on the GPU race).  The caller passes the output tensors."""
+        lens = np.ascontiguousarray(np.asarray(dec_ctx_lens, dtype=np.int32))
+        B = int(lens.shape[0])
+        _check(_lib.kairos_decode_static(self._h, B, _dp(q_dec), _dp(dec_page_tables), int(dec_page_tables.shape[1]) if B else 1,
+                                         lens.ctypes.data_as(_vp), _dp(out_dec), _dp(lse_dec), _stream_ptr(stream)))
 
     def tune_step(self, q_dec, dec_page_tables, dec_ctx_lens: Sequence[int], q_chunk, chunk_page_table, chunk_len: int,
                   prefix_len: int, out_dec, out_chunk, reps: int = 5, stream=None):
