@@ -274,11 +274,24 @@ class Point:
         self.torch.cuda.synchronize()
         self.info = self.reps[0].ctx.last_plan_info()
 
-    def timed(self, n_steps, barrier, profile=False):
-        """(device ms over n_steps, host seconds spent issuing them, summed attention-bracket us, brackets)."""
+    def timed(self, n_steps, barrier, profile=False, settle=0.0):
+        """(device ms over n_steps, host seconds spent issuing them, summed attention-bracket us, brackets).
+        settle > 0: the region starts from the state the first region of a point starts from -- that many seconds of idle, then
+        three untimed steps.  Under its power cap this chip drops its clocks ~7 % after ~70 ms of back-to-back tensor-bound
+        steps (measured: two 20-step regions of configs[4] in a row give 3.66 and 3.92 ms/step, whichever runs second), so a
+        region that follows another one without a pause is not comparable with it."""
         torch = self.torch
         for R in self.reps:
             R.ctx.profile_enable(profile)
+        if settle > 0:
+            barrier()
+            time.sleep(settle)
+            for i in range(3):
+                self.step(self.reps[i % self.replicas])
+            if profile:
+                barrier()
+                for R in self.reps:
+                    R.ctx.profile_read()  # drop the brackets of the untimed steps
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         t0 = time.perf_counter()
@@ -432,8 +445,10 @@ def main():
     sampler.start()
     ms_head, host_head, _, _ = pt.timed(args.steps, barrier)
     # roofline leg: the same K steps again with the attention kernels bracketed by CUDA events on their stream
-    ms_prof, _, kern_us, kern_n = pt.timed(args.steps, barrier, profile=True)
+    ms_prof, _, kern_us, kern_n = pt.timed(args.steps, barrier, profile=True, settle=1.0)
     clocks = sampler.stop()
+    # the same step issued back to back for 5x as long, with no pause before it: what a long serving loop sees under the power cap
+    ms_sus, _, _, _ = pt.timed(5 * args.steps, barrier)
 
 
     # ---- the other gated workloads (rank 0's own GPU, N = 1 only): same protocol, their own step counts
@@ -448,7 +463,7 @@ def main():
             ms, _, _, _ = sp.timed(10, barrier)  # sizes the timed region: at least K steps and about 30 ms
             n = int(min(max(args.steps, 30e3 / max(ms * 1e3 / 10, 1.0)), 400))
             ms, host_s, _, _ = sp.timed(n, barrier)
-            _, _, k_us, k_n = sp.timed(n, barrier, profile=True)
+            _, _, k_us, k_n = sp.timed(n, barrier, profile=True, settle=0.5)
             us, kern = ms * 1e3 / n, k_us / max(k_n, 1)
             e = {"workload": point_key(ci, cc), "B": sp.inp.n_dec, "C": sp.inp.chunk_len, "P": sp.inp.prefix_len,
                  "step_us": us, "kernel_us": kern, "host_enqueue_us": host_s * 1e6 / n, "steps": n, "l2": sp.l2,
@@ -544,6 +559,9 @@ def main():
                    "plan": info, "library": K.version()},
         "clocks": clocks,
         "host_enqueue_us": host_head * 1e6 / args.steps,
+        "sustained": {"us_per_step": ms_sus * 1e3 / (5 * args.steps), "steps": 5 * args.steps,
+                      "note": "back to back behind the two timed regions, no pause: the power cap has dropped the clocks by then; "
+                              "the timed regions each start after >= 1 s of idle + 3 untimed steps"},
         "e2e": e2e,
         "gpu_launches": int(args.steps * info["kernels"]),  # the bound step's kernels: append + attention grid(s) + combine
         "roofline": roof,
