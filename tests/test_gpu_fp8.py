@@ -260,3 +260,23 @@ def test_mixed_step_over_the_fp8_cache(lens, C, P):
     if inp.n_dec:
         ref_d, ref_ld = F.decode(r.pool8_ref, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.softmax_scale)
         _assert_close(W.bf16_bits_to_f32(first[0]), first[2], ref_d, ref_ld, f"decode rows beside C={C}")
+
+
+def test_mixed_step_config3_C512_in_the_bench_configuration():
+    """BASELINE.json configs[3] with C = 512 over the fp8 cache, as bench.py's fp8 leg times it: every chunk row and 8 sampled decodes"""
+    inp = W.make_config(3, chunk_len=512)
+    idx = sorted(set([0, 255] + np.random.default_rng(9).choice(256, 6, replace=False).tolist()))
+    r = Fp8Run(inp, oracle_requests=idx)
+    cpt, rows_pt, rows_len = _mixed_case(inp, r)
+    ws = r.torch.empty(r.K.workspace_bytes(inp.n_dec + inp.chunk_len, 0), dtype=r.torch.uint8, device="cuda")
+    ctx = r.K.Kairos(r.pool16, ws, inp.softmax_scale)
+    ctx.fp8_attach(r.pool8)
+    od, oc, ld, lc = ctx.fp8_mixed_step(r.q_dec, r.dec_pt, inp.dec_ctx_lens, r.K.bf16_tensor(inp.q_chunk), cpt, inp.chunk_len, inp.prefix_len)
+    r.torch.cuda.synchronize()
+    out_d, out_c = W.bf16_bits_to_f32(r.K.bf16_bits(od)), W.bf16_bits_to_f32(r.K.bf16_bits(oc))
+    assert np.isfinite(out_d).all() and np.isfinite(out_c).all()
+    ref_c, ref_lc = F.decode(r.pool8_ref, inp.q_chunk, rows_pt, rows_len, inp.softmax_scale)
+    _assert_close(out_c, lc.cpu().numpy(), ref_c, ref_lc, "configs[3] C=512 chunk rows")
+    ref_d, ref_ld = r.reference()
+    _assert_close(out_d[idx], ld.cpu().numpy()[idx], ref_d, ref_ld, "configs[3] C=512 sampled decodes")
+    assert ctx.last_plan_info()["work_items"] >= 256 + 512
