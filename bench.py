@@ -504,7 +504,8 @@ def main():
         e2e_s = time.perf_counter() - t0
         e2e_us = R_.max_over_ranks(e2e_s, dev) * 1e6 / (e2e_steps * world)
         e2e = {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "api": "kairos_mixed_step_host (pinned host buffers, synchronous)", "steps": e2e_steps}
+               "api": "kairos_mixed_step_host (pinned host buffers, synchronous; a large chunk runs in slices whose copies overlap the attention)",
+               "steps": e2e_steps}
 
     if rank != 0:
         if world > 1:

@@ -152,6 +152,12 @@ int kairos_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
  * synchronises the stream before returning.  All pointers are HOST pointers with the shapes of
  * kairos_mixed_step / kairos_append_latent; device staging comes from the context (grown on demand).
  * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied each way.
+ * A chunk of at least two rounds of the cluster grid (2 * (SMs / 2) * 8 tokens, 1184 on a B200) is cut into at most 7
+ * slices of whole rounds that run as successive mixed steps over a growing prefix (the same tiles over the same keys:
+ * chunk invariance; the whole chunk is appended first, the decodes ride with the first slice), with the next
+ * slice's queries copied up and the previous slice's outputs copied down on two streams of the context beside the
+ * attention on `cuda_stream`: the PCIe copies (34.8 KB per chunk token) overlap the step instead of bracketing it.
+ * Host buffers should be pinned for that overlap (pageable memory works, without it).  Nothing is left in flight on return.
  */
 int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const int32_t* dec_page_tables,
                            int32_t dec_table_stride, const int32_t* dec_ctx_lens, int32_t chunk_len,
@@ -513,6 +519,7 @@ int kairos_decode_static(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, cons
  *   "copy_stream" 0 = plan copies on the caller's stream; 1 default (the context's copy stream)
  *   "graph"       0 = never replay a plan as a CUDA graph; 1 default
  *   "plan_cache"  0 = plan every step; 1 default
+ *   "host_slice_tokens"  kairos_mixed_step_host: n > 0 = slices of n chunk tokens (rounded up to whole 8-token tiles); 0 default (its own rule)
  * Errors: INVALID_ARG for an unknown key.
  */
 int kairos_debug_set(kairos_ctx* ctx, const char* key, int32_t value);

@@ -668,6 +668,9 @@ int kairos_destroy(kairos_ctx* ctx) {
             if (b.last_use) cudaEventDestroy(b.last_use);
         }
     if (ctx->host_stage.dev) cudaFree(ctx->host_stage.dev);
+    for (auto e : ctx->host_stage.events) cudaEventDestroy(e);
+    if (ctx->host_stage.in) cudaStreamDestroy(ctx->host_stage.in);
+    if (ctx->host_stage.out) cudaStreamDestroy(ctx->host_stage.out);
     if (ctx->schedule.exec) cudaGraphExecDestroy(ctx->schedule.exec);
     if (ctx->schedule.host) cudaFreeHost(ctx->schedule.host);
     if (ctx->schedule.dev) cudaFree(ctx->schedule.dev);
@@ -764,6 +767,7 @@ int kairos_debug_set(kairos_ctx* ctx, const char* key, int32_t value) {
     else if (k == "copy_stream") ctx->use_copy_stream = value != 0;
     else if (k == "graph") ctx->use_graph = value != 0;
     else if (k == "plan_cache") ctx->use_plan_cache = value != 0;
+    else if (k == "host_slice_tokens") ctx->host_slice_tokens = value;
     else return fail(KAIROS_ERR_INVALID_ARG, "unknown debug key '" + k + "'");
     return KAIROS_OK;
 }
@@ -950,38 +954,94 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     uint8_t* d_oc = p;  p += b_oc;
     uint8_t* d_ld = p;  p += b_ld;
     uint8_t* d_lc = p;
+    // ---- slices.  A large chunk is cut into slices of whole rounds of the cluster grid (sm_count / 2 tiles of 8 tokens) and
+    // the slices run as successive mixed steps over a growing prefix -- the same tiles over the same keys, so by chunk
+    // invariance the same rows -- while the next slice's queries come up on a second stream and the previous
+    // slice's outputs go down on a third: the copies (34.8 KB per chunk token over PCIe) hide behind the attention instead
+    // of bracketing it.  At most 7 slices, so that their plans stay in the context's cache from call to call.
+    const int32_t tile = pair_tile_tokens();
+    const int32_t round_tokens = (ctx->sm_count / 2) * tile;
+    int32_t slice = chunk_len;
+    if (ctx->host_slice_tokens > 0) slice = (ctx->host_slice_tokens + tile - 1) / tile * tile;
+    else if (chunk_len >= 2 * round_tokens) slice = (chunk_len + 7 * round_tokens - 1) / (7 * round_tokens) * round_tokens;
+    const int32_t n_slices = chunk_len > 0 ? (chunk_len + slice - 1) / slice : 1;
+    HostStage& hs = ctx->host_stage;
+    cudaStream_t s_in = stream, s_out = stream;
+    if (n_slices > 1) {
+        if (!hs.in) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&hs.in, cudaStreamNonBlocking));
+        if (!hs.out) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&hs.out, cudaStreamNonBlocking));
+        while (hs.events.size() < size_t(2 * n_slices)) {
+            cudaEvent_t e;
+            KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            hs.events.push_back(e);
+        }
+        s_in = hs.in;
+        s_out = hs.out;
+    }
     uint64_t h2d = 0, d2h = 0;
     auto up = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
         if (!bytes) return cudaSuccess;
         h2d += bytes;
-        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, stream);
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s_in);
     };
     auto down = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
         if (!bytes || !dst) return cudaSuccess;
         d2h += bytes;
-        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, stream);
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s_out);
     };
-    KAIROS_CUDA_TRY(up(d_qd, q_dec, size_t(n_dec) * kHeads * kDim * 2));
-    KAIROS_CUDA_TRY(up(d_dpt, dec_page_tables, size_t(n_dec) * dec_table_stride * 4));
-    KAIROS_CUDA_TRY(up(d_qc, q_chunk, size_t(chunk_len) * kHeads * kDim * 2));
-    KAIROS_CUDA_TRY(up(d_cpt, chunk_page_table, size_t(chunk_len > 0 ? chunk_table_len : 0) * 4));
-    KAIROS_CUDA_TRY(up(d_lat, chunk_latent, size_t(chunk_len) * kLatent * 2));
-    KAIROS_CUDA_TRY(up(d_rope, chunk_k_rope, size_t(chunk_len) * kRope * 2));
-    if (chunk_len > 0) {
-        if (int rc = kairos_append_latent(ctx, d_lat, d_rope, chunk_len, reinterpret_cast<const int32_t*>(d_cpt),
-                                          chunk_table_len, prefix_len, cuda_stream))
-            return rc;
+    auto run = [&]() -> int {
+        KAIROS_CUDA_TRY(up(d_qd, q_dec, size_t(n_dec) * kHeads * kDim * 2));
+        KAIROS_CUDA_TRY(up(d_dpt, dec_page_tables, size_t(n_dec) * dec_table_stride * 4));
+        KAIROS_CUDA_TRY(up(d_cpt, chunk_page_table, size_t(chunk_len > 0 ? chunk_table_len : 0) * 4));
+        KAIROS_CUDA_TRY(up(d_lat, chunk_latent, size_t(chunk_len) * kLatent * 2));
+        KAIROS_CUDA_TRY(up(d_rope, chunk_k_rope, size_t(chunk_len) * kRope * 2));
+        for (int32_t i = 0; i < n_slices; ++i) {  // every slice's queries, in order, behind the small inputs
+            const int32_t off = i * slice, len = std::min(slice, chunk_len - off);
+            KAIROS_CUDA_TRY(up(d_qc + size_t(off) * kHeads * kDim * 2, static_cast<const uint8_t*>(q_chunk) + size_t(off) * kHeads * kDim * 2,
+                               size_t(len) * kHeads * kDim * 2));
+            if (n_slices > 1) KAIROS_CUDA_TRY(cudaEventRecord(hs.events[2 * i], s_in));
+        }
+        for (int32_t i = 0; i < n_slices; ++i) {
+            const int32_t off = i * slice, len = std::min(slice, chunk_len - off);
+            if (n_slices > 1) KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, hs.events[2 * i], 0));
+            if (i == 0 && chunk_len > 0) {  // the whole chunk is appended once: a slice's rows see no key past their own position
+                if (int rc = kairos_append_latent(ctx, d_lat, d_rope, chunk_len, reinterpret_cast<const int32_t*>(d_cpt),
+                                                  chunk_table_len, prefix_len, cuda_stream))
+                    return rc;
+            }
+            const int32_t nd = i == 0 ? n_dec : 0;  // the decodes ride with the first slice
+            if (int rc = mixed_step_impl(ctx, nd, d_qd, reinterpret_cast<const int32_t*>(d_dpt), dec_table_stride, dec_ctx_lens, len,
+                                         prefix_len + off, d_qc + size_t(off) * kHeads * kDim * 2, reinterpret_cast<const int32_t*>(d_cpt),
+                                         chunk_table_len, d_od, d_oc + size_t(off) * kHeads * kLatent * 2,
+                                         lse_dec ? reinterpret_cast<float*>(d_ld) : nullptr,
+                                         lse_chunk ? reinterpret_cast<float*>(d_lc) + size_t(off) * kHeads : nullptr, stream))
+                return rc;
+            if (n_slices > 1) {
+                KAIROS_CUDA_TRY(cudaEventRecord(hs.events[2 * i + 1], stream));
+                KAIROS_CUDA_TRY(cudaStreamWaitEvent(s_out, hs.events[2 * i + 1], 0));
+            }
+            if (i == 0) {
+                KAIROS_CUDA_TRY(down(out_dec, d_od, size_t(n_dec) * kHeads * kLatent * 2));
+                KAIROS_CUDA_TRY(down(lse_dec, d_ld, size_t(n_dec) * kHeads * 4));
+            }
+            KAIROS_CUDA_TRY(down(out_chunk ? static_cast<uint8_t*>(out_chunk) + size_t(off) * kHeads * kLatent * 2 : nullptr,
+                                 d_oc + size_t(off) * kHeads * kLatent * 2, size_t(len) * kHeads * kLatent * 2));
+            KAIROS_CUDA_TRY(down(lse_chunk ? lse_chunk + size_t(off) * kHeads : nullptr, d_lc + size_t(off) * kHeads * 4,
+                                 size_t(len) * kHeads * 4));
+        }
+        return KAIROS_OK;
+    };
+    const int rc = run();
+    // nothing of this call is left in flight when it returns, whether it succeeded or not (the host buffers are the caller's)
+    cudaError_t e1 = cudaSuccess, e2 = cudaSuccess, e3 = cudaStreamSynchronize(stream);
+    if (n_slices > 1) {
+        e1 = cudaStreamSynchronize(s_in);
+        e2 = cudaStreamSynchronize(s_out);
     }
-    if (int rc = mixed_step_impl(ctx, n_dec, d_qd, reinterpret_cast<const int32_t*>(d_dpt), dec_table_stride,
-                                 dec_ctx_lens, chunk_len, prefix_len, d_qc, reinterpret_cast<const int32_t*>(d_cpt),
-                                 chunk_table_len, d_od, d_oc, lse_dec ? reinterpret_cast<float*>(d_ld) : nullptr,
-                                 lse_chunk ? reinterpret_cast<float*>(d_lc) : nullptr, stream))
-        return rc;
-    KAIROS_CUDA_TRY(down(out_dec, d_od, size_t(n_dec) * kHeads * kLatent * 2));
-    KAIROS_CUDA_TRY(down(out_chunk, d_oc, size_t(chunk_len) * kHeads * kLatent * 2));
-    KAIROS_CUDA_TRY(down(lse_dec, d_ld, size_t(n_dec) * kHeads * 4));
-    KAIROS_CUDA_TRY(down(lse_chunk, d_lc, size_t(chunk_len) * kHeads * 4));
-    KAIROS_CUDA_TRY(cudaStreamSynchronize(stream));
+    if (rc) return rc;
+    KAIROS_CUDA_TRY(e3);
+    KAIROS_CUDA_TRY(e1);
+    KAIROS_CUDA_TRY(e2);
     if (h2d_bytes) *h2d_bytes = h2d;
     if (d2h_bytes) *d2h_bytes = d2h;
     return KAIROS_OK;

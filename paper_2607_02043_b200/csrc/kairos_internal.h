@@ -76,6 +76,8 @@ constexpr size_t kPartialSlotBytes = size_t(kHeads) * kLatent * 4 + size_t(kHead
 struct HostStage {  // device staging for kairos_mixed_step_host
     void* dev = nullptr;
     size_t bytes = 0;
+    cudaStream_t in = nullptr, out = nullptr;  // a sliced step's H2D / D2H copies run here, beside the attention on the caller's stream
+    std::vector<cudaEvent_t> events;           // [2i] slice i's queries are up, [2i + 1] slice i's step is done
 };
 
 struct StepArgs {
@@ -172,6 +174,7 @@ struct kairos_ctx {
     int force_pairs = -1;         // -1 auto, 0 never use the pair kernel, n > 0 decode grid first beside n clusters, -(n + 1) n clusters first
     int force_dec_only = -1;      // 0 = never use the decode-only instantiation
     int use_copy_stream = 1, use_graph = 1, use_plan_cache = 1;
+    int host_slice_tokens = 0;    // kairos_mixed_step_host: 0 = its own rule, n > 0 = slices of n chunk tokens
     std::vector<kairos::TunedShape> tuned;   // filled by kairos_tune_step; consulted when force_pairs == -1
     static constexpr int kPlanEntries = 8;
     kairos::PlanEntry plans[kPlanEntries];

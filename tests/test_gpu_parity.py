@@ -451,6 +451,37 @@ def test_host_buffer_step_matches_oracle_every_row(cfg):
     assert d2h == od.nbytes + oc.nbytes
 
 
+@pytest.mark.parametrize("cfg,slice_tokens", [(1, 136), (1, 8), (2, 0)])
+def test_host_buffer_step_in_slices_matches_oracle_every_row(cfg, slice_tokens):
+    """kairos_mixed_step_host cuts a large chunk into slices that run as successive steps over a growing prefix while the
+    copies of the neighbouring slices run beside them (three streams).  configs[1] with forced slices (ragged last slice;
+    8-token slices = 64 steps, more than the plan cache holds) and configs[2] under the call's own rule (4 slices of whole
+    rounds of the cluster grid): every row against the oracle, the pool bit-exact, the byte counts, twice in a row."""
+    import torch
+    from oracle import oracle
+    inp = W.make_config(cfg)
+    run = Hp.GpuRun(inp)
+    if slice_tokens:
+        run.ctx.debug_set("host_slice_tokens", slice_tokens)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    q_dec, q_chunk, lat, rope = pin(inp.q_dec), pin(inp.q_chunk), pin(inp.chunk_latent), pin(inp.chunk_k_rope)
+    od = torch.zeros((inp.n_dec, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+    oc = torch.zeros((inp.chunk_len, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+    pool_np = Hp.oracle_pool_after_append(inp)
+    rd, rc, _, _ = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
+                                     inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    for rep in range(2):
+        od[:] = 0
+        oc[:] = 0
+        h2d, d2h = run.ctx.mixed_step_host(q_dec, inp.dec_page_tables, inp.dec_ctx_lens, q_chunk, lat, rope,
+                                           inp.chunk_page_table, inp.chunk_len, inp.prefix_len, od, oc)
+        assert np.array_equal(run.pool_bits(), pool_np)
+        Hp.assert_attention_close([W.bf16_bits_to_f32(od), W.bf16_bits_to_f32(oc)], [rd, rc],
+                                  f"configs[{cfg}] through host buffers in slices of {slice_tokens or 'auto'} (call {rep})")
+        assert h2d == inp.q_dec.nbytes + inp.q_chunk.nbytes + inp.dec_page_tables.nbytes + inp.chunk_page_table.nbytes + inp.chunk_latent.nbytes + inp.chunk_k_rope.nbytes
+        assert d2h == od.nbytes + oc.nbytes
+
+
 def test_tuned_launch_order_keeps_parity_and_is_used():
     """kairos_tune_step pins a measured launch order for a shape; later steps of that shape use it (also through
     kairos_run_schedule / Kairos.bind_step) and still match the oracle on every row."""
