@@ -543,6 +543,10 @@ kairos_chunk_pair_kernel(const __grid_constant__ CUtensorMap pool_map_k, const _
             int idx = 0;
             if (rank == 0) {
                 if (lane == 0) {
+                    // Every item comes from the queue, the first one too.  A static first item (cluster i takes item i, as in the
+                    // decode grid) was measured and dropped: in the decode-first launch orders half of the clusters only become
+                    // resident when decode CTAs exit, and the long tiles at the head of the list (longest first) would wait for
+                    // them (configs[1] 48.7 -> 53 us, configs[3] C = 2048 175.6 -> 187 us).
                     idx = atomicAdd(p.counter, 1);
                     if (idx >= p.n_items) idx = -1;
                     mbar_wait_cluster(&sm->item_empty[slot], iph ^ 1);
