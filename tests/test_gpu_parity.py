@@ -451,22 +451,28 @@ def test_host_buffer_step_matches_oracle_every_row(cfg):
     assert d2h == od.nbytes + oc.nbytes
 
 
-@pytest.mark.parametrize("cfg,slice_tokens", [(1, 136), (1, 8), (2, 0)])
-def test_host_buffer_step_in_slices_matches_oracle_every_row(cfg, slice_tokens):
+@pytest.mark.parametrize("cfg,slice_tokens,pinned", [(1, 136, True), (1, 8, True), (1, 200, False), (2, 0, True)])
+def test_host_buffer_step_in_slices_matches_oracle_every_row(cfg, slice_tokens, pinned):
     """kairos_mixed_step_host cuts a large chunk into slices that run as successive steps over a growing prefix while the
     copies of the neighbouring slices run beside them (three streams).  configs[1] with forced slices (ragged last slice;
-    8-token slices = 64 steps, more than the plan cache holds) and configs[2] under the call's own rule (4 slices of whole
-    rounds of the cluster grid): every row against the oracle, the pool bit-exact, the byte counts, twice in a row."""
+    8-token slices = 64 steps, more than the plan cache holds; pageable host buffers) and configs[2] under the call's own
+    rule (4 slices of whole rounds of the cluster grid): every row against the oracle, the pool bit-exact, the byte counts,
+    twice in a row."""
     import torch
     from oracle import oracle
     inp = W.make_config(cfg)
     run = Hp.GpuRun(inp)
     if slice_tokens:
         run.ctx.debug_set("host_slice_tokens", slice_tokens)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    if pinned:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        od = torch.zeros((inp.n_dec, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+        oc = torch.zeros((inp.chunk_len, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
+    else:  # pageable host memory: the copies lose their overlap, the results must not change
+        pin = np.ascontiguousarray
+        od = np.zeros((inp.n_dec, 16, 512), np.uint16)
+        oc = np.zeros((inp.chunk_len, 16, 512), np.uint16)
     q_dec, q_chunk, lat, rope = pin(inp.q_dec), pin(inp.q_chunk), pin(inp.chunk_latent), pin(inp.chunk_k_rope)
-    od = torch.zeros((inp.n_dec, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
-    oc = torch.zeros((inp.chunk_len, 16, 512), dtype=torch.int16).pin_memory().numpy().view(np.uint16)
     pool_np = Hp.oracle_pool_after_append(inp)
     rd, rc, _, _ = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
                                      inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
