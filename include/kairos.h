@@ -154,7 +154,7 @@ int kairos_mixed_step(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, const i
  * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied each way.
  * A chunk of at least two rounds of the cluster grid (2 * (SMs / 2) * 8 tokens, 1184 on a B200) is cut into at most 7
  * slices of whole rounds that run as successive mixed steps over a growing prefix (the same tiles over the same keys:
- * chunk invariance; the whole chunk is appended first, the decodes ride with the first slice), with the next
+ * chunk invariance; the whole chunk is appended first, the decodes run ahead as a step of their own), with the next
  * slice's queries copied up and the previous slice's outputs copied down on two streams of the context beside the
  * attention on `cuda_stream`: the PCIe copies (34.8 KB per chunk token) overlap the step instead of bracketing it.
  * Host buffers should be pinned for that overlap (pageable memory works, without it).  Nothing is left in flight on return.

@@ -958,7 +958,7 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     // the slices run as successive mixed steps over a growing prefix -- the same tiles over the same keys, so by chunk
     // invariance the same rows -- while the next slice's queries come up on a second stream and the previous
     // slice's outputs go down on a third: the copies (34.8 KB per chunk token over PCIe) hide behind the attention instead
-    // of bracketing it.  At most 7 slices, so that their plans stay in the context's cache from call to call.
+    // of bracketing it.  At most 7 slices (+ the decodes' own step), so that their plans stay in the context's cache from call to call.
     const int32_t tile = pair_tile_tokens();
     const int32_t round_tokens = (ctx->sm_count / 2) * tile;
     int32_t slice = chunk_len;
@@ -970,7 +970,7 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
     if (n_slices > 1) {
         if (!hs.in) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&hs.in, cudaStreamNonBlocking));
         if (!hs.out) KAIROS_CUDA_TRY(cudaStreamCreateWithFlags(&hs.out, cudaStreamNonBlocking));
-        while (hs.events.size() < size_t(2 * n_slices)) {
+        while (hs.events.size() < size_t(2 * n_slices + 2)) {
             cudaEvent_t e;
             KAIROS_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
             hs.events.push_back(e);
@@ -989,9 +989,25 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
         d2h += bytes;
         return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s_out);
     };
+    // In a sliced step the decodes run first as a step of their own: they need only q_dec and the page tables (a few hundred
+    // KB), so their attention covers the upload of the first slice's queries.
+    const bool dec_first = n_slices > 1 && n_dec > 0;
     auto run = [&]() -> int {
         KAIROS_CUDA_TRY(up(d_qd, q_dec, size_t(n_dec) * kHeads * kDim * 2));
         KAIROS_CUDA_TRY(up(d_dpt, dec_page_tables, size_t(n_dec) * dec_table_stride * 4));
+        if (dec_first) {
+            cudaEvent_t e_in = hs.events[2 * n_slices], e_done = hs.events[2 * n_slices + 1];
+            KAIROS_CUDA_TRY(cudaEventRecord(e_in, s_in));
+            KAIROS_CUDA_TRY(cudaStreamWaitEvent(stream, e_in, 0));
+            if (int rc = mixed_step_impl(ctx, n_dec, d_qd, reinterpret_cast<const int32_t*>(d_dpt), dec_table_stride, dec_ctx_lens, 0, 0,
+                                         nullptr, nullptr, 0, d_od, nullptr, lse_dec ? reinterpret_cast<float*>(d_ld) : nullptr, nullptr,
+                                         stream))
+                return rc;
+            KAIROS_CUDA_TRY(cudaEventRecord(e_done, stream));
+            KAIROS_CUDA_TRY(cudaStreamWaitEvent(s_out, e_done, 0));
+            KAIROS_CUDA_TRY(down(out_dec, d_od, size_t(n_dec) * kHeads * kLatent * 2));
+            KAIROS_CUDA_TRY(down(lse_dec, d_ld, size_t(n_dec) * kHeads * 4));
+        }
         KAIROS_CUDA_TRY(up(d_cpt, chunk_page_table, size_t(chunk_len > 0 ? chunk_table_len : 0) * 4));
         KAIROS_CUDA_TRY(up(d_lat, chunk_latent, size_t(chunk_len) * kLatent * 2));
         KAIROS_CUDA_TRY(up(d_rope, chunk_k_rope, size_t(chunk_len) * kRope * 2));
@@ -1009,7 +1025,7 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
                                                   chunk_table_len, prefix_len, cuda_stream))
                     return rc;
             }
-            const int32_t nd = i == 0 ? n_dec : 0;  // the decodes ride with the first slice
+            const int32_t nd = (i == 0 && !dec_first) ? n_dec : 0;
             if (int rc = mixed_step_impl(ctx, nd, d_qd, reinterpret_cast<const int32_t*>(d_dpt), dec_table_stride, dec_ctx_lens, len,
                                          prefix_len + off, d_qc + size_t(off) * kHeads * kDim * 2, reinterpret_cast<const int32_t*>(d_cpt),
                                          chunk_table_len, d_od, d_oc + size_t(off) * kHeads * kLatent * 2,
@@ -1020,7 +1036,7 @@ int kairos_mixed_step_host(kairos_ctx* ctx, int32_t n_dec, const void* q_dec, co
                 KAIROS_CUDA_TRY(cudaEventRecord(hs.events[2 * i + 1], stream));
                 KAIROS_CUDA_TRY(cudaStreamWaitEvent(s_out, hs.events[2 * i + 1], 0));
             }
-            if (i == 0) {
+            if (i == 0 && !dec_first) {
                 KAIROS_CUDA_TRY(down(out_dec, d_od, size_t(n_dec) * kHeads * kLatent * 2));
                 KAIROS_CUDA_TRY(down(lse_dec, d_ld, size_t(n_dec) * kHeads * 4));
             }

@@ -176,7 +176,7 @@ struct kairos_ctx {
     int use_copy_stream = 1, use_graph = 1, use_plan_cache = 1;
     int host_slice_tokens = 0;    // kairos_mixed_step_host: 0 = its own rule, n > 0 = slices of n chunk tokens
     std::vector<kairos::TunedShape> tuned;   // filled by kairos_tune_step; consulted when force_pairs == -1
-    static constexpr int kPlanEntries = 8;
+    static constexpr int kPlanEntries = 12;  // a sliced host step alone uses up to 8 (7 slices + the decodes' step)
     kairos::PlanEntry plans[kPlanEntries];
     uint64_t plan_clock = 0;
     kairos::HostStage host_stage;
