@@ -261,14 +261,18 @@ class Point:
     def warm(self, n, tune=True):
         inp = self.inp
         self.tuned = None
-        if tune and inp.chunk_len and inp.n_dec and self.alg_flops <= 1.0e11:
-            # (short steps only: the planner's order is already the best one on the tensor-bound workloads, and a few hundred ms of
-            # candidate runs at full power right before the timed region would only heat the chip)
-            # kairos_tune_step (public API): each context measures the candidate launch orders of its step once and pins the fastest
+        if tune and inp.chunk_len and inp.n_dec and self.alg_flops <= 2.0e12:
+            # kairos_tune_step (public API): each context measures the candidate launch orders of its step once and pins the fastest.
+            # Not on configs[4] (4.4 TFLOP per step: the planner's order is the best one there and the candidate runs take seconds).
             for R in self.reps:
                 R.ctx.append_latent(R.latent, R.k_rope, R.chunk_pt, inp.prefix_len)
                 self.tuned = R.ctx.tune_step(R.q_dec, R.dec_pt, self.lens, R.q_chunk, R.chunk_pt, inp.chunk_len, inp.prefix_len,
                                              R.out_dec, R.out_chunk, reps=5)
+            if self.alg_flops > 1.0e11:
+                # the candidate runs of a tensor-bound step are tens of ms at full power: under the power cap the region that
+                # follows them directly runs 5-15 % slower, so the chip idles for a second before the warm-up
+                self.torch.cuda.synchronize()
+                time.sleep(1.0)
         for i in range(max(n, 3) * self.replicas):  # every copy plans, hits its cache and captures its graph before timing
             self.step(self.reps[i % self.replicas])
         self.torch.cuda.synchronize()
