@@ -90,9 +90,18 @@ void choose_pairs(const int32_t* dec_ctx_lens, int32_t n_dec, int32_t chunk_len,
         } else {
             // decode first only pays when the tiles outnumber the SM pairs at least twice (measured: with fewer tiles the
             // clusters that start late run alone at the end)
+            // t_dec_first is flat in c once the decode CTAs stream below the HBM floor (td * (ctas - 2c) is constant), so the
+            // tie decides: the LARGEST share of clusters whose decode grid still ends within 40 % of the estimate (the decode
+            // CTAs stream at their best rate on few SMs, but short requests and a loaded L2 make them slower than
+            // kDecPageCycles, and a decode grid that outlasts the chunk is the worst order of all).  Measured on a 90-point
+            // (B, K, C, P) grid (profiles/r02_order_sweep.md): the planner's loss against the best forced order went from a
+            // mean of 2.5 % (worst 19-26 %, three points above 10 %) to 1.8 % (worst 8 %).
             for (int32_t c = 1; n_tiles >= ctas && c <= std::min(max_pairs, (ctas - 2) / 2); ++c) {
+                const int64_t td = std::max(dec_pages * kDecPageCycles / (ctas - 2 * c), td_all);
                 const int64_t t = t_dec_first(c);
-                if (best < 0 || t < best) { best = t; best_c = c; best_n = 0; }
+                const bool better = best < 0 || t * 1000 < best * 999;
+                const bool tie = !better && t * 1000 <= best * 1001 && td * 5 <= t * 2;
+                if (better || tie) { best = best < 0 ? t : std::min(best, t); best_c = c; best_n = 0; }
             }
             for (int32_t n = 1; n <= max_pairs; ++n) {
                 const int64_t t = t_pairs_first(n);
