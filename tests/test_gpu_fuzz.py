@@ -66,3 +66,24 @@ def test_random_shapes_every_row(seed):
         assert np.abs(lc - rlc).max() <= Hp.LSE_TOL
     od2, oc2, _, _ = run.step()  # the cached plan (and its graph): the same bits
     assert np.array_equal(od, od2) and np.array_equal(oc, oc2)
+
+
+@pytest.mark.parametrize("seed", list(range(8)))
+def test_random_decode_batches_over_the_fp8_cache(seed):
+    """The fp8 latent cache (kairos_fp8_append / kairos_fp8_decode) on random decode batches: the quantising append bit for
+    bit and every request's attention against oracle/fp8_oracle.py, twice (the second call replays the cached plan)."""
+    from tests.test_gpu_fp8 import Fp8Run, _assert_close
+    rng = np.random.default_rng(2000 + seed)
+    n_dec = int(rng.integers(1, 40))
+    if seed % 2:
+        lens = [int(x) for x in rng.integers(1, 3000, n_dec)]
+    else:
+        lens = [int(x) for x in W.lognormal_contexts(rng, n_dec, median=float(rng.integers(64, 900)), sigma=0.9, lo=1, hi=5000)]
+    inp = W.make_inputs(f"fp8_fuzz{seed}", 6000 + seed, lens, 0, 0, q_scale=float(rng.choice([0.1, 0.3])), extra_pages=int(rng.integers(0, 20)))
+    r = Fp8Run(inp)
+    r.check_pool()
+    ref_out, ref_lse = r.reference()
+    out, lse, _ = r.decode()
+    _assert_close(out, lse, ref_out, ref_lse, f"fp8 fuzz seed {seed}: lens {lens}")
+    out2, lse2, _ = r.decode()
+    assert np.array_equal(out, out2) and np.array_equal(lse, lse2)
