@@ -61,6 +61,19 @@ CASES = [
 ]
 
 
+def _random_case(seed):
+    """A seeded random schedule off the hand-picked ones: 2-6 chunks of 1-600 tokens, 0-11 decodes, any prefix."""
+    rng = np.random.default_rng(300 + seed)
+    B = int(rng.integers(0, 12))
+    lens = [int(v) for v in rng.integers(1, 2000, B)]
+    chunks = [int(v) for v in rng.integers(1, 600, int(rng.integers(2, 7)))]
+    return (f"random{seed}", dict(lens=lens, prompt_len=sum(chunks), prefix=int(rng.integers(0, 700)), chunks=chunks,
+                                  grow=bool(rng.integers(0, 2)) and B > 0))
+
+
+CASES += [_random_case(s) for s in range(4)]
+
+
 @pytest.mark.parametrize("name,kw", CASES, ids=[c[0] for c in CASES])
 @pytest.mark.parametrize("pairs", [None, 0, 2])
 def test_run_schedule_every_row(name, kw, pairs):
