@@ -230,7 +230,13 @@ def _mixed_case(inp, r):
     return cpt, rows_pt, rows_len
 
 
-@pytest.mark.parametrize("lens,C,P", [([64, 128, 200, 256], 64, 128), ([300, 70], 100, 0), ([], 130, 61), ([1000, 2500, 65], 257, 700)])
+def _random_mixed(seed):
+    rng = np.random.default_rng(400 + seed)
+    return ([int(v) for v in rng.integers(1, 1800, int(rng.integers(0, 10)))], int(rng.integers(1, 400)), int(rng.integers(0, 900)))
+
+
+@pytest.mark.parametrize("lens,C,P", [([64, 128, 200, 256], 64, 128), ([300, 70], 100, 0), ([], 130, 61), ([1000, 2500, 65], 257, 700)]
+                         + [_random_mixed(s) for s in range(4)])
 def test_mixed_step_over_the_fp8_cache(lens, C, P):
     """kairos_fp8_mixed_step: decodes + a causal chunk, every row against the float64 definition over the dequantised cache"""
     inp = W.make_inputs("fp8_mixed", 17, lens, C, P)
