@@ -13,7 +13,7 @@ def _bits(rng, shape, scale=1.0):
     return W.f32_to_bf16_bits(np.float32(scale) * rng.standard_normal(shape, dtype=np.float32))
 
 
-@pytest.mark.parametrize("n", [1, 127, 128, 129, 700])
+@pytest.mark.parametrize("n", [1, 127, 128, 129, 700, 3, 255, 257, 1031, 2048])
 def test_projections_every_element(n):
     from oracle import proj_oracle as P
     from paper_2607_02043_b200 import kairos as K
