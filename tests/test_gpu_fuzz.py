@@ -87,3 +87,41 @@ def test_random_decode_batches_over_the_fp8_cache(seed):
     _assert_close(out, lse, ref_out, ref_lse, f"fp8 fuzz seed {seed}: lens {lens}")
     out2, lse2, _ = r.decode()
     assert np.array_equal(out, out2) and np.array_equal(lse, lse2)
+
+
+EXTREMES = [
+    ("one_decode_262144_tokens", dict(lens=[262144], C=0, P=0)),                       # 4096 pages in one request: ~150 splits
+    ("2000_tiny_decodes", dict(lens=[64 + (i * 37) % 70 for i in range(2000)], C=0, P=0)),
+    ("chunk_12345_tokens_alone", dict(lens=[], C=12345, P=0)),                         # 1544 tiles, ragged last tile and page
+    ("chunk_of_9_over_150000_prefix", dict(lens=[100], C=9, P=150000)),                # two tiles of 2344 pages each
+    ("2000_decodes_beside_a_3000_token_chunk", dict(lens=[70 + (i * 13) % 500 for i in range(2000)], C=3000, P=777)),
+]
+
+
+@pytest.mark.parametrize("name,kw", EXTREMES, ids=[e[0] for e in EXTREMES])
+def test_extreme_sizes(name, kw):
+    """The sizes the API does not bound (any lengths the page tables cover): a very long request, thousands of requests, a
+    chunk of a thousand tiles, a tiny chunk over a very long prefix.  Append bit-exact; every decode row and an evenly
+    spaced sample of the chunk rows that always holds the first, the last and the rows either side of every 1000th (the
+    oracle does a row at a time: rows are independent, so parity on them is exact); everything finite."""
+    inp = W.make_inputs(name, 7000 + len(name), kw["lens"], kw["C"], kw["P"], q_scale=0.1)
+    run = Hp.GpuRun(inp)
+    run.append()
+    pool_np = Hp.oracle_pool_after_append(inp)
+    assert np.array_equal(run.pool_bits(), pool_np), "append: pool bytes differ"
+    od, oc, ld, lc = run.step()
+    assert np.isfinite(od).all() and np.isfinite(oc).all()
+    C = inp.chunk_len
+    dec_idx = np.arange(inp.n_dec, dtype=np.int32) if inp.n_dec <= 64 else np.arange(0, inp.n_dec, 31, dtype=np.int32)
+    step = max(1, C // 160)
+    chunk_idx = np.unique(np.concatenate([np.arange(0, C, step), np.array([0, C - 1] if C else [], dtype=np.int64),
+                                          np.array([r + d for r in range(1000, C, 1000) for d in (-1, 0)], dtype=np.int64)])).astype(np.int32)
+    rd, rld, rc, rlc = Hp.oracle_sampled(inp, pool_np, dec_idx, chunk_idx)
+    parts_g, parts_r = [], []
+    if len(dec_idx):
+        parts_g.append(od[dec_idx]); parts_r.append(rd)
+        assert np.abs(ld[dec_idx] - rld).max() <= Hp.LSE_TOL
+    if len(chunk_idx):
+        parts_g.append(oc[chunk_idx]); parts_r.append(rc)
+        assert np.abs(lc[chunk_idx] - rlc).max() <= Hp.LSE_TOL
+    Hp.assert_attention_close(parts_g, parts_r, name)
