@@ -330,8 +330,10 @@ class Kairos:
     def mixed_step_host(self, q_dec: np.ndarray, dec_page_tables: np.ndarray, dec_ctx_lens: np.ndarray,
                         q_chunk: np.ndarray, chunk_latent: np.ndarray, chunk_k_rope: np.ndarray,
                         chunk_page_table: np.ndarray, chunk_len: int, prefix_len: int, out_dec: np.ndarray,
-                        out_chunk: np.ndarray, stream=None):
-        """HOST buffers in, HOST buffers out (numpy uint16 views of bf16; pin them with torch for speed)."""
+                        out_chunk: np.ndarray, stream=None, lse_dec: Optional[np.ndarray] = None,
+                        lse_chunk: Optional[np.ndarray] = None):
+        """HOST buffers in, HOST buffers out (numpy uint16 views of bf16; pin them with torch for speed); lse_* = optional
+        float32 HOST arrays [n_dec, 16] / [chunk_len, 16]."""
         lens = np.ascontiguousarray(dec_ctx_lens, dtype=np.int32)
         B, C = int(lens.shape[0]), int(chunk_len)
         h2d, d2h = _c.c_uint64(0), _c.c_uint64(0)
@@ -342,7 +344,7 @@ class Kairos:
         _check(_lib.kairos_mixed_step_host(self._h, B, hp(q_dec), hp(dec_page_tables), stride, hp(lens), C,
                                            int(prefix_len), hp(q_chunk), hp(chunk_latent), hp(chunk_k_rope),
                                            hp(chunk_page_table), int(chunk_page_table.size) if C else 0, hp(out_dec),
-                                           hp(out_chunk), None, None, _c.byref(h2d), _c.byref(d2h),
+                                           hp(out_chunk), hp(lse_dec), hp(lse_chunk), _c.byref(h2d), _c.byref(d2h),
                                            _stream_ptr(stream)))
         return int(h2d.value), int(d2h.value)
 

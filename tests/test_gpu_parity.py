@@ -474,18 +474,23 @@ def test_host_buffer_step_in_slices_matches_oracle_every_row(cfg, slice_tokens, 
         oc = np.zeros((inp.chunk_len, 16, 512), np.uint16)
     q_dec, q_chunk, lat, rope = pin(inp.q_dec), pin(inp.q_chunk), pin(inp.chunk_latent), pin(inp.chunk_k_rope)
     pool_np = Hp.oracle_pool_after_append(inp)
-    rd, rc, _, _ = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
-                                     inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    rd, rc, rld, rlc = oracle.mixed_step(pool_np, inp.q_dec, inp.dec_page_tables, inp.dec_ctx_lens, inp.chunk_len, inp.prefix_len,
+                                         inp.q_chunk, inp.chunk_page_table, inp.softmax_scale)
+    ld = np.zeros((inp.n_dec, 16), np.float32)
+    lc = np.zeros((inp.chunk_len, 16), np.float32)
     for rep in range(2):
         od[:] = 0
         oc[:] = 0
+        ld[:] = 0
+        lc[:] = 0
         h2d, d2h = run.ctx.mixed_step_host(q_dec, inp.dec_page_tables, inp.dec_ctx_lens, q_chunk, lat, rope,
-                                           inp.chunk_page_table, inp.chunk_len, inp.prefix_len, od, oc)
+                                           inp.chunk_page_table, inp.chunk_len, inp.prefix_len, od, oc, lse_dec=ld, lse_chunk=lc)
         assert np.array_equal(run.pool_bits(), pool_np)
         Hp.assert_attention_close([W.bf16_bits_to_f32(od), W.bf16_bits_to_f32(oc)], [rd, rc],
                                   f"configs[{cfg}] through host buffers in slices of {slice_tokens or 'auto'} (call {rep})")
+        assert np.abs(ld - rld).max() <= Hp.LSE_TOL and np.abs(lc - rlc).max() <= Hp.LSE_TOL  # every slice's lse lands at its own rows
         assert h2d == inp.q_dec.nbytes + inp.q_chunk.nbytes + inp.dec_page_tables.nbytes + inp.chunk_page_table.nbytes + inp.chunk_latent.nbytes + inp.chunk_k_rope.nbytes
-        assert d2h == od.nbytes + oc.nbytes
+        assert d2h == od.nbytes + oc.nbytes + ld.nbytes + lc.nbytes
 
 
 def test_tuned_launch_order_keeps_parity_and_is_used():
